@@ -1,0 +1,154 @@
+/* emm.h -- C ABI of libemm_b200.so: B200-native fictitious-wave-domain 3-D CSEM FDTD.
+ *
+ * The calls follow the paper's statement of the problem (arxiv 2304.00233; citations are
+ * /root/reference/PAPER.md line numbers): a rectilinear non-uniform grid (L402-443, L644-660), a
+ * conductivity model (L662-668, Eq. 26), and a survey of sources, frequencies and receivers
+ * (L622-642, L670-680) for which the library returns the complex frequency-domain Green's
+ * functions at the receivers (Eq. 7; output columns of L688-711).
+ *
+ * Conventions.  SI units; z positive downward (L646-649); arrays are x-fastest, a[k][j][i]
+ * (L514).  Every pointer argument is a HOST pointer unless its name starts with `d_`.  Arrays
+ * passed in are copied before the call returns; output buffers are caller-allocated.  Handles are
+ * opaque and released only by emm_grid_destroy.  All time stepping runs in CUDA kernels on the
+ * device memory and stream bound with emm_bind_device (PyTorch owns both); there is no CPU
+ * fallback: without a bound workspace the run calls return EMM_ECUDA.
+ *
+ * Every function returns 0 on success or a negative EMM_E* code; it never throws, exits or
+ * prints.  emm_last_error() returns a thread-local message for the last failure.
+ */
+#ifndef EMM_H
+#define EMM_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EMM_EINVAL  (-1) /* bad dims, non-monotone coordinates, sigma<=0, rd not in {1,2,3}, source or
+                            receiver outside the interior, bad option                                */
+#define EMM_ENOMEM  (-2) /* host allocation failed or bound workspace too small                      */
+#define EMM_ECUDA   (-3) /* CUDA/cuFFT error, or no device workspace bound                            */
+#define EMM_ENOCONV (-4) /* max_steps reached before convergence (outputs are still written)         */
+#define EMM_ENAN    (-5) /* non-finite field detected by the convergence check                        */
+
+#define EMM_TOP_CPML 0   /* CPML on the top face too (whole-space problems)                           */
+#define EMM_TOP_AIR  1   /* air-water boundary at the first z node (Eq. 17-21)              */
+
+#define EMM_CHECK_CORNERS 0 /* 8 corners of the non-CPML box (L528, Fig. 2)                           */
+#define EMM_CHECK_FACES   1 /* its six faces ("the boundaries of the computing volume", L387)         */
+#define EMM_CHECK_FULL    2 /* whole box (Yang 2021, L528)                                            */
+
+typedef struct emm_grid emm_grid;
+
+typedef struct {
+  int rd;        /* half length of the FD operator, 1..3 => order 2*rd (L200, L684)                    */
+  int nb;        /* CPML cells per face (L305, L686)                                                   */
+  int ne;        /* buffer cells between CPML and interior (L686); <0 => rd+5                          */
+  int top;       /* EMM_TOP_*                                                                          */
+  double f0;     /* omega0 = 2*pi*f0 of the fictitious transform sigma = 2*omega0*eps (L47); <=0 => 1  */
+  double cfl;    /* dt = cfl/eta (Eq. 15-16); <=0 => 0.99                                        */
+  double aux_dx; /* spacing of the auxiliary uniform plane used by the air boundary when x-y is
+                    non-uniform (L288); <=0 => smallest horizontal spacing                             */
+} emm_grid_opts;
+
+typedef struct {
+  double pos[3]; /* x,y,z of the point dipole (anywhere inside the model, L640)                        */
+  double dir[3]; /* polarisation of the electric current J (normalised internally)                     */
+} emm_src;
+
+typedef struct {
+  int max_steps;   /* cap on time steps; <=0 => 100000                                                 */
+  int fixed_steps; /* >0: run exactly this many steps and skip the convergence stop                    */
+  double tol;      /* relative change of the lowest-frequency accumulators over check_every steps
+                      below which the run stops (L385-387); <=0 => 1e-6                                 */
+  int check_every; /* <=0 => 100 (L458)                                                                */
+  int check_set;   /* EMM_CHECK_*                                                                      */
+  double fmax;     /* source wavelet parameter; <=0 => 4*sqrt(max f * f0)                              */
+  int batched;     /* 1: advance all sources in one launch per kernel (they share grid and
+                      coefficients); 0: one source after the other                                     */
+} emm_run_opts;
+
+/* integer grid facts for emm_grid_info(): */
+enum { EMM_I_N1 = 0, EMM_I_N2, EMM_I_N3,          /* padded array dims n?pad (L305-312)                  */
+       EMM_I_LO1, EMM_I_LO2, EMM_I_LO3,           /* padding cells on the low side of each axis          */
+       EMM_I_K0,                                  /* z index of the air-water plane, -1 without          */
+       EMM_I_UNIFORM_XY,
+       EMM_I_BOX_LO1, EMM_I_BOX_LO2, EMM_I_BOX_LO3, /* DTFT box = padded grid minus CPML (L365-370)     */
+       EMM_I_BOX_HI1, EMM_I_BOX_HI2, EMM_I_BOX_HI3, /* inclusive                                         */
+       EMM_I_AUX_M1, EMM_I_AUX_M2,                /* FFT plane of the air boundary                       */
+       EMM_I_PITCH,                               /* floats per x row in device memory                   */
+       EMM_I_COUNT };
+
+/* items for emm_get(): state of the run in progress / last finished run */
+enum { EMM_GET_E1 = 0, EMM_GET_E2, EMM_GET_E3, EMM_GET_H1, EMM_GET_H2, EMM_GET_H3,
+                                   /* float [N3][N2][N1]: time-domain fields after the last step        */
+       EMM_GET_F_E1 = 10, EMM_GET_F_E2, EMM_GET_F_E3, EMM_GET_F_H1, EMM_GET_F_H2, EMM_GET_F_H3,
+                                   /* float complex [N3][N2][N1] (re,im pairs): DTFT accumulator of
+                                      frequency `ifreq` (Eq. 25), zero outside the DTFT box              */
+       EMM_GET_CE1 = 20, EMM_GET_CE2, EMM_GET_CE3, /* float [N3][N2][N1]: dt/eps of each E component   */
+       EMM_GET_JW = 30,            /* double complex [nfreq]: J'(omega') accumulated so far (Eq. 7)     */
+       EMM_GET_DELTA = 31          /* double [2]: relative change of E and H accumulators at the last
+                                      convergence check                                                  */
+};
+
+/* ---- host-side pieces of the method (also the diagnostic surface) ------------------------------- */
+
+/* Optimal geometric grid, Eq. 27-29 / L402-443: n intervals over length len, first interval dx.
+ * x_out: n+1 node coordinates starting at 0; q_out (may be NULL): the stretching ratio.             */
+int emm_nugrid(int n, double len, double dx, double *x_out, double *q_out);
+
+/* Interpolation (row 0) and first-derivative (row 1) weights of `npts` arbitrary nodes for the
+ * point x0, by Vandermonde inversion (Eq. 9-12).  Either output may be NULL.                */
+int emm_fd_weights(int npts, const double *nodes, double x0, double *w_interp, double *w_deriv);
+
+/* ---- problem set-up --------------------------------------------------------------------------------- */
+
+/* Node coordinates of the model (n?1 = cells+1 values each, strictly increasing).  Builds the padded
+ * grid (L305-312), the per-node D+/D- coefficient tables (Eq. 13-14) and the air-boundary plan.      */
+int emm_grid_create(const double *x, int nx1, const double *y, int ny1, const double *z, int nz1,
+                    const emm_grid_opts *opts, emm_grid **out);
+void emm_grid_destroy(emm_grid *g);
+int emm_grid_info(const emm_grid *g, int *ints /* EMM_I_COUNT */, double *dt /* 0 before emm_model_set */);
+int emm_grid_coords(const emm_grid *g, int axis, double *nodes_out /* padded nodes, n?pad+1 */);
+int emm_grid_fdcoef(const emm_grid *g, int axis, int plus, double *out /* [n?pad][2*rd] */);
+
+/* Device memory and stream (both owned by the caller, e.g. a torch uint8 tensor and the current torch
+ * stream).  emm_workspace_bytes: bytes needed for nsrc simultaneously resident sources, nfreq
+ * frequencies, up to max_steps steps and nrec receivers with check_set <= EMM_CHECK_FACES (0 on error).
+ * The workspace must be 256-byte aligned and stay alive while the grid is used; binding it uploads
+ * the per-grid tables and invalidates any earlier model.                                             */
+size_t emm_workspace_bytes(const emm_grid *g, int nsrc, int nfreq, int max_steps, int nrec);
+int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, void *cuda_stream);
+
+/* Per-cell conductivity [nz][ny][nx] (S/m, finite, >0); sigma_v NULL => isotropic (VTI otherwise, L43).
+ * Does the padding, the effective medium at each E component (Eq. 26), sigma -> fictitious
+ * permittivity (L47), the time step (Eq. 15-16) and uploads dt/eps.  Needs a bound workspace.        */
+int emm_model_set(emm_grid *g, const float *sigma_h, const float *sigma_v);
+
+/* ---- the run (Algorithm 1) ------------------------------------------------------------------ */
+
+/* One call: every source stepped to convergence (or fixed_steps).
+ * out:    double complex [nsrc][nfreq][nrec][6] as (re,im) pairs: Green's functions Ex,Ey,Ez,Hx,Hy,Hz
+ *         per unit dipole moment (Eq. 7); nsteps: [nsrc] steps executed.                             */
+int emm_run(emm_grid *g, const emm_src *src, int nsrc, const double *freqs_hz, int nfreq,
+            const double *rec_xyz, int nrec, const emm_run_opts *opts, double *out, int *nsteps);
+
+/* Split-phase form of the same loop for device-resident stepping: begin uploads the tables and zeroes
+ * the state of all nsrc sources (resident together); steps enqueues n more iterations of lines 9-23
+ * for every unfinished source and returns after the stream has drained; end applies Eq. 7 and
+ * gathers the receivers.  emm_run_enqueue only enqueues (no host sync) and is meant for timing.      */
+int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const double *freqs_hz, int nfreq,
+                  const double *rec_xyz, int nrec, const emm_run_opts *opts);
+int emm_run_steps(emm_grid *g, int n, int *nsteps /* [nsrc] */, int *all_done);
+int emm_run_enqueue(emm_grid *g, int n);
+int emm_run_end(emm_grid *g, double *out, int *nsteps);
+int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_out);
+
+/* number of kernel launches issued by this library since the grid was created (bench evidence) */
+long long emm_launch_count(const emm_grid *g);
+
+const char *emm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

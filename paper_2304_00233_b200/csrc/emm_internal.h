@@ -1,0 +1,122 @@
+// emm_internal.h -- internal types of libemm_b200.so (not part of the ABI; see include/emm.h).
+//
+// Host side keeps everything in double (grid, FD tables, CPML, wavelet, twiddles, Eq. 7); the device
+// holds fp32 fields/accumulators.  Citations are PAPER.md line numbers; [Rn] = DESIGN.md readings.
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <complex>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/emm.h"
+
+namespace emm {
+
+constexpr double kMu0 = 4e-7 * 3.14159265358979323846;
+constexpr double kPi = 3.14159265358979323846;
+constexpr int kMaxR = 3;
+constexpr int kMaxNF = 16;
+
+int fail(int code, const char *fmt, ...);
+
+// Yee lattice of component c (Ex,Ey,Ez,Hx,Hy,Hz) along axis a: 1 = half nodes, 0 = nodes [R2]
+constexpr int kLat[6][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}, {0, 1, 1}, {1, 0, 1}, {1, 1, 0}};
+
+struct Stencil1 { int start; double w[8]; };
+
+// ---- bump allocator over the caller's device workspace (dry-run mode computes sizes only) ----
+struct Arena {
+  char *base = nullptr;
+  size_t cap = 0, off = 0;
+  bool dry = true;
+  bool overflow = false;
+  template <class T> T *take(size_t n) {
+    size_t bytes = (n * sizeof(T) + 255) & ~size_t(255);
+    size_t at = off;
+    off += bytes;
+    if (dry) return nullptr;
+    if (off > cap) { overflow = true; return nullptr; }
+    return reinterpret_cast<T *>(base + at);
+  }
+};
+
+// ---- device-side view handed to the kernels by value ----
+struct DevGrid {
+  int N1, N2, N3, P1;          // padded dims and x pitch (floats)
+  long long PS, VS;            // plane stride P1*N2, volume stride PS*N3
+  int r, nb;
+  int klo;                     // first updated z index (= r)
+  int zslab_lo;                // 1: CPML slab at low z exists (top=CPML)
+  int blo[3], bhi[3];          // DTFT box, inclusive
+  int NZB;                     // bhi[2]-blo[2]+1
+  int XS;                      // x-slab row length (2*nb rounded up to 4)
+  const float *cm[3], *cp[3];  // FD tables [N][2r]
+  const float *am[3], *bm[3], *ap[3], *bp[3];  // CPML tables [2*nb]
+  const float *ce[3];          // dt/eps [N3][N2][P1]
+  float dtmu;                  // dt/mu0
+};
+
+struct DevState {              // per run; arrays carry a leading source dimension
+  float *E[3], *H[3];          // [nsrc][N3][N2][P1]
+  float *psx[2][2];            // [E/H kernel][2]: x-slab psi [nsrc][N3][N2][XS]
+  float *psy[2][2];            // y-slab psi [nsrc][N3][2nb][P1]
+  float *psz[2][2];            // z-slab psi [nsrc][2nb][N2][P1]
+  float2 *F;                   // [nsrc][nf][6][NZB][N2][P1]
+  const float2 *twE, *twH;     // [max_steps][nf]
+  const float *wav;            // [max_steps]
+  int *it;                     // device step counter
+  int *done;                   // [nsrc]
+  int nf, nsrc;
+};
+
+struct DevTables {             // device pointers of the per-grid region
+  float *ce[3], *cm[3], *cp[3];
+  double *xn[3];
+  int *ta_start[2][2], *fa_start[2][2];   // [axis][lattice]: lattice -> aux plane, aux plane -> lattice
+  float *ta_w[2][2], *fa_w[2][2];
+  float *kx, *ky;                          // signed wavenumbers of the FFT plane
+  void *fft_ws[3];
+};
+
+struct Run;
+
+}  // namespace emm
+
+struct emm_grid {
+  // options
+  int r = 1, nb = 0, ne = 0, top = 0;
+  double f0 = 1, w0 = 0, cfl = 0.99, aux_dx = 0;
+  int nc[3] = {0, 0, 0}, N[3] = {0, 0, 0}, lo[3] = {0, 0, 0};
+  std::vector<double> xn[3], xh[3];      // padded nodes [N+1], half nodes [N]
+  std::vector<double> cm[3], cp[3];      // [N][2r]
+  double Dmax[3] = {0, 0, 0};
+  int k0 = -1, klo = 1, uniform_xy = 0;
+  int blo[3] = {0, 0, 0}, bhi[3] = {0, 0, 0};
+  int P1 = 0, XS = 0;
+  // air boundary
+  int M1 = 0, M2 = 0;
+  double dxa = 0, dya = 0;
+  std::vector<emm::Stencil1> toaux[2][2], fromaux[2][2];
+  // model
+  bool have_model = false;
+  std::vector<float> sig_h, sig_v;       // raw per-cell model (kept for sigma_bar at source nodes, v_ref)
+  bool vti = false;
+  double dt = 0, smin = 0;
+  // device
+  void *d_ws = nullptr;
+  size_t ws_bytes = 0;
+  cudaStream_t stream = nullptr;
+  bool bound = false;
+  size_t fixed_bytes = 0;                // arena offset after the per-grid (model) region
+  emm::DevGrid dg{};
+  emm::DevTables T{};                    // per-grid device tables (fixed region of the workspace)
+  cufftHandle plan_fwd = 0, plan_inv_e = 0, plan_inv_h = 0;
+  bool have_plans = false;
+  size_t fft_ws[3] = {0, 0, 0};             // cuFFT work-area bytes: forward, inverse (E), inverse (H)
+  double vref[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // CPML reference speed per face [R5]
+  emm::Run *run = nullptr;
+  long long launches = 0;
+};

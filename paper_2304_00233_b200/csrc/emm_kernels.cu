@@ -1,0 +1,459 @@
+// emm_kernels.cu -- the per-time-step CUDA kernels of libemm_b200.so (sm_100a).
+//
+// One template, k_update<R, NF, IS_H>, is both fused passes of Algorithm 1:
+//   IS_H = 0:  curl H (Eq. 14) + CPML psi (Eq. 22-24) + E += dt/eps * curl (Eq. 8) + DTFT of the new E
+//   IS_H = 1:  DTFT of the old H (Eq. 25) + curl E (Eq. 13) + CPML psi + H -= dt/mu * curl
+// so no curl arrays are written and the DTFT costs no extra field read (the paper's five separate
+// kernels, Fig. 10).  Both curls have the same shape
+//   (D2 A3 - D3 A2,  D3 A1 - D1 A3,  D1 A2 - D2 A1)
+// with A = H and the D- tables, or A = E and the D+ tables whose stencil is shifted by one node.
+//
+// Mapping: a thread owns 4 consecutive x nodes (128-bit loads/stores) of one y row and marches along z
+// over a chunk of planes, keeping the 2R z-neighbour planes of A1 and A2 in a register queue; x and y
+// neighbours come through L1/L2 (rows are 128-byte aligned).  The DTFT accumulators are streamed with
+// evict-first loads/stores: they are the dominant HBM traffic (96*nf of 84+96*nf bytes per node-step).
+#include <cstdio>
+
+#include "emm_kernels.cuh"
+
+namespace emm {
+
+__device__ __forceinline__ float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ __forceinline__ void st4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
+__device__ __forceinline__ float4 ldcs4(const float *p) { return __ldcs(reinterpret_cast<const float4 *>(p)); }
+__device__ __forceinline__ void stcs4(float *p, float4 v) { __stcs(reinterpret_cast<float4 *>(p), v); }
+__device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
+__device__ __forceinline__ float4 fma4(float a, float4 b, float4 c) {
+  return make_float4(fmaf(a, b.x, c.x), fmaf(a, b.y, c.y), fmaf(a, b.z, c.z), fmaf(a, b.w, c.w));
+}
+__device__ __forceinline__ float4 sub4(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
+__device__ __forceinline__ float4 add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+
+// slab index along an axis of length N (L317-333): low slab i < nb -> i, high slab -> nb + (N-1-i)
+__device__ __forceinline__ int slab_of(int i, int N, int nb, int has_lo) {
+  if (i < nb) return has_lo ? i : -1;
+  if (i > N - 1 - nb) return nb + (N - 1 - i);
+  return -1;
+}
+
+// x derivative of 4 nodes from a 12-wide window w[] holding nodes i0-4 .. i0+7; tap m of node n sits at
+// i0+n-R+XO+m, i.e. window slot 4+n-R+XO+m.
+template <int R, int XO>
+__device__ __forceinline__ float4 ddx(const float (&w)[12], const float (&cx)[4][2 * R]) {
+  float d[4];
+#pragma unroll
+  for (int n = 0; n < 4; ++n) {
+    float acc = 0.f;
+#pragma unroll
+    for (int m = 0; m < 2 * R; ++m) acc = fmaf(cx[n][m], w[4 + n - R + XO + m], acc);
+    d[n] = acc;
+  }
+  return make_float4(d[0], d[1], d[2], d[3]);
+}
+
+__device__ __forceinline__ void window(float (&w)[12], float4 l, float4 c, float4 r) {
+  w[0] = l.x; w[1] = l.y; w[2] = l.z; w[3] = l.w;
+  w[4] = c.x; w[5] = c.y; w[6] = c.z; w[7] = c.w;
+  w[8] = r.x; w[9] = r.y; w[10] = r.z; w[11] = r.w;
+}
+
+// CPML recursion on a quad: psi <- b psi + a D ; D <- D + psi  (Eq. 22-23 with kappa = 1, L317-333)
+__device__ __forceinline__ void cpml4(float *psi, float a, float b, float4 &D) {
+  float4 p = ld4(psi);
+  p = make_float4(fmaf(b, p.x, a * D.x), fmaf(b, p.y, a * D.y), fmaf(b, p.z, a * D.z), fmaf(b, p.w, a * D.w));
+  st4(psi, p);
+  D = add4(D, p);
+}
+
+// DTFT of 4 nodes of one component into NF accumulators (Eq. 25): F[f] += u * tw[f]
+template <int NF>
+__device__ __forceinline__ void dtft4(float2 *F0, size_t fstride, float4 u, const float2 (&tw)[NF > 0 ? NF : 1]) {
+  float4 a[NF > 0 ? NF : 1][2];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    const float *p = reinterpret_cast<const float *>(F0 + f * fstride);
+    a[f][0] = ldcs4(p);
+    a[f][1] = ldcs4(p + 4);
+  }
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    a[f][0].x = fmaf(u.x, tw[f].x, a[f][0].x); a[f][0].y = fmaf(u.x, tw[f].y, a[f][0].y);
+    a[f][0].z = fmaf(u.y, tw[f].x, a[f][0].z); a[f][0].w = fmaf(u.y, tw[f].y, a[f][0].w);
+    a[f][1].x = fmaf(u.z, tw[f].x, a[f][1].x); a[f][1].y = fmaf(u.z, tw[f].y, a[f][1].y);
+    a[f][1].z = fmaf(u.w, tw[f].x, a[f][1].z); a[f][1].w = fmaf(u.w, tw[f].y, a[f][1].w);
+    float *p = reinterpret_cast<float *>(F0 + f * fstride);
+    stcs4(p, a[f][0]);
+    stcs4(p + 4, a[f][1]);
+  }
+}
+
+// runtime-nf fallback (one frequency at a time)
+__device__ __forceinline__ void dtft4_rt(float2 *F0, size_t fstride, float4 u, const float2 *tw, int nf) {
+  for (int f = 0; f < nf; ++f) {
+    const float2 t = __ldg(tw + f);
+    float *p = reinterpret_cast<float *>(F0 + f * fstride);
+    float4 a0 = ldcs4(p), a1 = ldcs4(p + 4);
+    a0.x = fmaf(u.x, t.x, a0.x); a0.y = fmaf(u.x, t.y, a0.y); a0.z = fmaf(u.y, t.x, a0.z); a0.w = fmaf(u.y, t.y, a0.w);
+    a1.x = fmaf(u.z, t.x, a1.x); a1.y = fmaf(u.z, t.y, a1.y); a1.z = fmaf(u.w, t.x, a1.z); a1.w = fmaf(u.w, t.y, a1.w);
+    stcs4(p, a0);
+    stcs4(p + 4, a1);
+  }
+}
+
+template <int R, int NF, bool IS_H>
+__global__ void __launch_bounds__(128) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks) {
+  constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
+  const int src = blockIdx.z / nchunks, chunk = blockIdx.z - src * nchunks;
+  if (s.done[src]) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  if (i0 >= g.N1 || j < R || j > g.N2 - 1 - R) return;
+  const int kbeg = g.klo + chunk * kc;
+  const int kend = min(kbeg + kc, g.N3 - R);
+  if (kbeg >= kend) return;
+  const int it = *s.it;
+
+  const float *A1 = (IS_H ? s.E[0] : s.H[0]) + (size_t)src * g.VS;
+  const float *A2 = (IS_H ? s.E[1] : s.H[1]) + (size_t)src * g.VS;
+  const float *A3 = (IS_H ? s.E[2] : s.H[2]) + (size_t)src * g.VS;
+  float *U1 = (IS_H ? s.H[0] : s.E[0]) + (size_t)src * g.VS;
+  float *U2 = (IS_H ? s.H[1] : s.E[1]) + (size_t)src * g.VS;
+  float *U3 = (IS_H ? s.H[2] : s.E[2]) + (size_t)src * g.VS;
+  const float *tx = IS_H ? g.cp[0] : g.cm[0];
+  const float *ty = IS_H ? g.cp[1] : g.cm[1];
+  const float *tz = IS_H ? g.cp[2] : g.cm[2];
+
+  float cx[4][2 * R], cy[2 * R];
+#pragma unroll
+  for (int n = 0; n < 4; ++n)
+#pragma unroll
+    for (int m = 0; m < 2 * R; ++m) cx[n][m] = __ldg(tx + (size_t)(i0 + n) * 2 * R + m);
+#pragma unroll
+  for (int m = 0; m < 2 * R; ++m) cy[m] = __ldg(ty + (size_t)j * 2 * R + m);
+
+  // per-node update mask (outermost R layers are never updated, L563)
+  bool upd[4];
+#pragma unroll
+  for (int n = 0; n < 4; ++n) upd[n] = (i0 + n >= R) && (i0 + n <= g.N1 - 1 - R);
+  const bool has_l = i0 >= 4, has_r = i0 + 4 < g.P1;
+
+  // CPML bookkeeping that does not depend on k
+  const int sj = slab_of(j, g.N2, g.nb, 1);
+  const bool xq = (i0 < g.nb) || (i0 + 3 > g.N1 - 1 - g.nb);
+  const float *ta[3] = {IS_H ? g.ap[0] : g.am[0], IS_H ? g.ap[1] : g.am[1], IS_H ? g.ap[2] : g.am[2]};
+  const float *tb[3] = {IS_H ? g.bp[0] : g.bm[0], IS_H ? g.bp[1] : g.bm[1], IS_H ? g.bp[2] : g.bm[2]};
+  float ay = 0.f, by = 0.f;
+  if (sj >= 0) { ay = __ldg(ta[1] + sj); by = __ldg(tb[1] + sj); }
+  const int KI = IS_H ? 1 : 0;
+  float *psx0 = s.psx[KI][0] + (size_t)src * g.N3 * g.N2 * g.XS, *psx1 = s.psx[KI][1] + (size_t)src * g.N3 * g.N2 * g.XS;
+  float *psy0 = s.psy[KI][0] + (size_t)src * g.N3 * 2 * g.nb * g.P1, *psy1 = s.psy[KI][1] + (size_t)src * g.N3 * 2 * g.nb * g.P1;
+  float *psz0 = s.psz[KI][0] + (size_t)src * 2 * g.nb * g.PS, *psz1 = s.psz[KI][1] + (size_t)src * 2 * g.nb * g.PS;
+
+  // DTFT bookkeeping
+  const int nf = s.nf;
+  const bool dft_xy = (nf > 0) && (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);
+  const size_t fstride = (size_t)6 * g.NZB * g.PS;      // float2 elements between frequencies
+  float2 *Fsrc = s.F + (size_t)src * nf * fstride + (size_t)(IS_H ? 3 : 0) * g.NZB * g.PS;
+  const float2 *twp = (IS_H ? s.twH : s.twE) + (size_t)it * nf;
+  float2 tw[NF > 0 ? NF : 1];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) tw[f] = __ldg(twp + f);
+
+  const size_t row = (size_t)j * g.P1 + i0;
+  // z queues of A1, A2: planes k-R+O .. k+R-1+O
+  float4 q1[2 * R], q2[2 * R];
+#pragma unroll
+  for (int m = 1; m < 2 * R; ++m) {
+    const size_t o = (size_t)(kbeg - R + O + m - 1) * g.PS + row;
+    q1[m] = ld4(A1 + o);
+    q2[m] = ld4(A2 + o);
+  }
+
+  for (int k = kbeg; k < kend; ++k) {
+    const size_t c0 = (size_t)k * g.PS + row;
+#pragma unroll
+    for (int m = 0; m < 2 * R - 1; ++m) { q1[m] = q1[m + 1]; q2[m] = q2[m + 1]; }
+    {
+      const size_t o = (size_t)(k + R - 1 + O) * g.PS + row;
+      q1[2 * R - 1] = ld4(A1 + o);
+      q2[2 * R - 1] = ld4(A2 + o);
+    }
+    float cz[2 * R];
+#pragma unroll
+    for (int m = 0; m < 2 * R; ++m) cz[m] = __ldg(tz + (size_t)k * 2 * R + m);
+    const float4 a1c = q1[R - O], a2c = q2[R - O];      // plane k of A1, A2
+    const float4 a3c = ld4(A3 + c0);
+
+    // z derivatives (listing L212-236)
+    float4 D3A1 = zero4(), D3A2 = zero4();
+#pragma unroll
+    for (int m = 0; m < 2 * R; ++m) { D3A1 = fma4(cz[m], q1[m], D3A1); D3A2 = fma4(cz[m], q2[m], D3A2); }
+    // y derivatives: rows j-R+O+m of plane k
+    float4 D2A3 = zero4(), D2A1 = zero4();
+#pragma unroll
+    for (int m = 0; m < 2 * R; ++m) {
+      const int dj = m - R + O;
+      const float4 v3 = dj == 0 ? a3c : ld4(A3 + c0 + (ptrdiff_t)dj * g.P1);
+      const float4 v1 = dj == 0 ? a1c : ld4(A1 + c0 + (ptrdiff_t)dj * g.P1);
+      D2A3 = fma4(cy[m], v3, D2A3);
+      D2A1 = fma4(cy[m], v1, D2A1);
+    }
+    // x derivatives from 12-wide windows
+    float4 D1A3, D1A2;
+    {
+      float w[12];
+      window(w, has_l ? ld4(A3 + c0 - 4) : zero4(), a3c, has_r ? ld4(A3 + c0 + 4) : zero4());
+      D1A3 = ddx<R, O>(w, cx);
+      window(w, has_l ? ld4(A2 + c0 - 4) : zero4(), a2c, has_r ? ld4(A2 + c0 + 4) : zero4());
+      D1A2 = ddx<R, O>(w, cx);
+    }
+
+    // CPML memory variables (only inside the slabs)
+    if (xq) {
+      float d3[4] = {D1A3.x, D1A3.y, D1A3.z, D1A3.w}, d2[4] = {D1A2.x, D1A2.y, D1A2.z, D1A2.w};
+      const size_t pr = ((size_t)k * g.N2 + j) * g.XS;
+#pragma unroll
+      for (int n = 0; n < 4; ++n) {
+        const int si = (i0 + n < g.N1) ? slab_of(i0 + n, g.N1, g.nb, 1) : -1;
+        if (si >= 0) {
+          const float a = __ldg(ta[0] + si), b = __ldg(tb[0] + si);
+          float p = fmaf(b, psx0[pr + si], a * d3[n]); psx0[pr + si] = p; d3[n] += p;
+          p = fmaf(b, psx1[pr + si], a * d2[n]); psx1[pr + si] = p; d2[n] += p;
+        }
+      }
+      D1A3 = make_float4(d3[0], d3[1], d3[2], d3[3]);
+      D1A2 = make_float4(d2[0], d2[1], d2[2], d2[3]);
+    }
+    if (sj >= 0) {
+      const size_t po = ((size_t)k * 2 * g.nb + sj) * g.P1 + i0;
+      cpml4(psy0 + po, ay, by, D2A3);
+      cpml4(psy1 + po, ay, by, D2A1);
+    }
+    const int sk = slab_of(k, g.N3, g.nb, g.zslab_lo);
+    if (sk >= 0) {
+      const float a = __ldg(ta[2] + sk), b = __ldg(tb[2] + sk);
+      const size_t po = (size_t)sk * g.PS + row;
+      cpml4(psz0 + po, a, b, D3A2);
+      cpml4(psz1 + po, a, b, D3A1);
+    }
+
+    // curl (L338-346)
+    const float4 c1 = sub4(D2A3, D3A2), c2 = sub4(D3A1, D1A3), c3 = sub4(D1A2, D2A1);
+    float4 u1 = ld4(U1 + c0), u2 = ld4(U2 + c0), u3 = ld4(U3 + c0);
+    const bool dft = dft_xy && k >= g.blo[2] && k <= g.bhi[2];
+    float2 *Fk = Fsrc + (size_t)(k - g.blo[2]) * g.PS + row;
+    const size_t cstride = (size_t)g.NZB * g.PS;
+
+    if (IS_H) {
+      if (dft) {        // old H sits at t = it*dt, the time level of J (Eq. 8; [R6])
+        if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
+        else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
+      }
+      const float m0 = upd[0] ? g.dtmu : 0.f, m1 = upd[1] ? g.dtmu : 0.f, m2 = upd[2] ? g.dtmu : 0.f, m3 = upd[3] ? g.dtmu : 0.f;
+      u1 = make_float4(fmaf(-m0, c1.x, u1.x), fmaf(-m1, c1.y, u1.y), fmaf(-m2, c1.z, u1.z), fmaf(-m3, c1.w, u1.w));
+      u2 = make_float4(fmaf(-m0, c2.x, u2.x), fmaf(-m1, c2.y, u2.y), fmaf(-m2, c2.z, u2.z), fmaf(-m3, c2.w, u2.w));
+      u3 = make_float4(fmaf(-m0, c3.x, u3.x), fmaf(-m1, c3.y, u3.y), fmaf(-m2, c3.z, u3.z), fmaf(-m3, c3.w, u3.w));
+      st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
+    } else {
+      const float4 e1 = ld4(g.ce[0] + c0), e2 = ld4(g.ce[1] + c0), e3 = ld4(g.ce[2] + c0);   // 0 where not updated
+      u1 = make_float4(fmaf(e1.x, c1.x, u1.x), fmaf(e1.y, c1.y, u1.y), fmaf(e1.z, c1.z, u1.z), fmaf(e1.w, c1.w, u1.w));
+      u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
+      u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
+      st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
+      if (dft) {        // new E sits at t = (it+1/2)*dt [R6]
+        if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
+        else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
+      }
+    }
+  }
+}
+
+// ---- source injection: E_c[node] -= s(it*dt) * (dt/eps * W_c)[node]  (Eq. 8, [R7]) ----
+__global__ void k_inject(const DevGrid g, const DevState s, const int *__restrict__ off, const int *__restrict__ idx,
+                         const float *__restrict__ w) {
+  const int src = blockIdx.x;
+  if (s.done[src]) return;
+  const float st = s.wav[*s.it];
+  for (int c = 0; c < 3; ++c) {
+    float *E = s.E[c] + (size_t)src * g.VS;
+    for (int n = off[src * 3 + c] + threadIdx.x; n < off[src * 3 + c + 1]; n += blockDim.x) E[idx[n]] -= st * w[n];
+  }
+}
+
+// ---- check set: separate fp64 accumulators of the lowest frequency, fed by the fp32 fields [R9] ----
+__global__ void k_check_acc(const DevGrid g, const DevState s, const int *__restrict__ cidx, const int nchk,
+                            double2 *__restrict__ C, const double2 *__restrict__ twE, const double2 *__restrict__ twH) {
+  const int src = blockIdx.z, c = blockIdx.y;
+  if (s.done[src]) return;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= nchk) return;
+  const int it = *s.it;
+  const float *fld = (c < 3 ? s.E[c] : s.H[c - 3]) + (size_t)src * g.VS;
+  const double u = (double)fld[cidx[p]];
+  const double2 t = c < 3 ? twE[it] : twH[it];
+  double2 &a = C[((size_t)src * 6 + c) * nchk + p];
+  a.x += u * t.x;
+  a.y += u * t.y;
+}
+
+// relative change since the previous check: warp shuffle + block reduction + one atomic per block
+__global__ void k_check_reduce(const DevState s, const int nchk, const double2 *__restrict__ C, double2 *__restrict__ Cprev,
+                               double *__restrict__ red) {
+  const int src = blockIdx.z, c = blockIdx.y;
+  if (s.done[src]) return;
+  double num = 0.0, den = 0.0;
+  const size_t base = ((size_t)src * 6 + c) * nchk;
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < nchk; p += gridDim.x * blockDim.x) {
+    const double2 a = C[base + p], b = Cprev[base + p];
+    const double dx = a.x - b.x, dy = a.y - b.y;
+    num += dx * dx + dy * dy;
+    den += a.x * a.x + a.y * a.y;
+    Cprev[base + p] = a;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    num += __shfl_xor_sync(0xffffffffu, num, o);
+    den += __shfl_xor_sync(0xffffffffu, den, o);
+  }
+  __shared__ double sn[32], sd[32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) { sn[wid] = num; sd[wid] = den; }
+  __syncthreads();
+  if (wid == 0) {
+    const int nw = (blockDim.x + 31) >> 5;
+    num = lane < nw ? sn[lane] : 0.0;
+    den = lane < nw ? sd[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      num += __shfl_xor_sync(0xffffffffu, num, o);
+      den += __shfl_xor_sync(0xffffffffu, den, o);
+    }
+    if (lane == 0) {
+      atomicAdd(&red[src * 4 + (c / 3) * 2 + 0], num);
+      atomicAdd(&red[src * 4 + (c / 3) * 2 + 1], den);
+    }
+  }
+}
+
+// decision per source; runs before k_step_end of the same step so *it is the index of that step
+__global__ void k_check_final(const DevState s, double *__restrict__ red, double *__restrict__ delta, int *__restrict__ nsteps,
+                              int *__restrict__ status, const int it_min, const double tol, const int stop_enabled) {
+  const int src = blockIdx.x * blockDim.x + threadIdx.x;
+  if (src >= s.nsrc || s.done[src]) return;
+  const int it = *s.it;
+  const double nE = red[src * 4 + 0], dE = red[src * 4 + 1], nH = red[src * 4 + 2], dH = red[src * 4 + 3];
+  red[src * 4 + 0] = red[src * 4 + 1] = red[src * 4 + 2] = red[src * 4 + 3] = 0.0;
+  nsteps[src] = it + 1;
+  if (!isfinite(nE) || !isfinite(dE) || !isfinite(nH) || !isfinite(dH)) {
+    status[src] = EMM_ENAN;
+    s.done[src] = 1;
+    return;
+  }
+  const double qE = dE > 0 ? sqrt(nE / dE) : nan(""), qH = dH > 0 ? sqrt(nH / dH) : nan("");
+  delta[src * 2 + 0] = qE;
+  delta[src * 2 + 1] = qH;
+  if (stop_enabled && it >= it_min && dE > 0 && dH > 0 && qE < tol && qH < tol) s.done[src] = 1;
+}
+
+__global__ void k_step_end(const DevState s) { *s.it += 1; }
+
+// receivers: gather accumulators on the interpolation stencils (Eq. 7 and the weights are applied on the host)
+__global__ void k_gather(const DevGrid g, const DevState s, const int *__restrict__ ridx, float2 *__restrict__ out, const int nn) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  const int c = blockIdx.y % 6, f = blockIdx.y / 6, src = blockIdx.z;
+  if (n >= nn) return;
+  const int t = ridx[(size_t)c * nn + n];              // node index in the padded volume
+  const int k = t / (int)g.PS, rem = t - k * (int)g.PS;
+  const float2 *F = s.F + ((((size_t)src * s.nf + f) * 6 + c) * g.NZB + (k - g.blo[2])) * g.PS + rem;
+  out[(((size_t)src * s.nf + f) * 6 + c) * nn + n] = *F;
+}
+
+// ---------------------------------------------------------------------------------------------------
+#define EMM_LAUNCH_CHECK(g, what)                                                      \
+  do {                                                                                 \
+    cudaError_t e_ = cudaGetLastError();                                               \
+    if (e_ != cudaSuccess) return fail(EMM_ECUDA, "%s: %s", what, cudaGetErrorString(e_)); \
+    (g)->launches++;                                                                   \
+  } while (0)
+
+template <int R, bool IS_H>
+static void launch_update_nf(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks) {
+  switch (s.nf) {
+    case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 1: k_update<R, 1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 2: k_update<R, 2, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 3: k_update<R, 3, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 4: k_update<R, 4, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 5: k_update<R, 5, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+  }
+}
+
+int launch_update(emm_grid *g, const DevState &s, int is_h) {
+  const DevGrid &dg = g->dg;
+  const int quads = dg.P1 / 4;
+  // block: TX quads wide (64 or 128 nodes), 128 threads; pick the width that wastes fewer lanes
+  int TX = 16;
+  if (((quads + 31) / 32) * 32 <= ((quads + 15) / 16) * 16) TX = 32;
+  if (quads <= 8) TX = 8;
+  const int TY = 128 / TX;
+  const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
+  int kc = 16;
+  const int nchunks = (nk + kc - 1) / kc;
+  dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
+  if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
+  cudaStream_t st = g->stream;
+  if (is_h) {
+    if (dg.r == 1) launch_update_nf<1, true>(dg, s, grid, block, st, kc, nchunks);
+    else if (dg.r == 2) launch_update_nf<2, true>(dg, s, grid, block, st, kc, nchunks);
+    else launch_update_nf<3, true>(dg, s, grid, block, st, kc, nchunks);
+  } else {
+    if (dg.r == 1) launch_update_nf<1, false>(dg, s, grid, block, st, kc, nchunks);
+    else if (dg.r == 2) launch_update_nf<2, false>(dg, s, grid, block, st, kc, nchunks);
+    else launch_update_nf<3, false>(dg, s, grid, block, st, kc, nchunks);
+  }
+  EMM_LAUNCH_CHECK(g, is_h ? "k_update<H>" : "k_update<E>");
+  return 0;
+}
+
+int launch_inject(emm_grid *g, const DevState &s, const DevRun &r) {
+  k_inject<<<s.nsrc, 128, 0, g->stream>>>(g->dg, s, r.src_off, r.src_idx, r.src_w);
+  EMM_LAUNCH_CHECK(g, "k_inject");
+  return 0;
+}
+
+int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r) {
+  if (r.nchk <= 0) return 0;
+  dim3 grid((r.nchk + 255) / 256, 6, s.nsrc);
+  k_check_acc<<<grid, 256, 0, g->stream>>>(g->dg, s, r.chk_idx, r.nchk, r.C, r.twE64, r.twH64);
+  EMM_LAUNCH_CHECK(g, "k_check_acc");
+  return 0;
+}
+
+int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled) {
+  int nb = (r.nchk + 255) / 256;
+  if (nb > 148) nb = 148;
+  if (nb < 1) nb = 1;
+  dim3 grid(nb, 6, s.nsrc);
+  k_check_reduce<<<grid, 256, 0, g->stream>>>(s, r.nchk, r.C, r.Cprev, r.red);
+  EMM_LAUNCH_CHECK(g, "k_check_reduce");
+  k_check_final<<<(s.nsrc + 31) / 32, 32, 0, g->stream>>>(s, r.red, r.delta, r.nsteps, r.status, it_min, tol, stop_enabled);
+  EMM_LAUNCH_CHECK(g, "k_check_final");
+  return 0;
+}
+
+int launch_step_end(emm_grid *g, const DevState &s) {
+  k_step_end<<<1, 1, 0, g->stream>>>(s);
+  EMM_LAUNCH_CHECK(g, "k_step_end");
+  return 0;
+}
+
+int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nn) {
+  if (nn <= 0) return 0;
+  dim3 grid((nn + 127) / 128, 6 * s.nf, s.nsrc);
+  k_gather<<<grid, 128, 0, g->stream>>>(g->dg, s, r.rec_idx, r.rec_val, nn);
+  EMM_LAUNCH_CHECK(g, "k_gather");
+  return 0;
+}
+
+}  // namespace emm

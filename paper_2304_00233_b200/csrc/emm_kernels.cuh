@@ -1,0 +1,43 @@
+// emm_kernels.cuh -- launch wrappers implemented in emm_kernels.cu / emm_air.cu.
+#pragma once
+#include "emm_internal.h"
+
+namespace emm {
+
+// host-visible description of the per-run device buffers that are not in DevState
+struct DevRun {
+  // sources
+  int *src_off = nullptr;      // [nsrc*3+1] offsets into src_idx / src_w (component-major per source)
+  int *src_idx = nullptr;      // node index inside one source's volume
+  float *src_w = nullptr;      // dt/eps * W (c-6)
+  // check set
+  int *chk_idx = nullptr;
+  int nchk = 0;
+  double2 *C = nullptr, *Cprev = nullptr;   // [nsrc][6][nchk]
+  double2 *twE64 = nullptr, *twH64 = nullptr;  // [max_steps] lowest frequency, fp64
+  double *red = nullptr;       // [nsrc][4]
+  double *delta = nullptr;     // [nsrc][2]
+  int *nsteps = nullptr;       // [nsrc]
+  int *status = nullptr;       // [nsrc]
+  // receivers
+  int *rec_idx = nullptr;      // [6][nrec*np^3]
+  float2 *rec_val = nullptr;   // [nsrc][nf][6][nrec*np^3]
+  int nrec_nodes = 0;
+  // air boundary scratch: complex planes [1 + r][M2][M1]
+  float2 *air = nullptr;
+};
+
+// one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
+int launch_update(emm_grid *g, const DevState &s, int is_h);
+int launch_inject(emm_grid *g, const DevState &s, const DevRun &r);
+int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
+int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);
+int launch_step_end(emm_grid *g, const DevState &s);
+int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nrec_nodes);
+// air-water boundary (Eq. 17-21): ghost planes of Ex,Ey (is_h=0) or Hx,Hy (is_h=1)
+int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h);
+// model: effective medium (Eq. 26) -> min sigma (for Eq. 15) and dt/eps
+int launch_sigma_min(emm_grid *g, const float *d_sh, const float *d_sv, double *d_min);
+int launch_make_ce(emm_grid *g, const float *d_sh, const float *d_sv, double scale);
+
+}  // namespace emm

@@ -1,0 +1,693 @@
+// emm_run.cu -- device binding, emm_model_set and the run driver (Algorithm 1).
+// Host code only prepares tables (fp64) and enqueues kernels; no field arithmetic happens on the host.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "emm_kernels.cuh"
+
+namespace emm {
+
+bool make_stencil(const double *S, int n, double t, int p, int lo_ok, int hi_ok, bool clamp, Stencil1 *st);
+
+struct Run {
+  int nsrc = 0, nf = 0, nrec = 0, np = 4;
+  std::vector<double> freqs;
+  std::vector<std::complex<double>> wp;     // omega' (Eq. 4)
+  int fmin = 0;
+  double fmax = 0, beta = 0, t0 = 0, tol = 1e-6;
+  int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
+  int it_min = 0, it_host = 0, table_steps = 0;
+  std::vector<double> wav;                  // s(it*dt) rounded to fp32 (what the device injects)
+  std::vector<Stencil1> rst;                // [nrec][6][3]
+  std::vector<int> nsteps, done, status;
+  DevState ds{};
+  DevRun dr{};
+  int nrec_nodes = 0;
+};
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) return fail(EMM_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));        \
+  } while (0)
+
+static size_t vol(const emm_grid *g) { return (size_t)g->P1 * g->N[1] * g->N[2]; }
+
+// cuFFT plans of the air boundary; their work areas are carved from the caller's workspace
+static int ensure_plans(emm_grid *g) {
+  if (g->top != EMM_TOP_AIR || g->have_plans) return 0;
+  int n[2] = {g->M2, g->M1};
+  cufftHandle *pl[3] = {&g->plan_fwd, &g->plan_inv_e, &g->plan_inv_h};
+  const int batch[3] = {1, g->r - 1, g->r};
+  for (int q = 0; q < 3; ++q) {
+    g->fft_ws[q] = 0;
+    if (batch[q] < 1) continue;
+    if (cufftCreate(pl[q]) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftCreate failed (no CUDA device?)");
+    cufftSetAutoAllocation(*pl[q], 0);
+    if (cufftMakePlanMany(*pl[q], 2, n, nullptr, 1, g->M1 * g->M2, nullptr, 1, g->M1 * g->M2, CUFFT_C2C, batch[q],
+                          &g->fft_ws[q]) != CUFFT_SUCCESS)
+      return fail(EMM_ECUDA, "cufftMakePlanMany failed for a %d x %d plane", g->M2, g->M1);
+  }
+  g->have_plans = true;
+  return 0;
+}
+
+// per-grid region: FD tables, node coordinates, dt/eps, air-boundary tables, cuFFT work areas
+static void layout_fixed(emm_grid *g, Arena &A) {
+  const int r2 = 2 * g->r;
+  for (int a = 0; a < 3; ++a) {
+    const size_t n = (size_t)std::max(g->N[a], a == 0 ? g->P1 : 0) + 4;
+    g->T.cm[a] = A.take<float>(n * r2);
+    g->T.cp[a] = A.take<float>(n * r2);
+    g->T.xn[a] = A.take<double>((size_t)g->N[a] + 1);
+  }
+  for (int c = 0; c < 3; ++c) g->T.ce[c] = A.take<float>(vol(g));
+  if (g->top == EMM_TOP_AIR) {
+    g->T.kx = A.take<float>(g->M1);
+    g->T.ky = A.take<float>(g->M2);
+    if (!g->uniform_xy)
+      for (int a = 0; a < 2; ++a)
+        for (int l = 0; l < 2; ++l) {
+          const int M = a == 0 ? g->M1 : g->M2;
+          g->T.ta_start[a][l] = A.take<int>(M);
+          g->T.ta_w[a][l] = A.take<float>((size_t)4 * M);
+          g->T.fa_start[a][l] = A.take<int>(g->N[a]);
+          g->T.fa_w[a][l] = A.take<float>((size_t)4 * g->N[a]);
+        }
+    for (int q = 0; q < 3; ++q) g->T.fft_ws[q] = A.take<char>(g->fft_ws[q] + 256);
+  }
+}
+
+static size_t chk_count(const emm_grid *g, int check_set) {
+  const size_t n0 = g->bhi[0] - g->blo[0] + 1, n1 = g->bhi[1] - g->blo[1] + 1, n2 = g->bhi[2] - g->blo[2] + 1;
+  if (check_set == EMM_CHECK_CORNERS) return 8;
+  if (check_set == EMM_CHECK_FULL) return n0 * n1 * n2;
+  const size_t i0 = n0 > 2 ? n0 - 2 : 0, i1 = n1 > 2 ? n1 - 2 : 0, i2 = n2 > 2 ? n2 - 2 : 0;
+  return n0 * n1 * n2 - i0 * i1 * i2;
+}
+
+// per-run region
+static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps, int nrec, size_t nchk, DevState &s, DevRun &r) {
+  const size_t V = vol(g), PS = (size_t)g->P1 * g->N[1];
+  const int np = std::max(2 * g->r, 4);
+  const size_t np3 = (size_t)np * np * np;
+  for (int c = 0; c < 3; ++c) { s.E[c] = A.take<float>(V * nsrc); s.H[c] = A.take<float>(V * nsrc); }
+  for (int k = 0; k < 2; ++k)
+    for (int q = 0; q < 2; ++q) {
+      s.psx[k][q] = A.take<float>((size_t)nsrc * g->N[2] * g->N[1] * g->XS);
+      s.psy[k][q] = A.take<float>((size_t)nsrc * g->N[2] * 2 * g->nb * g->P1);
+      s.psz[k][q] = A.take<float>((size_t)nsrc * 2 * g->nb * PS);
+    }
+  const size_t nzb = g->bhi[2] - g->blo[2] + 1;
+  s.F = A.take<float2>((size_t)nsrc * nf * 6 * nzb * PS);
+  s.twE = A.take<float2>((size_t)table_steps * nf);
+  s.twH = A.take<float2>((size_t)table_steps * nf);
+  s.wav = A.take<float>(table_steps);
+  s.it = A.take<int>(1);
+  s.done = A.take<int>(nsrc);
+  s.nf = nf;
+  s.nsrc = nsrc;
+  r.src_off = A.take<int>((size_t)nsrc * 3 + 1);
+  r.src_idx = A.take<int>((size_t)nsrc * 3 * np3);
+  r.src_w = A.take<float>((size_t)nsrc * 3 * np3);
+  r.chk_idx = A.take<int>(nchk);
+  r.nchk = (int)nchk;
+  r.C = A.take<double2>((size_t)nsrc * 6 * nchk);
+  r.Cprev = A.take<double2>((size_t)nsrc * 6 * nchk);
+  r.twE64 = A.take<double2>(table_steps);
+  r.twH64 = A.take<double2>(table_steps);
+  r.red = A.take<double>((size_t)nsrc * 4);
+  r.delta = A.take<double>((size_t)nsrc * 2);
+  r.nsteps = A.take<int>(nsrc);
+  r.status = A.take<int>(nsrc);
+  r.rec_idx = A.take<int>((size_t)6 * nrec * np3);
+  r.rec_val = A.take<float2>((size_t)nsrc * nf * 6 * nrec * np3);
+  if (g->top == EMM_TOP_AIR) r.air = A.take<float2>((size_t)(1 + g->r) * g->M1 * g->M2);
+}
+
+template <class T>
+static int upload(emm_grid *g, T *dst, const std::vector<T> &v) {
+  if (v.empty()) return 0;
+  CU(cudaMemcpyAsync(dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, g->stream));
+  CU(cudaStreamSynchronize(g->stream));    // v may be a temporary (pageable memory)
+  return 0;
+}
+
+static void free_run(emm_grid *g) {
+  delete g->run;
+  g->run = nullptr;
+}
+
+}  // namespace emm
+
+using namespace emm;
+
+extern "C" void emm_grid_destroy(emm_grid *g) {
+  if (!g) return;
+  free_run(g);
+  if (g->have_plans) {
+    if (g->plan_fwd) cufftDestroy(g->plan_fwd);
+    if (g->plan_inv_e) cufftDestroy(g->plan_inv_e);
+    if (g->plan_inv_h) cufftDestroy(g->plan_inv_h);
+  }
+  delete g;
+}
+
+extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, int max_steps, int nrec) {
+  emm_grid *g = const_cast<emm_grid *>(cg);
+  if (!g || nsrc < 1 || nfreq < 0 || nrec < 0) { fail(EMM_EINVAL, "emm_workspace_bytes: bad arguments"); return 0; }
+  if (ensure_plans(g)) return 0;
+  if (max_steps <= 0) max_steps = 100000;
+  const DevTables keep = g->T;       // dry-run layout: the live grid's pointers are restored below
+  Arena A;
+  layout_fixed(g, A);
+  const size_t fixed = A.off;
+  DevState s{};
+  DevRun r{};
+  layout_run(g, A, nsrc, nfreq, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), s, r);
+  g->T = keep;
+  // emm_model_set stages the raw model in the run region: make sure it fits as well
+  const size_t stage = fixed + 2 * ((size_t)g->nc[0] * g->nc[1] * g->nc[2] * sizeof(float) + 256) + 512;
+  return std::max(A.off, stage) + 4096;
+}
+
+extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, void *cuda_stream) {
+  if (!g || !d_workspace) return fail(EMM_EINVAL, "emm_bind_device: null argument");
+  if (reinterpret_cast<uintptr_t>(d_workspace) % 256) return fail(EMM_EINVAL, "emm_bind_device: workspace must be 256-byte aligned");
+  int rc = ensure_plans(g);
+  if (rc) return rc;
+  free_run(g);
+  g->have_model = false;
+  g->d_ws = d_workspace;
+  g->ws_bytes = bytes;
+  g->stream = static_cast<cudaStream_t>(cuda_stream);
+  Arena A;
+  A.base = static_cast<char *>(d_workspace);
+  A.cap = bytes;
+  A.dry = false;
+  layout_fixed(g, A);
+  if (A.overflow) return fail(EMM_ENOMEM, "emm_bind_device: workspace of %zu bytes too small (grid tables need %zu)", bytes, A.off);
+  g->fixed_bytes = A.off;
+  // upload the per-grid tables
+  const int r2 = 2 * g->r;
+  for (int a = 0; a < 3; ++a) {
+    const size_t n = (size_t)std::max(g->N[a], a == 0 ? g->P1 : 0) + 4;
+    std::vector<float> m(n * r2, 0.f), p(n * r2, 0.f);
+    for (size_t t = 0; t < (size_t)g->N[a] * r2; ++t) { m[t] = (float)g->cm[a][t]; p[t] = (float)g->cp[a][t]; }
+    if ((rc = upload(g, g->T.cm[a], m)) || (rc = upload(g, g->T.cp[a], p)) || (rc = upload(g, g->T.xn[a], g->xn[a]))) return rc;
+  }
+  if (g->top == EMM_TOP_AIR) {
+    for (int a = 0; a < 2; ++a) {
+      const int M = a == 0 ? g->M1 : g->M2;
+      const double d = a == 0 ? g->dxa : g->dya;
+      std::vector<float> k(M);
+      for (int n = 0; n < M; ++n) k[n] = (float)(2.0 * kPi * (double)(n <= M / 2 ? n : n - M) / ((double)M * d));
+      if ((rc = upload(g, a == 0 ? g->T.kx : g->T.ky, k))) return rc;
+      if (!g->uniform_xy)
+        for (int l = 0; l < 2; ++l) {
+          std::vector<int> st(M), sf(g->N[a]);
+          std::vector<float> wt((size_t)4 * M), wf((size_t)4 * g->N[a]);
+          for (int m = 0; m < M; ++m) { st[m] = g->toaux[a][l][m].start; for (int q = 0; q < 4; ++q) wt[4 * m + q] = (float)g->toaux[a][l][m].w[q]; }
+          for (int i = 0; i < g->N[a]; ++i) { sf[i] = g->fromaux[a][l][i].start; for (int q = 0; q < 4; ++q) wf[4 * i + q] = (float)g->fromaux[a][l][i].w[q]; }
+          if ((rc = upload(g, g->T.ta_start[a][l], st)) || (rc = upload(g, g->T.ta_w[a][l], wt)) ||
+              (rc = upload(g, g->T.fa_start[a][l], sf)) || (rc = upload(g, g->T.fa_w[a][l], wf))) return rc;
+        }
+    }
+    cufftHandle pl[3] = {g->plan_fwd, g->plan_inv_e, g->plan_inv_h};
+    const int batch[3] = {1, g->r - 1, g->r};
+    for (int q = 0; q < 3; ++q) {
+      if (batch[q] < 1) continue;
+      if (cufftSetStream(pl[q], g->stream) != CUFFT_SUCCESS || cufftSetWorkArea(pl[q], g->T.fft_ws[q]) != CUFFT_SUCCESS)
+        return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
+    }
+  }
+  // device view of the grid (CPML and dt/eps pointers are completed later)
+  DevGrid &d = g->dg;
+  d = DevGrid{};
+  d.N1 = g->N[0]; d.N2 = g->N[1]; d.N3 = g->N[2]; d.P1 = g->P1;
+  d.PS = (long long)g->P1 * g->N[1];
+  d.VS = d.PS * g->N[2];
+  d.r = g->r; d.nb = g->nb; d.klo = g->klo;
+  d.zslab_lo = g->top == EMM_TOP_CPML;
+  for (int a = 0; a < 3; ++a) { d.blo[a] = g->blo[a]; d.bhi[a] = g->bhi[a]; d.cm[a] = g->T.cm[a]; d.cp[a] = g->T.cp[a]; d.ce[a] = g->T.ce[a]; }
+  d.NZB = g->bhi[2] - g->blo[2] + 1;
+  d.XS = g->XS;
+  g->bound = true;
+  return 0;
+}
+
+// Medium (Eq. 26, [R3]) and time step (Eq. 15-16, [R4]); effective medium evaluated on the device.
+extern "C" int emm_model_set(emm_grid *g, const float *sigma_h, const float *sigma_v) {
+  if (!g || !sigma_h) return fail(EMM_EINVAL, "emm_model_set: null argument");
+  if (!g->bound) return fail(EMM_ECUDA, "emm_model_set: no device workspace bound (emm_bind_device)");
+  free_run(g);
+  g->have_model = false;
+  const size_t nc = (size_t)g->nc[0] * g->nc[1] * g->nc[2];
+  for (size_t t = 0; t < nc; ++t) {
+    if (!(sigma_h[t] > 0) || !std::isfinite(sigma_h[t])) return fail(EMM_EINVAL, "emm_model_set: sigma_h must be finite and > 0");
+    if (sigma_v && (!(sigma_v[t] > 0) || !std::isfinite(sigma_v[t]))) return fail(EMM_EINVAL, "emm_model_set: sigma_v must be finite and > 0");
+  }
+  try {
+    g->sig_h.assign(sigma_h, sigma_h + nc);
+    if (sigma_v) g->sig_v.assign(sigma_v, sigma_v + nc); else g->sig_v.clear();
+  } catch (const std::bad_alloc &) { return fail(EMM_ENOMEM, "emm_model_set: out of memory"); }
+  g->vti = sigma_v != nullptr;
+  // stage the raw model behind the fixed region
+  Arena A;
+  A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
+  float *d_sh = A.take<float>(nc);
+  float *d_sv = sigma_v ? A.take<float>(nc) : d_sh;
+  double *d_min = A.take<double>(1);
+  if (A.overflow) return fail(EMM_ENOMEM, "emm_model_set: workspace too small to stage the model");
+  CU(cudaMemcpyAsync(d_sh, sigma_h, nc * sizeof(float), cudaMemcpyHostToDevice, g->stream));
+  if (sigma_v) CU(cudaMemcpyAsync(d_sv, sigma_v, nc * sizeof(float), cudaMemcpyHostToDevice, g->stream));
+  const unsigned long long inf_bits = 0x7ff0000000000000ULL;
+  CU(cudaMemcpyAsync(d_min, &inf_bits, sizeof inf_bits, cudaMemcpyHostToDevice, g->stream));
+  int rc = launch_sigma_min(g, d_sh, d_sv, d_min);
+  if (rc) return rc;
+  double smin = 0;
+  CU(cudaMemcpyAsync(&smin, d_min, sizeof smin, cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
+  if (!(smin > 0) || !std::isfinite(smin)) return fail(EMM_EINVAL, "emm_model_set: non-positive effective conductivity at an updated node");
+  g->smin = smin;
+  const double vmax = 1.0 / std::sqrt(kMu0 * smin / (2 * g->w0));                       // v = 1/sqrt(mu eps), eps = sigma/(2 w0)
+  const double eta = 0.5 * vmax * std::sqrt(g->Dmax[0] * g->Dmax[0] + g->Dmax[1] * g->Dmax[1] + g->Dmax[2] * g->Dmax[2]);
+  g->dt = g->cfl / eta;                                                                  // Eq. 15
+  if ((rc = launch_make_ce(g, d_sh, d_sv, g->dt * 2 * g->w0))) return rc;
+  CU(cudaStreamSynchronize(g->stream));
+  g->dg.dtmu = (float)(g->dt / kMu0);
+  // CPML reference speed per face = fastest padded cell inside the slab [R5]
+  for (int a = 0; a < 3; ++a)
+    for (int side = 0; side < 2; ++side) {
+      int lo = side == 0 ? 0 : g->N[a] - g->nb, hi = side == 0 ? g->nb - 1 : g->N[a] - 1;   // padded cell range
+      int c0 = std::min(std::max(lo - g->lo[a], 0), g->nc[a] - 1), c1 = std::min(std::max(hi - g->lo[a], 0), g->nc[a] - 1);
+      double smn = INFINITY;
+      int b0[3] = {0, 0, 0}, b1[3] = {g->nc[0] - 1, g->nc[1] - 1, g->nc[2] - 1};
+      b0[a] = c0; b1[a] = c1;
+      if (a == 2 && side == 0 && g->top == EMM_TOP_AIR) { g->vref[a][side] = 0; continue; }
+      for (int k = b0[2]; k <= b1[2]; ++k) for (int j = b0[1]; j <= b1[1]; ++j) for (int i = b0[0]; i <= b1[0]; ++i) {
+        const size_t t = (size_t)i + (size_t)g->nc[0] * ((size_t)j + (size_t)g->nc[1] * (size_t)k);
+        double s = g->sig_h[t];
+        if (g->vti) s = std::min(s, (double)g->sig_v[t]);
+        smn = std::min(smn, s);
+      }
+      g->vref[a][side] = 1.0 / std::sqrt(kMu0 * smn / (2 * g->w0));
+    }
+  g->have_model = true;
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------
+namespace emm {
+
+// effective conductivity of E component c at node (i,j,k), same rule as the device pass ([R3])
+static double sigma_bar_host(const emm_grid *g, int c, int i, int j, int k) {
+  auto cell = [&](const std::vector<float> &s, int ii, int jj, int kk) -> double {
+    int ci = ii - g->lo[0], cj = jj - g->lo[1], ck = kk - g->lo[2];
+    if (g->top == EMM_TOP_AIR && ck < 0) return 0.0;
+    ci = std::min(std::max(ci, 0), g->nc[0] - 1);
+    cj = std::min(std::max(cj, 0), g->nc[1] - 1);
+    ck = std::min(std::max(ck, 0), g->nc[2] - 1);
+    return (double)s[(size_t)ci + (size_t)g->nc[0] * ((size_t)cj + (size_t)g->nc[1] * (size_t)ck)];
+  };
+  const std::vector<float> &sh = g->sig_h, &sv = g->vti ? g->sig_v : g->sig_h;
+  const int idx[3] = {i, j, k};
+  const int a1 = (c + 1) % 3, a2 = (c + 2) % 3;        // the two transverse axes
+  double num = 0, den = 0;
+  for (int d1 = -1; d1 <= 0; ++d1)
+    for (int d2 = -1; d2 <= 0; ++d2) {
+      int q[3] = {idx[0], idx[1], idx[2]};
+      q[a1] = std::max(idx[a1] + d1, 0);
+      q[a2] = std::max(idx[a2] + d2, 0);
+      const double w = (g->xn[a1][q[a1] + 1] - g->xn[a1][q[a1]]) * (g->xn[a2][q[a2] + 1] - g->xn[a2][q[a2]]);
+      num += cell(c == 2 ? sv : sh, q[0], q[1], q[2]) * w;
+      den += w;
+    }
+  return num / den;
+}
+
+static double node_width(const emm_grid *g, int a, int half, int i) {
+  return half ? g->xn[a][i + 1] - g->xn[a][i] : g->xh[a][i] - g->xh[a][i - 1];
+}
+
+// CPML coefficients (Eq. 24) with the profile of [R5]; index convention of L324-326
+static void cpml_tables(const emm_grid *g, int a, double fmax, std::vector<float> &am, std::vector<float> &bm,
+                        std::vector<float> &ap, std::vector<float> &bp) {
+  const int N = g->N[a], nb = g->nb;
+  am.assign(2 * nb, 0.f); ap.assign(2 * nb, 0.f); bm.assign(2 * nb, 1.f); bp.assign(2 * nb, 1.f);
+  const double Rc = 1e-3;
+  for (int side = 0; side < 2; ++side) {
+    if (a == 2 && side == 0 && g->top == EMM_TOP_AIR) continue;     // no CPML at the top (L292)
+    const double x_in = side == 0 ? g->xn[a][nb] : g->xn[a][N - 1 - nb];
+    const double L = side == 0 ? g->xn[a][nb] - g->xn[a][0] : g->xn[a][N - 1] - g->xn[a][N - 1 - nb];
+    const double d0 = -3.0 * g->vref[a][side] * std::log(Rc) / (2.0 * L);
+    for (int q = 0; q < nb; ++q) {
+      const int i = side == 0 ? q : N - 1 - q, ii = side == 0 ? q : nb + q;
+      for (int half = 0; half < 2; ++half) {
+        const double p = half ? g->xh[a][i] : g->xn[a][i];
+        const double xi = std::max(side == 0 ? x_in - p : p - x_in, 0.0);
+        const double d = d0 * (xi / L) * (xi / L);
+        const double al = std::max(kPi * (fmax / 2) * (1 - xi / L), 0.0);
+        const double b = std::exp(-(d + al) * g->dt);
+        const double aa = d > 0 ? d / (d + al) * (b - 1) : 0.0;
+        (half ? ap : am)[ii] = (float)aa;
+        (half ? bp : bm)[ii] = (float)b;
+      }
+    }
+  }
+}
+
+static int enqueue_steps(emm_grid *g, int n) {
+  Run *R = g->run;
+  int rc;
+  for (int q = 0; q < n; ++q) {
+    if (R->it_host >= R->table_steps) return fail(EMM_EINVAL, "run: step %d beyond the twiddle table (max_steps)", R->it_host);
+    if ((rc = launch_inject(g, R->ds, R->dr))) return rc;                     // Alg. 1 L477 (before the update: same sum)
+    if ((rc = launch_update(g, R->ds, 0))) return rc;                         // L476-479 + E part of L483
+    if (g->top == EMM_TOP_AIR && (rc = launch_air(g, R->ds, R->dr, 0))) return rc;   // L481
+    if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                  // check-set part of L483
+    if ((rc = launch_update(g, R->ds, 1))) return rc;                         // H part of L483 + L486-489
+    if (g->top == EMM_TOP_AIR && (rc = launch_air(g, R->ds, R->dr, 1))) return rc;   // L491
+    if ((R->it_host + 1) % R->check_every == 0 &&
+        (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
+    if ((rc = launch_step_end(g, R->ds))) return rc;
+    R->it_host++;
+  }
+  return 0;
+}
+
+static int fetch_flags(emm_grid *g) {
+  Run *R = g->run;
+  std::vector<int> dn(R->nsrc), ns(R->nsrc), stt(R->nsrc);
+  CU(cudaMemcpyAsync(dn.data(), R->ds.done, sizeof(int) * R->nsrc, cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaMemcpyAsync(ns.data(), R->dr.nsteps, sizeof(int) * R->nsrc, cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaMemcpyAsync(stt.data(), R->dr.status, sizeof(int) * R->nsrc, cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
+  for (int s = 0; s < R->nsrc; ++s) {
+    if (dn[s] && !R->done[s]) { R->done[s] = 1; R->nsteps[s] = ns[s]; R->status[s] = stt[s]; }
+    if (!R->done[s]) R->nsteps[s] = R->it_host;
+  }
+  return 0;
+}
+
+}  // namespace emm
+
+extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const double *freqs, int nf, const double *rec, int nrec,
+                             const emm_run_opts *o) {
+  if (!g || !src || !freqs || !o || (nrec > 0 && !rec)) return fail(EMM_EINVAL, "emm_run_begin: null argument");
+  if (!g->bound) return fail(EMM_ECUDA, "emm_run_begin: no device workspace bound");
+  if (!g->have_model) return fail(EMM_EINVAL, "emm_run_begin: emm_model_set not called");
+  if (nsrc < 1 || nf < 1 || nrec < 0) return fail(EMM_EINVAL, "emm_run_begin: bad counts");
+  free_run(g);
+  Run *R = new (std::nothrow) Run();
+  if (!R) return fail(EMM_ENOMEM, "emm_run_begin: out of memory");
+  g->run = R;
+  const int r = g->r, nb = g->nb;
+  int rc = 0;
+  try {
+    R->nsrc = nsrc; R->nf = nf; R->nrec = nrec;
+    R->max_steps = o->max_steps > 0 ? o->max_steps : 100000;
+    R->fixed_steps = o->fixed_steps > 0 ? o->fixed_steps : 0;
+    R->tol = o->tol > 0 ? o->tol : 1e-6;
+    R->check_every = o->check_every > 0 ? o->check_every : 100;
+    R->check_set = o->check_set;
+    if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
+    R->table_steps = (R->fixed_steps ? R->fixed_steps : R->max_steps) + 1;
+    double fhi = 0;
+    for (int f = 0; f < nf; ++f) {
+      if (!(freqs[f] > 0) || !std::isfinite(freqs[f])) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: frequencies must be > 0"); }
+      R->freqs.push_back(freqs[f]);
+      R->wp.push_back(std::complex<double>(1.0, 1.0) * std::sqrt(2 * kPi * freqs[f] * g->w0));   // Eq. 4
+      fhi = std::max(fhi, freqs[f]);
+      if (freqs[f] < freqs[R->fmin]) R->fmin = f;
+    }
+    R->fmax = o->fmax > 0 ? o->fmax : 4.0 * std::sqrt(fhi * g->f0);         // [R8]
+    R->beta = kPi * R->fmax * R->fmax;
+    R->t0 = kPi / R->fmax;
+    R->np = std::max(2 * r, 4);
+    const int np = R->np;
+    const size_t np3 = (size_t)np * np * np;
+    R->it_min = 0;
+    while (!((double)R->it_min * g->dt >= 2.0 * R->t0)) R->it_min++;        // [R9]
+    R->nsteps.assign(nsrc, 0); R->done.assign(nsrc, 0); R->status.assign(nsrc, 0);
+
+    // receivers (L167-178, L640)
+    R->rst.resize((size_t)std::max(nrec, 1) * 18);
+    for (int q = 0; q < nrec; ++q) for (int c = 0; c < 6; ++c) for (int a = 0; a < 3; ++a) {
+      const double *S = kLat[c][a] ? g->xh[a].data() : g->xn[a].data();
+      if (!make_stencil(S, g->N[a], rec[3 * q + a], np, a == 2 ? g->klo : r, g->N[a] - 1 - r, false, &R->rst[((size_t)q * 6 + c) * 3 + a])) {
+        free_run(g); return fail(EMM_EINVAL, "emm_run_begin: receiver %d outside the interior", q);
+      }
+      const Stencil1 &st = R->rst[((size_t)q * 6 + c) * 3 + a];
+      if (st.start < g->blo[a] || st.start + np - 1 > g->bhi[a]) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: receiver %d stencil leaves the DFT box", q); }
+    }
+    // check set [R9]
+    std::vector<int> chk;
+    for (int k = g->blo[2]; k <= g->bhi[2]; ++k) for (int j = g->blo[1]; j <= g->bhi[1]; ++j) for (int i = g->blo[0]; i <= g->bhi[0]; ++i) {
+      const bool ei = i == g->blo[0] || i == g->bhi[0], ej = j == g->blo[1] || j == g->bhi[1], ek = k == g->blo[2] || k == g->bhi[2];
+      const bool take = R->check_set == EMM_CHECK_FULL ? true : R->check_set == EMM_CHECK_FACES ? (ei || ej || ek) : (ei && ej && ek);
+      if (take) chk.push_back((int)(((size_t)k * g->N[1] + j) * g->P1 + i));
+    }
+    // workspace layout
+    Arena A;
+    A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
+    layout_run(g, A, nsrc, nf, R->table_steps, nrec, chk.size(), R->ds, R->dr);
+    if (A.overflow) { size_t need = A.off; free_run(g); return fail(EMM_ENOMEM, "emm_run_begin: workspace too small (%zu bytes needed)", need); }
+    // zero the whole run region (fields, psi, accumulators, flags)
+    CU(cudaMemsetAsync(static_cast<char *>(g->d_ws) + g->fixed_bytes, 0, A.off - g->fixed_bytes, g->stream));
+
+    // wavelet and twiddles (fp64 -> fp32), [R6]/[R8]
+    const int T = R->table_steps;
+    std::vector<float> wav(T);
+    std::vector<float2> twE((size_t)T * nf), twH((size_t)T * nf);
+    std::vector<double2> twE64(T), twH64(T);
+    R->wav.resize(T);
+    for (int it = 0; it < T; ++it) {
+      const double t = (double)it * g->dt, u = t - R->t0;
+      wav[it] = (float)(-2.0 * R->beta * u * std::sqrt(R->beta / kPi) * std::exp(-R->beta * u * u));
+      R->wav[it] = (double)wav[it];
+      for (int f = 0; f < nf; ++f) {
+        const std::complex<double> I(0, 1);
+        const std::complex<double> h = std::exp(I * R->wp[f] * t), e = std::exp(I * R->wp[f] * (((double)it + 0.5) * g->dt));
+        twH[(size_t)it * nf + f] = make_float2((float)h.real(), (float)h.imag());
+        twE[(size_t)it * nf + f] = make_float2((float)e.real(), (float)e.imag());
+        if (f == R->fmin) { twH64[it] = make_double2(h.real(), h.imag()); twE64[it] = make_double2(e.real(), e.imag()); }
+      }
+    }
+    if ((rc = upload(g, const_cast<float *>(R->ds.wav), wav)) || (rc = upload(g, const_cast<float2 *>(R->ds.twE), twE)) ||
+        (rc = upload(g, const_cast<float2 *>(R->ds.twH), twH)) || (rc = upload(g, R->dr.twE64, twE64)) ||
+        (rc = upload(g, R->dr.twH64, twH64)) || (rc = upload(g, R->dr.chk_idx, chk))) { free_run(g); return rc; }
+
+    // CPML tables
+    DevGrid &d = g->dg;
+    {
+      Arena B = A;           // continue after the run region
+      for (int a = 0; a < 3; ++a) {
+        std::vector<float> am, bm, ap, bp;
+        cpml_tables(g, a, R->fmax, am, bm, ap, bp);
+        float *dam = B.take<float>(2 * nb), *dbm = B.take<float>(2 * nb), *dap = B.take<float>(2 * nb), *dbp = B.take<float>(2 * nb);
+        if (B.overflow) { free_run(g); return fail(EMM_ENOMEM, "emm_run_begin: workspace too small (CPML tables)"); }
+        if ((rc = upload(g, dam, am)) || (rc = upload(g, dbm, bm)) || (rc = upload(g, dap, ap)) || (rc = upload(g, dbp, bp))) { free_run(g); return rc; }
+        d.am[a] = dam; d.bm[a] = dbm; d.ap[a] = dap; d.bp[a] = dbp;
+      }
+    }
+
+    // sources: W_c = dir_c w_x w_y w_z / V on the component's lattice, premultiplied by dt/eps ([R7])
+    std::vector<int> soff(nsrc * 3 + 1, 0), sidx;
+    std::vector<float> sw;
+    for (int s = 0; s < nsrc; ++s) {
+      const double *dir = src[s].dir, *pos = src[s].pos;
+      const double dn = std::sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
+      if (!(dn > 0) || !std::isfinite(dn)) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: source %d has zero direction", s); }
+      for (int c = 0; c < 3; ++c) {
+        soff[s * 3 + c] = (int)sidx.size();
+        if (dir[c] == 0.0) continue;
+        Stencil1 st[3];
+        for (int a = 0; a < 3; ++a) {
+          const double *S = kLat[c][a] ? g->xh[a].data() : g->xn[a].data();
+          if (pos[a] < g->xn[a][g->lo[a]] || pos[a] > g->xn[a][g->lo[a] + g->nc[a]] ||
+              !make_stencil(S, g->N[a], pos[a], np, a == 2 ? g->klo : r, g->N[a] - 1 - r, false, &st[a])) {
+            free_run(g); return fail(EMM_EINVAL, "emm_run_begin: source %d outside the interior", s);
+          }
+        }
+        for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1) {
+          const int i = st[0].start + c1, j = st[1].start + c2, k = st[2].start + c3;
+          const double V = node_width(g, 0, kLat[c][0], i) * node_width(g, 1, kLat[c][1], j) * node_width(g, 2, kLat[c][2], k);
+          const double W = dir[c] / dn * st[0].w[c1] * st[1].w[c2] * st[2].w[c3] / V;
+          const double ce = g->dt * 2 * g->w0 / sigma_bar_host(g, c, i, j, k);
+          sidx.push_back((int)(((size_t)k * g->N[1] + j) * g->P1 + i));
+          sw.push_back((float)(ce * W));
+        }
+      }
+      soff[s * 3 + 3] = (int)sidx.size();
+    }
+    for (int s = 0; s < nsrc; ++s) for (int c = 0; c < 3; ++c) if (soff[s * 3 + c + 1] < soff[s * 3 + c]) soff[s * 3 + c + 1] = soff[s * 3 + c];
+    (void)np3;
+    if ((rc = upload(g, R->dr.src_off, soff)) || (rc = upload(g, R->dr.src_idx, sidx)) || (rc = upload(g, R->dr.src_w, sw))) { free_run(g); return rc; }
+
+    // receiver gather list
+    std::vector<int> ridx((size_t)6 * nrec * np3);
+    R->nrec_nodes = (int)(nrec * np3);
+    for (int c = 0; c < 6; ++c) for (int q = 0; q < nrec; ++q) {
+      const Stencil1 *st = &R->rst[((size_t)q * 6 + c) * 3];
+      size_t n = 0;
+      for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1)
+        ridx[((size_t)c * nrec + q) * np3 + n++] = (int)(((size_t)(st[2].start + c3) * g->N[1] + st[1].start + c2) * g->P1 + st[0].start + c1);
+    }
+    if ((rc = upload(g, R->dr.rec_idx, ridx))) { free_run(g); return rc; }
+    CU(cudaStreamSynchronize(g->stream));
+  } catch (const std::bad_alloc &) {
+    free_run(g);
+    return fail(EMM_ENOMEM, "emm_run_begin: out of memory");
+  }
+  return 0;
+}
+
+extern "C" int emm_run_enqueue(emm_grid *g, int n) {
+  if (!g || !g->run) return fail(EMM_EINVAL, "emm_run_enqueue: no run in progress");
+  return enqueue_steps(g, n);
+}
+
+extern "C" int emm_run_steps(emm_grid *g, int n, int *nsteps, int *all_done) {
+  if (!g || !g->run) return fail(EMM_EINVAL, "emm_run_steps: no run in progress");
+  Run *R = g->run;
+  int rc = 0, left = n;
+  bool alldone = false, noconv = false;
+  while (left > 0 && !alldone) {
+    int chunk = std::min(left, R->check_every - R->it_host % R->check_every);      // stop at every check
+    if (R->fixed_steps) chunk = std::min(chunk, R->fixed_steps - R->it_host);
+    else chunk = std::min(chunk, R->max_steps - R->it_host);
+    if (chunk > 0) {
+      if ((rc = enqueue_steps(g, chunk))) return rc;
+      left -= chunk;
+    }
+    if ((rc = fetch_flags(g))) return rc;
+    alldone = true;
+    for (int s = 0; s < R->nsrc; ++s) alldone = alldone && R->done[s];
+    if (R->fixed_steps && R->it_host >= R->fixed_steps) { for (int s = 0; s < R->nsrc; ++s) R->done[s] = 1; alldone = true; }
+    if (!R->fixed_steps && R->it_host >= R->max_steps && !alldone) { noconv = true; for (int s = 0; s < R->nsrc; ++s) R->done[s] = 1; alldone = true; }
+    if (chunk <= 0) break;
+  }
+  if (left <= 0 && !alldone) { if ((rc = fetch_flags(g))) return rc; }
+  for (int s = 0; s < R->nsrc; ++s) if (nsteps) nsteps[s] = R->nsteps[s];
+  if (all_done) *all_done = alldone ? 1 : 0;
+  for (int s = 0; s < R->nsrc; ++s) if (R->status[s] == EMM_ENAN) return fail(EMM_ENAN, "emm_run_steps: non-finite field (source %d)", s);
+  if (noconv) return fail(EMM_ENOCONV, "emm_run_steps: max_steps reached before convergence");
+  return 0;
+}
+
+// compute_green_function + extract_emf (Alg. 1): Eq. 7 and receiver interpolation, fp64 on the host
+extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
+  if (!g || !g->run) return fail(EMM_EINVAL, "emm_run_end: no run in progress");
+  Run *R = g->run;
+  int rc;
+  if ((rc = fetch_flags(g))) return rc;
+  for (int s = 0; s < R->nsrc; ++s) if (nsteps) nsteps[s] = R->nsteps[s];
+  if (!out_ || R->nrec == 0) return 0;
+  const int nf = R->nf, np = R->np, nn = R->nrec_nodes;
+  const size_t np3 = (size_t)np * np * np;
+  if ((rc = launch_gather(g, R->ds, R->dr, nn))) return rc;
+  std::vector<float2> val((size_t)R->nsrc * nf * 6 * nn);
+  CU(cudaMemcpyAsync(val.data(), R->dr.rec_val, val.size() * sizeof(float2), cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
+  std::complex<double> *out = reinterpret_cast<std::complex<double> *>(out_);
+  const std::complex<double> I(0, 1);
+  for (int s = 0; s < R->nsrc; ++s)
+    for (int f = 0; f < nf; ++f) {
+      std::complex<double> Jw = 0;                                             // J'(omega') = sum s[it] e^{i w' it dt}
+      for (int it = 0; it < R->nsteps[s]; ++it) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
+      const std::complex<double> sc = std::sqrt(-I * 2.0 * kPi * R->freqs[f] / (2 * g->w0));   // Eq. 7a, principal root
+      for (int q = 0; q < R->nrec; ++q)
+        for (int c = 0; c < 6; ++c) {
+          const Stencil1 *st = &R->rst[((size_t)q * 6 + c) * 3];
+          const float2 *v = &val[(((size_t)s * nf + f) * 6 + c) * nn + (size_t)q * np3];
+          std::complex<double> acc = 0;
+          size_t n = 0;
+          for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1, ++n)
+            acc += st[0].w[c1] * st[1].w[c2] * st[2].w[c3] * std::complex<double>(v[n].x, v[n].y);
+          std::complex<double> G = acc / Jw;                                   // Eq. 7b
+          if (c < 3) G *= sc;
+          out[(((size_t)s * nf + f) * R->nrec + q) * 6 + c] = G;
+        }
+    }
+  return 0;
+}
+
+extern "C" int emm_run(emm_grid *g, const emm_src *src, int nsrc, const double *freqs, int nf, const double *rec, int nrec,
+                       const emm_run_opts *o, double *out, int *nsteps) {
+  if (!g || !src || nsrc < 1 || !o) return fail(EMM_EINVAL, "emm_run: bad arguments");
+  const int group = o->batched ? nsrc : 1;
+  int worst = 0;
+  for (int s0 = 0; s0 < nsrc; s0 += group) {
+    int rc = emm_run_begin(g, src + s0, group, freqs, nf, rec, nrec, o);
+    if (rc) return rc;
+    int done = 0;
+    std::vector<int> ns(group, 0);
+    while (!done) {
+      rc = emm_run_steps(g, g->run->check_every, ns.data(), &done);
+      if (rc == EMM_ENOCONV) { worst = rc; break; }
+      if (rc) return rc;
+    }
+    rc = emm_run_end(g, out ? out + (size_t)s0 * nf * nrec * 12 : nullptr, ns.data());
+    if (rc) return rc;
+    if (nsteps) for (int s = 0; s < group; ++s) nsteps[s0 + s] = ns[s];
+  }
+  if (worst) return fail(worst, "emm_run: max_steps reached before convergence");
+  return 0;
+}
+
+extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_out) {
+  if (!g || !host_out) return fail(EMM_EINVAL, "emm_get: null argument");
+  if (!g->bound) return fail(EMM_ECUDA, "emm_get: no device workspace bound");
+  const int N1 = g->N[0], N2 = g->N[1], N3 = g->N[2], P1 = g->P1;
+  if (what >= EMM_GET_CE1 && what <= EMM_GET_CE3) {
+    if (!g->have_model) return fail(EMM_EINVAL, "emm_get: no model");
+    CU(cudaMemcpy2DAsync(host_out, (size_t)N1 * 4, g->T.ce[what - EMM_GET_CE1], (size_t)P1 * 4, (size_t)N1 * 4, (size_t)N2 * N3,
+                         cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    return 0;
+  }
+  Run *R = g->run;
+  if (!R || isrc < 0 || isrc >= R->nsrc) return fail(EMM_EINVAL, "emm_get: no run state for that source");
+  if (what >= EMM_GET_E1 && what <= EMM_GET_H3) {
+    const float *p = (what < EMM_GET_H1 ? R->ds.E[what] : R->ds.H[what - EMM_GET_H1]) + (size_t)isrc * g->dg.VS;
+    CU(cudaMemcpy2DAsync(host_out, (size_t)N1 * 4, p, (size_t)P1 * 4, (size_t)N1 * 4, (size_t)N2 * N3, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    return 0;
+  }
+  if (what >= EMM_GET_F_E1 && what <= EMM_GET_F_H3) {
+    if (ifreq < 0 || ifreq >= R->nf) return fail(EMM_EINVAL, "emm_get: bad ifreq");
+    const int c = what - EMM_GET_F_E1;
+    float2 *o = static_cast<float2 *>(host_out);
+    std::memset(o, 0, sizeof(float2) * (size_t)N1 * N2 * N3);
+    const float2 *F = R->ds.F + (((size_t)isrc * R->nf + ifreq) * 6 + c) * g->dg.NZB * g->dg.PS;
+    CU(cudaMemcpy2DAsync(o + (size_t)g->blo[2] * N2 * N1, (size_t)N1 * 8, F, (size_t)P1 * 8, (size_t)N1 * 8, (size_t)N2 * g->dg.NZB,
+                         cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    for (int k = g->blo[2]; k <= g->bhi[2]; ++k) for (int j = 0; j < N2; ++j) {
+      float2 *row = o + ((size_t)k * N2 + j) * N1;
+      const bool jin = j >= g->blo[1] && j <= g->bhi[1];
+      for (int i = 0; i < N1; ++i) if (!jin || i < g->blo[0] || i > g->bhi[0]) row[i] = make_float2(0.f, 0.f);
+    }
+    return 0;
+  }
+  if (what == EMM_GET_JW) {
+    int rc = fetch_flags(g);
+    if (rc) return rc;
+    std::complex<double> *o = static_cast<std::complex<double> *>(host_out);
+    const std::complex<double> I(0, 1);
+    for (int f = 0; f < R->nf; ++f) {
+      std::complex<double> Jw = 0;
+      for (int it = 0; it < R->nsteps[isrc]; ++it) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
+      o[f] = Jw;
+    }
+    return 0;
+  }
+  if (what == EMM_GET_DELTA) {
+    CU(cudaMemcpyAsync(host_out, R->dr.delta + 2 * isrc, 2 * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    return 0;
+  }
+  return fail(EMM_EINVAL, "emm_get: unknown item %d", what);
+}

@@ -1,0 +1,293 @@
+"""Thin ctypes binding of libemm_b200.so (include/emm.h): argument marshalling only.
+
+Every step of the method runs in the library's CUDA kernels; PyTorch is used here for device
+memory (the workspace tensor) and the stream, as the ABI asks.  There is no CPU fallback: a
+missing library or a missing CUDA device raises.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libemm_b200.so")
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_air.cu", "emm_run.cu")]
+_HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh")] + \
+       [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
+
+TOP_CPML, TOP_AIR = 0, 1
+CHECK_CORNERS, CHECK_FACES, CHECK_FULL = 0, 1, 2
+EINVAL, ENOMEM, ECUDA, ENOCONV, ENAN = -1, -2, -3, -4, -5
+_GET = {"E1": 0, "E2": 1, "E3": 2, "H1": 3, "H2": 4, "H3": 5,
+        "F_E1": 10, "F_E2": 11, "F_E3": 12, "F_H1": 13, "F_H2": 14, "F_H3": 15,
+        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31}
+_INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "box_lo2", "box_lo3",
+         "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2", "pitch")
+# every symbol include/emm.h declares (tests check that the library exports all of them)
+SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
+           "emm_grid_fdcoef", "emm_workspace_bytes", "emm_bind_device", "emm_model_set", "emm_run", "emm_run_begin",
+           "emm_run_steps", "emm_run_enqueue", "emm_run_end", "emm_get", "emm_launch_count", "emm_last_error")
+
+
+def build(force=False, verbose=False):
+    """nvcc -> libemm_b200.so in-tree, sm_100a only."""
+    deps = _SRC + _HDR
+    if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(os.path.getmtime(p) for p in deps):
+        return _SO
+    cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
+           "-Xcompiler", "-fPIC", "-shared", "-o", _SO] + _SRC + ["-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+    if verbose:
+        cmd.insert(1, "-Xptxas=-v")
+    subprocess.check_call(cmd)
+    return _SO
+
+
+class GridOpts(C.Structure):
+    _fields_ = [("rd", C.c_int), ("nb", C.c_int), ("ne", C.c_int), ("top", C.c_int),
+                ("f0", C.c_double), ("cfl", C.c_double), ("aux_dx", C.c_double)]
+
+
+class Src(C.Structure):
+    _fields_ = [("pos", C.c_double * 3), ("dir", C.c_double * 3)]
+
+
+class RunOpts(C.Structure):
+    _fields_ = [("max_steps", C.c_int), ("fixed_steps", C.c_int), ("tol", C.c_double),
+                ("check_every", C.c_int), ("check_set", C.c_int), ("fmax", C.c_double), ("batched", C.c_int)]
+
+
+class EmmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libemm_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise RuntimeError("libemm_b200.so is not built (run __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(_SO)
+        dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p
+        L.emm_last_error.restype = C.c_char_p
+        L.emm_nugrid.argtypes = [C.c_int, C.c_double, C.c_double, dp, dp]
+        L.emm_fd_weights.argtypes = [C.c_int, dp, C.c_double, dp, dp]
+        L.emm_grid_create.argtypes = [dp, C.c_int, dp, C.c_int, dp, C.c_int, C.POINTER(GridOpts), C.POINTER(vp)]
+        L.emm_grid_destroy.argtypes = [vp]
+        L.emm_grid_destroy.restype = None
+        L.emm_grid_info.argtypes = [vp, ip, dp]
+        L.emm_grid_coords.argtypes = [vp, C.c_int, dp]
+        L.emm_grid_fdcoef.argtypes = [vp, C.c_int, C.c_int, dp]
+        L.emm_workspace_bytes.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.emm_workspace_bytes.restype = C.c_size_t
+        L.emm_bind_device.argtypes = [vp, vp, C.c_size_t, vp]
+        L.emm_model_set.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.emm_run.argtypes = [vp, C.POINTER(Src), C.c_int, dp, C.c_int, dp, C.c_int, C.POINTER(RunOpts), dp, ip]
+        L.emm_run_begin.argtypes = [vp, C.POINTER(Src), C.c_int, dp, C.c_int, dp, C.c_int, C.POINTER(RunOpts)]
+        L.emm_run_steps.argtypes = [vp, C.c_int, ip, ip]
+        L.emm_run_enqueue.argtypes = [vp, C.c_int]
+        L.emm_run_end.argtypes = [vp, dp, ip]
+        L.emm_get.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+        L.emm_launch_count.argtypes = [vp]
+        L.emm_launch_count.restype = C.c_longlong
+        _lib = L
+    return _lib
+
+
+def _chk(rc, allow=()):
+    if rc != 0 and rc not in allow:
+        raise EmmError(rc, lib().emm_last_error().decode())
+    return rc
+
+
+def _dptr(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def emm_nugrid(n, length, dx):
+    x = np.zeros(n + 1)
+    q = C.c_double()
+    _chk(lib().emm_nugrid(n, length, dx, _dptr(x), C.byref(q)))
+    return x, q.value
+
+
+def emm_fd_weights(nodes, x0):
+    nodes = np.ascontiguousarray(nodes, dtype=np.float64)
+    wi, wd = np.zeros(len(nodes)), np.zeros(len(nodes))
+    _chk(lib().emm_fd_weights(len(nodes), _dptr(nodes), x0, _dptr(wi), _dptr(wd)))
+    return wi, wd
+
+
+nugrid, fd_weights = emm_nugrid, emm_fd_weights     # same names as the oracle binding, for shared test helpers
+
+
+def _srcs(sources):
+    arr = (Src * len(sources))()
+    for s, (pos, d) in zip(arr, sources):
+        s.pos[:] = [float(v) for v in pos]
+        s.dir[:] = [float(v) for v in d]
+    return arr
+
+
+def _ropts(o):
+    o = dict(o or {})
+    r = RunOpts(int(o.pop("max_steps", 0)), int(o.pop("fixed_steps", 0)), float(o.pop("tol", 0)),
+                int(o.pop("check_every", 0)), int(o.pop("check_set", CHECK_FACES)), float(o.pop("fmax", 0)),
+                int(o.pop("batched", 0)))
+    o.pop("sparse_dft", None)
+    if o:
+        raise TypeError("unknown run options %s" % sorted(o))
+    return r
+
+
+class Grid:
+    """emm_grid handle + the torch workspace it is bound to."""
+
+    def __init__(self, x, y, z, rd, nb, ne=-1, top=TOP_CPML, f0=1.0, cfl=0.99, aux_dx=0.0):
+        x, y, z = (np.ascontiguousarray(v, dtype=np.float64) for v in (x, y, z))
+        o = GridOpts(rd, nb, ne, top, f0, cfl, aux_dx)
+        h = C.c_void_p()
+        _chk(lib().emm_grid_create(_dptr(x), len(x), _dptr(y), len(y), _dptr(z), len(z), C.byref(o), C.byref(h)))
+        self._h = h
+        self.ncell = (len(x) - 1, len(y) - 1, len(z) - 1)
+        self.rd = rd
+        self._ws = None
+        self._plan = None
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().emm_grid_destroy(self._h)
+            self._h = None
+        self._ws = None
+
+    __del__ = close
+
+    def info(self):
+        ints = (C.c_int * len(_INFO))()
+        dt = C.c_double()
+        _chk(lib().emm_grid_info(self._h, ints, C.byref(dt)))
+        d = dict(zip(_INFO, list(ints)))
+        d["dt"] = dt.value
+        return d
+
+    @property
+    def shape(self):
+        i = self.info()
+        return (i["N3"], i["N2"], i["N1"])
+
+    def coords(self, axis):
+        n = self.info()["N%d" % (axis + 1)]
+        out = np.zeros(n + 1)
+        _chk(lib().emm_grid_coords(self._h, axis, _dptr(out)))
+        return out
+
+    def fdcoef(self, axis, plus):
+        n = self.info()["N%d" % (axis + 1)]
+        out = np.zeros((n, 2 * self.rd))
+        _chk(lib().emm_grid_fdcoef(self._h, axis, int(plus), _dptr(out)))
+        return out
+
+    # -- device memory and stream come from torch --
+    def workspace_bytes(self, nsrc, nfreq, max_steps, nrec):
+        n = lib().emm_workspace_bytes(self._h, nsrc, nfreq, max_steps, nrec)
+        if n == 0:
+            raise EmmError(ECUDA, lib().emm_last_error().decode())
+        return n
+
+    def bind(self, nsrc=1, nfreq=1, max_steps=0, nrec=64, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libemm_b200 needs a CUDA device; there is no CPU fallback")
+        max_steps = max_steps or 100000
+        plan = (nsrc, nfreq, max_steps, nrec)
+        if self._ws is not None and self._plan is not None and all(a <= b for a, b in zip(plan, self._plan)):
+            return
+        torch.cuda.set_device(device)
+        n = self.workspace_bytes(nsrc, nfreq, max_steps, nrec)
+        self._ws = None
+        self._ws = torch.empty(n, dtype=torch.uint8, device=device)
+        stream = torch.cuda.current_stream(device).cuda_stream
+        _chk(lib().emm_bind_device(self._h, C.c_void_p(self._ws.data_ptr()), n, C.c_void_p(stream)))
+        self._plan = plan
+        self._model = None
+
+    def model_set(self, sigma_h, sigma_v=None):
+        sh = np.ascontiguousarray(sigma_h, dtype=np.float32)
+        assert sh.shape == self.ncell[::-1], (sh.shape, self.ncell)
+        sv = None if sigma_v is None else np.ascontiguousarray(sigma_v, dtype=np.float32)
+        self._model = (sh, sv)
+        if self._ws is None:
+            self.bind()
+        fp = C.POINTER(C.c_float)
+        _chk(lib().emm_model_set(self._h, sh.ctypes.data_as(fp), None if sv is None else sv.ctypes.data_as(fp)))
+
+    def _ensure(self, nsrc, nfreq, nrec, opts):
+        """grow the workspace if this run needs more than what is bound (re-uploads the model)"""
+        o = opts or {}
+        steps = int(o.get("fixed_steps", 0)) or int(o.get("max_steps", 0)) or 100000
+        resident = nsrc if (o.get("batched", 0) or o.get("_resident", 0)) else 1
+        plan = (resident, nfreq, steps, max(nrec, 1))
+        if self._plan is None or any(a > b for a, b in zip(plan, self._plan)):
+            model = getattr(self, "_model", None)
+            self.bind(*[max(a, b) for a, b in zip(plan, self._plan or plan)])
+            if model is not None:
+                self.model_set(*model)
+
+    def run(self, sources, freqs, receivers, opts=None, allow_noconv=False):
+        freqs = np.ascontiguousarray(freqs, dtype=np.float64)
+        rec = np.ascontiguousarray(receivers, dtype=np.float64).reshape(-1, 3)
+        self._ensure(len(sources), len(freqs), len(rec), opts)
+        out = np.zeros((len(sources), len(freqs), len(rec), 6), dtype=np.complex128)
+        ns = np.zeros(len(sources), dtype=np.int32)
+        o = _ropts(opts)
+        self.last_rc = _chk(lib().emm_run(self._h, _srcs(sources), len(sources), _dptr(freqs), len(freqs), _dptr(rec), len(rec),
+                                          C.byref(o), out.ctypes.data_as(C.POINTER(C.c_double)),
+                                          ns.ctypes.data_as(C.POINTER(C.c_int))), allow=(ENOCONV,) if allow_noconv else ())
+        return out, ns
+
+    def run_begin(self, sources, freqs, receivers, opts=None):
+        freqs = np.ascontiguousarray(freqs, dtype=np.float64)
+        rec = np.ascontiguousarray(receivers, dtype=np.float64).reshape(-1, 3)
+        o2 = dict(opts or {})
+        o2["_resident"] = 1
+        self._ensure(len(sources), len(freqs), len(rec), o2)
+        self._shape_out = (len(sources), len(freqs), len(rec), 6)
+        o = _ropts(opts)
+        _chk(lib().emm_run_begin(self._h, _srcs(sources), len(sources), _dptr(freqs), len(freqs), _dptr(rec), len(rec),
+                                 C.byref(o)))
+
+    def run_steps(self, n, allow_noconv=True):
+        ns = np.zeros(self._shape_out[0], dtype=np.int32)
+        done = C.c_int()
+        _chk(lib().emm_run_steps(self._h, n, ns.ctypes.data_as(C.POINTER(C.c_int)), C.byref(done)),
+             allow=(ENOCONV,) if allow_noconv else ())
+        return ns, bool(done.value)
+
+    def run_enqueue(self, n):
+        _chk(lib().emm_run_enqueue(self._h, n))
+
+    def run_end(self):
+        out = np.zeros(self._shape_out, dtype=np.complex128)
+        ns = np.zeros(self._shape_out[0], dtype=np.int32)
+        _chk(lib().emm_run_end(self._h, out.ctypes.data_as(C.POINTER(C.c_double)), ns.ctypes.data_as(C.POINTER(C.c_int))))
+        return out, ns
+
+    def get(self, what, isrc=0, ifreq=0):
+        code = _GET[what]
+        if what == "JW":
+            out = np.zeros(self._shape_out[1], dtype=np.complex128)
+        elif what == "DELTA":
+            out = np.zeros(2)
+        elif what.startswith("F_"):
+            out = np.zeros(self.shape, dtype=np.complex64)
+        else:
+            out = np.zeros(self.shape, dtype=np.float32)
+        _chk(lib().emm_get(self._h, isrc, code, ifreq, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def launch_count(self):
+        return int(lib().emm_launch_count(self._h))

@@ -1,0 +1,162 @@
+"""GPU parity (`-m gpu`): the CUDA path, driven through the C ABI, against the fp64 oracle on the same
+seeded inputs, element by element.  Tolerances are north_star's: fp32 fields after 200 steps within 1e-5
+relative L2; converged receivers within 1e-3 at every receiver above 1e-3 of the peak; step counts exact.
+Sizes span several thread tiles (64 x-nodes, 8 rows, 16-plane chunks) and ragged tails."""
+import numpy as np
+import pytest
+
+from helpers import make_grid
+from paper_2304_00233_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+FIELDS = ("E1", "E2", "E3", "H1", "H2", "H3")
+
+
+@pytest.fixture(scope="module")
+def emm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2304_00233_b200 import emm as m
+    m.build()
+    return m
+
+
+def _rel_l2(a, b):
+    a = np.asarray(a, dtype=np.complex128 if np.iscomplexobj(a) else np.float64)
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a)
+
+
+def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, batched=0):
+    sources = sources or w["sources"]
+    opts = dict(fixed_steps=nsteps, batched=batched)
+    ga, gb = make_grid(emm, w), make_grid(oracle, w)
+    assert abs(ga.info()["dt"] / gb.info()["dt"] - 1) < 1e-12
+    for c in ("CE1", "CE2", "CE3"):
+        assert _rel_l2(ga.get(c), gb.get(c)) < 1e-7, c
+    ga.run_begin(sources, w["freqs"], w["receivers"], opts)
+    gb.run_begin(sources, w["freqs"], w["receivers"], opts)
+    nsa, da = ga.run_steps(nsteps)
+    nsb, db = gb.run_steps(nsteps)
+    assert list(nsa) == list(nsb) == [nsteps] * len(sources) and da and db
+    worst = {}
+    for s in range(len(sources)):
+        for c in FIELDS:
+            fa, fb = ga.get(c, isrc=s), gb.get(c, isrc=s)
+            assert np.all(np.isfinite(fa))
+            e = _rel_l2(fa, fb)
+            worst[c] = max(worst.get(c, 0), e)
+            assert e < tol, (w["name"], s, c, e)
+        for f in range(len(w["freqs"])):
+            for c in FIELDS:
+                Fa, Fb = ga.get("F_" + c, isrc=s, ifreq=f), gb.get("F_" + c, isrc=s, ifreq=f)
+                e = _rel_l2(Fa, Fb)
+                assert e < ftol, (w["name"], s, f, "F_" + c, e)
+    oa, _ = ga.run_end()
+    ob, _ = gb.run_end()
+    big = np.abs(ob) > 1e-3 * np.abs(ob).max()
+    assert np.all(np.abs(oa - ob)[big] <= 1e-3 * np.abs(ob)[big])
+    ga.close()
+    return worst
+
+
+@pytest.mark.parametrize("rd", [1, 2, 3])
+def test_fields_wholespace_cpml(emm, oracle, rd):
+    """configs[0] scaled: homogeneous, CPML on six faces; 70 x-nodes (2 tiles + ragged tail), 200 steps."""
+    w = W.cfg1(n=40 - 2 * rd, dx=100.0, rd=rd, nb=7)
+    _field_parity(emm, oracle, w, 200)
+
+
+@pytest.mark.parametrize("rd", [1, 2, 3])
+def test_fields_layered_air_uniform(emm, oracle, rd):
+    """configs[1] scaled: layered marine model, FFT air-water boundary on the padded plane itself."""
+    w = W.cfg2(nx=36, nz=24, dx=100.0, rd=rd, nb=8)
+    _field_parity(emm, oracle, w, 200)
+
+
+@pytest.mark.parametrize("rd,builder", [(2, "cfg3"), (3, "cfg4")])
+def test_fields_nonuniform_aux_plane_vti(emm, oracle, rd, builder):
+    """configs[2]/[3] scaled: non-uniform x-y-z, VTI cells from sub-sampling, auxiliary-plane air boundary."""
+    kw = dict(nx=40, nz=36, rd=rd, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
+    w = W.build(builder, oracle.nugrid, **kw)
+    w["receivers"] = w["receivers"] * 0.1 + np.array([0, 0, 900.0])      # keep them inside the small model
+    w["sigma_v"] = (w["sigma_v"] * 0.6).astype(np.float32)                # make the anisotropy bite everywhere
+    _field_parity(emm, oracle, w, 200)
+
+
+def test_fields_batched_sources(emm, oracle):
+    """configs[4] scaled: several sources advanced by one launch per kernel, each against its own oracle run."""
+    w = W.cfg5(oracle.nugrid, nx=32, nz=30, rd=2, nb=6, n_water=6, nsrc=3, n_rec_side=3, aux_dx=100.0)
+    srcs = [((-180.0 + 170.0 * i, 40.0 * i, 950.0), (1.0, 0.3 * i, 0.1)) for i in range(3)]
+    w["receivers"] = w["receivers"] * 0.1 + np.array([0, 0, 900.0])
+    _field_parity(emm, oracle, w, 120, sources=srcs, batched=1)
+
+
+def test_converged_run_matches_oracle_steps_and_receivers(emm, oracle):
+    """configs[1] scaled, run to convergence: integer step count exact, receivers within 1e-3."""
+    w = W.cfg2(nx=40, nz=28, dx=100.0, rd=2, nb=8)
+    opts = dict(tol=1e-6, check_every=100)
+    ga, gb = make_grid(emm, w), make_grid(oracle, w)
+    oa, nsa = ga.run(w["sources"], w["freqs"], w["receivers"], opts)
+    ob, nsb = gb.run(w["sources"], w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
+    assert list(nsa) == list(nsb) and nsa[0] % 100 == 0 and nsa[0] > 0
+    big = np.abs(ob) > 1e-3 * np.abs(ob).max()
+    rel = np.abs(oa - ob)[big] / np.abs(ob)[big]
+    assert rel.max() < 1e-3, rel.max()
+    da = ga.get("DELTA")
+    assert np.all(da < 1e-6)
+
+
+def test_converged_cfg1_fixed_500_steps(emm, oracle):
+    """configs[0] itself (48^3, rd=1, 500 fixed steps, 20 in-line receivers)."""
+    w = W.cfg1()
+    ga, gb = make_grid(emm, w), make_grid(oracle, w)
+    oa, nsa = ga.run(w["sources"], w["freqs"], w["receivers"], w["run"])
+    ob, nsb = gb.run(w["sources"], w["freqs"], w["receivers"], w["run"])
+    assert list(nsa) == list(nsb) == [500]
+    ex_a, ex_b = oa[0, 0, :, 0], ob[0, 0, :, 0]
+    assert np.abs(ex_a / ex_b - 1).max() < 1e-3
+
+
+def test_batched_equals_sequential_and_nsteps_per_source(emm, oracle):
+    w = W.cfg2(nx=32, nz=24, dx=100.0, rd=2, nb=8)
+    srcs = [((-300.0, 0.0, 950.0), (1, 0, 0)), ((250.0, 100.0, 900.0), (0, 1, 0))]
+    ga = make_grid(emm, w)
+    opts = dict(tol=1e-6, check_every=100)
+    o_seq, n_seq = ga.run(srcs, w["freqs"], w["receivers"], dict(opts, batched=0))
+    o_bat, n_bat = ga.run(srcs, w["freqs"], w["receivers"], dict(opts, batched=1))
+    assert list(n_seq) == list(n_bat)
+    assert np.array_equal(o_seq, o_bat)               # same kernels, same arithmetic, source by source
+    gb = make_grid(oracle, w)
+    o_or, n_or = gb.run(srcs, w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
+    assert list(n_or) == list(n_bat)
+
+
+def test_edge_cases(emm, oracle):
+    w = W.cfg1(n=12, dx=100.0, rd=1, nb=3)
+    ga = make_grid(emm, w)
+    # no receivers: nothing to write, step count still returned
+    out, ns = ga.run(w["sources"], w["freqs"], np.zeros((0, 3)), dict(fixed_steps=7))
+    assert out.shape == (1, 1, 0, 6) and ns[0] == 7
+    # max_steps reached -> EMM_ENOCONV, outputs still finite
+    out, ns = ga.run(w["sources"], w["freqs"], w["receivers"][:2], dict(tol=1e-30, check_every=20, max_steps=60), allow_noconv=True)
+    assert ga.last_rc == emm.ENOCONV and ns[0] == 60 and np.all(np.isfinite(out))
+    # source / receiver outside the interior
+    with pytest.raises(emm.EmmError) as e:
+        ga.run([((5000.0, 600.0, 600.0), (1, 0, 0))], w["freqs"], w["receivers"][:1], dict(fixed_steps=3))
+    assert e.value.code == emm.EINVAL
+    with pytest.raises(emm.EmmError):
+        ga.run(w["sources"], w["freqs"], [[-400.0, 600.0, 600.0]], dict(fixed_steps=3))
+    with pytest.raises(emm.EmmError):
+        ga.model_set(-np.ones((12, 12, 12), np.float32))
+    # maximum number of frequencies on the unrolled path + the runtime fallback give the same accumulators as the oracle
+    ga = make_grid(emm, w)
+    gb = make_grid(oracle, w)
+    freqs = np.array([0.25, 0.5, 0.75, 1.0, 1.25, 1.5, 2.0])
+    ga.run_begin(w["sources"], freqs, w["receivers"][:2], dict(fixed_steps=40))
+    gb.run_begin(w["sources"], freqs, w["receivers"][:2], dict(fixed_steps=40))
+    ga.run_steps(40)
+    gb.run_steps(40)
+    for f in (0, 6):
+        assert _rel_l2(ga.get("F_E1", ifreq=f), gb.get("F_E1", ifreq=f)) < 2e-5
+        assert _rel_l2(ga.get("F_H2", ifreq=f), gb.get("F_H2", ifreq=f)) < 2e-5
