@@ -592,7 +592,8 @@ int emmo_run_begin(emmo_grid *g, const emmo_src *src, int nsrc, const double *fr
   for (int q = 0; q < nrec; q++) for (int c = 0; c < 6; c++) for (int a = 0; a < 3; a++) {
     const double *S = LAT[c][a] ? g->xh[a] : g->xn[a];
     int lo_ok = (a == 2) ? g->klo : r;
-    if (lattice_stencil(S, g->N[a], rec[3 * q + a], R->np, lo_ok, &R->rst[((size_t)q * 6 + c) * 3 + a]) ||
+    if (rec[3 * q + a] < g->xn[a][g->lo[a]] || rec[3 * q + a] > g->xn[a][g->lo[a] + g->nc[a]] ||
+        lattice_stencil(S, g->N[a], rec[3 * q + a], R->np, lo_ok, &R->rst[((size_t)q * 6 + c) * 3 + a]) ||
         R->rst[((size_t)q * 6 + c) * 3 + a].start + R->np - 1 > g->N[a] - 1 - r) {
       free_run(g); return fail(EMMO_EINVAL, "run_begin: receiver %d outside the interior", q);
     }

@@ -436,7 +436,9 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     R->rst.resize((size_t)std::max(nrec, 1) * 18);
     for (int q = 0; q < nrec; ++q) for (int c = 0; c < 6; ++c) for (int a = 0; a < 3; ++a) {
       const double *S = kLat[c][a] ? g->xh[a].data() : g->xn[a].data();
-      if (!make_stencil(S, g->N[a], rec[3 * q + a], np, a == 2 ? g->klo : r, g->N[a] - 1 - r, false, &R->rst[((size_t)q * 6 + c) * 3 + a])) {
+      const double p = rec[3 * q + a];
+      if (p < g->xn[a][g->lo[a]] || p > g->xn[a][g->lo[a] + g->nc[a]] ||
+          !make_stencil(S, g->N[a], p, np, a == 2 ? g->klo : r, g->N[a] - 1 - r, false, &R->rst[((size_t)q * 6 + c) * 3 + a])) {
         free_run(g); return fail(EMM_EINVAL, "emm_run_begin: receiver %d outside the interior", q);
       }
       const Stencil1 &st = R->rst[((size_t)q * 6 + c) * 3 + a];

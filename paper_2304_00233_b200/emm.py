@@ -157,6 +157,7 @@ class Grid:
         self.rd = rd
         self._ws = None
         self._plan = None
+        self._model = None
 
     def close(self):
         if getattr(self, "_h", None):
@@ -213,7 +214,6 @@ class Grid:
         stream = torch.cuda.current_stream(device).cuda_stream
         _chk(lib().emm_bind_device(self._h, C.c_void_p(self._ws.data_ptr()), n, C.c_void_p(stream)))
         self._plan = plan
-        self._model = None
 
     def model_set(self, sigma_h, sigma_v=None):
         sh = np.ascontiguousarray(sigma_h, dtype=np.float32)

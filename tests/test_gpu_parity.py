@@ -27,7 +27,27 @@ def _rel_l2(a, b):
     return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a)
 
 
+def _group_errors(ga, gb, s):
+    """per field: ||a-b||_2, ||b||_2; plus the E and H group norms (a component that vanishes by symmetry,
+    e.g. Hx of an x-dipole, is measured against its group)"""
+    d, n = {}, {}
+    for c in FIELDS:
+        fa, fb = ga.get(c, isrc=s), gb.get(c, isrc=s)
+        assert np.all(np.isfinite(fa)), c
+        d[c] = np.linalg.norm(fa.astype(np.float64) - fb)
+        n[c] = np.linalg.norm(fb)
+    grp = {"E": max(n[c] for c in FIELDS[:3]), "H": max(n[c] for c in FIELDS[3:])}
+    return d, n, grp
+
+
 def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, batched=0):
+    """Field parity at four checkpoints up to `nsteps` (200 in north_star).
+
+    Tolerance: relative L2 <= 1e-5 per field wherever the field still
+    carries >= 10 % of its peak norm; everywhere ||a-b|| <= 1e-5 * peak norm.  The second form is needed
+    because the fictitious wave domain is lossless: fp32 rounding at the source node leaves a static,
+    curl-free residual of ~1e-8 of the peak that never radiates away, while on these small test grids the
+    wave itself has left through the CPML long before step 200."""
     sources = sources or w["sources"]
     opts = dict(fixed_steps=nsteps, batched=batched)
     ga, gb = make_grid(emm, w), make_grid(oracle, w)
@@ -36,34 +56,49 @@ def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, bat
         assert _rel_l2(ga.get(c), gb.get(c)) < 1e-7, c
     ga.run_begin(sources, w["freqs"], w["receivers"], opts)
     gb.run_begin(sources, w["freqs"], w["receivers"], opts)
-    nsa, da = ga.run_steps(nsteps)
-    nsb, db = gb.run_steps(nsteps)
-    assert list(nsa) == list(nsb) == [nsteps] * len(sources) and da and db
-    worst = {}
-    for s in range(len(sources)):
-        for c in FIELDS:
-            fa, fb = ga.get(c, isrc=s), gb.get(c, isrc=s)
-            assert np.all(np.isfinite(fa))
-            e = _rel_l2(fa, fb)
-            worst[c] = max(worst.get(c, 0), e)
-            assert e < tol, (w["name"], s, c, e)
-        for f in range(len(w["freqs"])):
+    peak = [{"E": 0.0, "H": 0.0} for _ in sources]
+    done_steps, strict_checks = 0, 0
+    for q in range(4):
+        n = nsteps * (q + 1) // 4 - done_steps
+        nsa, da = ga.run_steps(n)
+        nsb, db = gb.run_steps(n)
+        done_steps += n
+        assert list(nsa) == list(nsb) == [done_steps] * len(sources)
+        for s in range(len(sources)):
+            d, nrm, grp = _group_errors(ga, gb, s)
+            for k in ("E", "H"):
+                peak[s][k] = max(peak[s][k], grp[k])
             for c in FIELDS:
-                Fa, Fb = ga.get("F_" + c, isrc=s, ifreq=f), gb.get("F_" + c, isrc=s, ifreq=f)
-                e = _rel_l2(Fa, Fb)
+                k = c[0]
+                assert d[c] <= tol * peak[s][k], (w["name"], done_steps, s, c, d[c] / peak[s][k])
+                if grp[k] >= 0.1 * peak[s][k] and nrm[c] > 1e-3 * grp[k]:
+                    strict_checks += 1
+                    assert d[c] <= tol * nrm[c], (w["name"], done_steps, s, c, d[c] / nrm[c])
+    assert da and db and strict_checks >= 5
+    for s in range(len(sources)):
+        for f in range(len(w["freqs"])):
+            Fn = {c: gb.get("F_" + c, isrc=s, ifreq=f) for c in FIELDS}
+            for c in FIELDS:
+                grp = max(np.linalg.norm(Fn[x]) for x in FIELDS if x[0] == c[0])
+                e = np.linalg.norm(ga.get("F_" + c, isrc=s, ifreq=f).astype(np.complex128) - Fn[c]) / grp
                 assert e < ftol, (w["name"], s, f, "F_" + c, e)
     oa, _ = ga.run_end()
     ob, _ = gb.run_end()
-    big = np.abs(ob) > 1e-3 * np.abs(ob).max()
-    assert np.all(np.abs(oa - ob)[big] <= 1e-3 * np.abs(ob)[big])
+    for s in range(len(sources)):
+        for k in (slice(0, 3), slice(3, 6)):
+            A, B = oa[s][..., k], ob[s][..., k]
+            big = np.abs(B) > 1e-3 * np.abs(B).max()
+            assert np.all(np.abs(A - B)[big] <= 1e-3 * np.abs(B)[big])
     ga.close()
-    return worst
 
 
 @pytest.mark.parametrize("rd", [1, 2, 3])
 def test_fields_wholespace_cpml(emm, oracle, rd):
     """configs[0] scaled: homogeneous, CPML on six faces; 70 x-nodes (2 tiles + ragged tail), 200 steps."""
     w = W.cfg1(n=40 - 2 * rd, dx=100.0, rd=rd, nb=7)
+    src = np.array(w["sources"][0][0])
+    offs = np.array([300.0, 600.0, 900.0, 1200.0])        # off-axis, off-grid: all six components are non-zero
+    w["receivers"] = np.stack([src[0] + 0.8 * offs, src[1] + 0.36 * offs, src[2] - 0.48 * offs], axis=1)
     _field_parity(emm, oracle, w, 200)
 
 
@@ -74,12 +109,18 @@ def test_fields_layered_air_uniform(emm, oracle, rd):
     _field_parity(emm, oracle, w, 200)
 
 
+def _small_receivers():
+    g = np.array([-310.0, -95.0, 140.0, 330.0])
+    X, Y = np.meshgrid(g, g * 0.9, indexing="xy")
+    return np.stack([X.ravel(), Y.ravel(), np.full(X.size, 1000.0)], axis=1)
+
+
 @pytest.mark.parametrize("rd,builder", [(2, "cfg3"), (3, "cfg4")])
 def test_fields_nonuniform_aux_plane_vti(emm, oracle, rd, builder):
     """configs[2]/[3] scaled: non-uniform x-y-z, VTI cells from sub-sampling, auxiliary-plane air boundary."""
     kw = dict(nx=40, nz=36, rd=rd, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
     w = W.build(builder, oracle.nugrid, **kw)
-    w["receivers"] = w["receivers"] * 0.1 + np.array([0, 0, 900.0])      # keep them inside the small model
+    w["receivers"] = _small_receivers()
     w["sigma_v"] = (w["sigma_v"] * 0.6).astype(np.float32)                # make the anisotropy bite everywhere
     _field_parity(emm, oracle, w, 200)
 
@@ -88,7 +129,7 @@ def test_fields_batched_sources(emm, oracle):
     """configs[4] scaled: several sources advanced by one launch per kernel, each against its own oracle run."""
     w = W.cfg5(oracle.nugrid, nx=32, nz=30, rd=2, nb=6, n_water=6, nsrc=3, n_rec_side=3, aux_dx=100.0)
     srcs = [((-180.0 + 170.0 * i, 40.0 * i, 950.0), (1.0, 0.3 * i, 0.1)) for i in range(3)]
-    w["receivers"] = w["receivers"] * 0.1 + np.array([0, 0, 900.0])
+    w["receivers"] = _small_receivers()
     _field_parity(emm, oracle, w, 120, sources=srcs, batched=1)
 
 
