@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""bench.py -- Gcell-updates/s of the whole FDTD step (E and H updates with CPML, air-water boundary,
+source, DTFT, convergence bookkeeping) on BASELINE.json's production config (configs[3]: non-uniform
+400x400x200, 5 frequencies), one JSON line on stdout.  See DESIGN.md "Measurement".
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--rd 3] [--impl reference]
+
+A "step" is one pass of Algorithm 1 lines 9-23 over the padded grid.  `value` times K steps with all
+inputs resident in HBM (CUDA events on the stream the kernels run on); `e2e` is the same metric through
+emm_model_set + emm_run with host buffers.  Multi-GPU = independent replicas (one process per GPU, no
+data-path collective: the method does not shard).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2304_00233_b200 import workloads as W  # noqa: E402
+
+METRIC = "Gcell-updates/s (E+H, fp32), whole FDTD step incl. CPML, air-water BC, source, DTFT"
+
+
+def build_workload(args, nugrid):
+    kw = {}
+    if args.workload in ("cfg3", "cfg4", "cfg5"):
+        kw = dict(rd=args.rd) if args.rd else {}
+        if args.scale != 1.0:
+            base = {"cfg3": (200, 120), "cfg4": (400, 200), "cfg5": (256, 160)}[args.workload]
+            kw.update(nx=int(base[0] * args.scale) // 2 * 2, nz=int(base[1] * args.scale),
+                      n_water=max(4, int(round(28 * args.scale))))
+        if args.aux_dx:
+            kw["aux_dx"] = args.aux_dx
+        w = W.build(args.workload, nugrid, **kw)
+        if args.workload == "cfg4" and args.nf:
+            w["freqs"] = w["freqs"][: args.nf]
+    else:
+        w = W.build(args.workload, None, **({"rd": args.rd} if args.rd else {}))
+    return w
+
+
+def describe(w, info, nsrc):
+    return {"workload": "%s: %dx%dx%d cells, rd=%d (order %d), %s, nf=%d, nsrc=%d, padded %dx%dx%d" % (
+        w["name"], len(w["x"]) - 1, len(w["y"]) - 1, len(w["z"]) - 1, w["grid"]["rd"], 2 * w["grid"]["rd"],
+        "non-uniform" if not info["uniform_xy"] else "uniform x-y", len(w["freqs"]), nsrc, info["N1"], info["N2"], info["N3"]),
+        "padded_nodes": info["N1"] * info["N2"] * info["N3"],
+        "air_plane": [info["aux_M1"], info["aux_M2"]],
+        "l2": "working set (fields + DTFT accumulators) is >> the 126 MB L2; no flush needed"}
+
+
+def algorithmic_bytes(info, nf, nb, kernel):
+    """E kernel reads 3 H, RMWs 3 E, reads 3 dt/eps = 48 B/node; H kernel reads 3 E, RMWs 3 H
+    = 36 B/node; each RMWs 3*nf complex accumulators (48*nf B) per DTFT-box node; plus 8 B per active CPML
+    memory variable (two per slab membership)."""
+    N1, N2, N3 = info["N1"], info["N2"], info["N3"]
+    N = N1 * N2 * N3
+    box = ((info["box_hi1"] - info["box_lo1"] + 1) * (info["box_hi2"] - info["box_lo2"] + 1)
+           * (info["box_hi3"] - info["box_lo3"] + 1))
+    zs = (2 if info["k0"] < 0 else 1) * nb
+    psi = 16 * (2 * nb * N2 * N3 + 2 * nb * N1 * N3 + zs * N1 * N2)
+    return (48 if kernel == "E" else 36) * N + 48 * nf * box + psi
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                       "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+        time.sleep(0.3)
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.1)
+        self.p.terminate()
+        self.p.wait()
+        self.f.flush()
+        rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.strip() == "Active":
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(w_full, budget_s, steps, warmup, args):
+    """Oracle (as it stands) on the host cores, on a bounded sample: the same recipe at a size chosen so that
+    steps+warmup time steps take about budget_s.  Returns (Mcell/s, seconds per step list, description)."""
+    from oracle import emm_oracle as O
+    O.build()
+    ncores = os.cpu_count() or 1
+    # calibrate on a tiny instance of the same recipe
+    scale = 0.12
+    rate = None
+    for _ in range(3):
+        a2 = argparse.Namespace(**vars(args))
+        a2.scale = scale
+        w = build_workload(a2, O.nugrid)
+        g = O.Grid(w["x"], w["y"], w["z"], **w["grid"])
+        g.model_set(w["sigma_h"], w.get("sigma_v"))
+        i = g.info()
+        n = i["N1"] * i["N2"] * i["N3"]
+        g.run_begin(w["sources"][:1], w["freqs"], w["receivers"][:4], dict(fixed_steps=10 ** 6, sparse_dft=0))
+        g.run_steps(1)
+        t = time.perf_counter()
+        g.run_steps(2)
+        dt2 = (time.perf_counter() - t) / 2
+        g.close()
+        rate = n / dt2
+        target = min(budget_s * rate / max(steps + warmup, 1), 12e6)   # nodes of a sample that fits the budget (and ~8 GB of host RAM)
+        full = None
+        if args.workload not in ("cfg1", "cfg2"):
+            full = (len(w_full["x"]) - 1) ** 2 * (len(w_full["z"]) - 1) * 1.35
+        new_scale = min(1.0, scale * (target / n) ** (1 / 3.0)) if full else 1.0
+        if args.workload in ("cfg1", "cfg2") or abs(new_scale - scale) < 0.25 * scale or new_scale <= scale:
+            break
+        scale = new_scale
+    a2 = argparse.Namespace(**vars(args))
+    a2.scale = scale
+    w = build_workload(a2, O.nugrid)
+    g = O.Grid(w["x"], w["y"], w["z"], **w["grid"])
+    g.model_set(w["sigma_h"], w.get("sigma_v"))
+    i = g.info()
+    n = i["N1"] * i["N2"] * i["N3"]
+    g.run_begin(w["sources"][:1], w["freqs"], w["receivers"][:4], dict(fixed_steps=10 ** 6, sparse_dft=0))
+    g.run_steps(warmup)
+    t = time.perf_counter()
+    g.run_steps(steps)
+    el = time.perf_counter() - t
+    g.close()
+    desc = ("%s recipe at %dx%dx%d cells (padded %dx%dx%d, nf=%d, full-box DTFT), %d steps after %d warm-up, fp64, "
+            "gcc -O2 -fopenmp" % (w["name"], len(w["x"]) - 1, len(w["y"]) - 1, len(w["z"]) - 1, i["N1"], i["N2"], i["N3"],
+                                  len(w["freqs"]), steps, warmup))
+    return n * steps / el / 1e9, el / steps * 1e3, ncores, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w_full = build_workload(args, None) if args.workload in ("cfg1", "cfg2") else None
+    if w_full is None:
+        from oracle import emm_oracle as O
+        O.build()
+        w_full = build_workload(args, O.nugrid)
+    val, ms, cores, desc = oracle_rate(w_full, 120.0, args.steps, args.warmup, args)
+    from oracle import emm_oracle as O
+    gi = O.Grid(w_full["x"], w_full["y"], w_full["z"], **w_full["grid"]).info()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "Gcell-updates/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": describe(w_full, gi, 1),
+            "cpu_baseline": {"value": val, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": "Gcell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2304_00233_b200 import emm
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    emm.build()
+    w = build_workload(args, emm.emm_nugrid)
+    nsrc = len(w["sources"]) if w["run"].get("batched") else 1
+    srcs = w["sources"][:nsrc]
+    K, Wm = args.steps, max(args.warmup, 3)
+    g = emm.Grid(w["x"], w["y"], w["z"], **w["grid"])
+    g.bind(nsrc=nsrc, nfreq=len(w["freqs"]), max_steps=K + Wm + 8, nrec=len(w["receivers"]), device=dev)
+    info = g.info()
+    N = info["N1"] * info["N2"] * info["N3"]
+
+    # ---- end to end through the C ABI with host buffers (model upload + run + receiver read-back) ----
+    sh = np.ascontiguousarray(w["sigma_h"], np.float32)
+    sv = None if w.get("sigma_v") is None else np.ascontiguousarray(w["sigma_v"], np.float32)
+    g.model_set(sh, sv)                                        # warm-up of the whole path (plans, kernels)
+    g.run(srcs, w["freqs"], w["receivers"], dict(fixed_steps=3, batched=1 if nsrc > 1 else 0))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    g.model_set(sh, sv)
+    out, ns = g.run(srcs, w["freqs"], w["receivers"], dict(fixed_steps=K, batched=1 if nsrc > 1 else 0))
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    assert int(ns[0]) == K and np.all(np.isfinite(out))
+    h2d = sh.nbytes + (sv.nbytes if sv is not None else 0) + (K + 1) * (len(w["freqs"]) * 16 + 4 + 32)
+    npnt = max(2 * w["grid"]["rd"], 4) ** 3
+    d2h = nsrc * len(w["freqs"]) * 6 * len(w["receivers"]) * npnt * 8
+    if world > 1:
+        tt = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = float(tt.item())
+
+    # ---- device-resident stepping: K steps timed with CUDA events on the library's stream ----
+    g.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=K + Wm + 4, batched=1 if nsrc > 1 else 0))
+    g.run_enqueue(Wm)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = g.launch_count()
+    g.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    g.run_enqueue(K)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    prof = g.profile_read()
+    g.profile(False)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        dist.barrier()
+        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    g.run_steps(1)
+    for c in ("E1", "H2"):
+        assert np.all(np.isfinite(g.get(c)))
+
+    if rank == 0:
+        value = world * nsrc * N * K / (ms * 1e-3) / 1e9
+        peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(peaks_file):
+            peak, peak_src = float(json.load(open(peaks_file))["hbm_gbs"]), "of measured (MEASURED_PEAKS.json hbm_gbs)"
+        else:
+            peak, peak_src = 6650.0, "of fallback (B200_PROFILING.md)"
+        dom = "E" if prof["E"][0] >= prof["H"][0] else "H"
+        kms = prof[dom][0] / max(prof[dom][1], 1)
+        abytes = nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], dom)
+        achieved = abytes / (kms * 1e-3) / 1e9
+        traffic = None
+        tf = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+        if os.path.exists(tf):
+            traffic = json.load(open(tf)).get("%s:%s:rd%d:nf%d" % (w["name"], dom, w["grid"]["rd"], len(w["freqs"])))
+        roofline = {"bound": "hbm", "kernel": "k_update<%s>" % dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "algorithmic_bytes_per_launch": abytes,
+                    "kernel_ms": kms, "kernels_ms_per_step": {"E": prof["E"][0] / max(prof["E"][1], 1), "H": prof["H"][0] / max(prof["H"][1], 1)},
+                    "step_frac_in_update_kernels": (prof["E"][0] + prof["H"][0]) / ms}
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            v, cms, cores, desc = oracle_rate(w, 20.0, 3, 1, args)
+            cpu = {"value": v, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc, "ms_per_step": cms}
+        line = {"metric": METRIC, "value": value, "unit": "Gcell-updates/s", "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic", "config": describe(w, info, nsrc), "clocks": clocks,
+                "e2e": {"value": world * nsrc * N * K / t_e2e / 1e9, "unit": "Gcell-updates/s", "h2d_bytes_per_step": h2d / K,
+                        "d2h_bytes_per_step": d2h / K, "seconds": t_e2e,
+                        "what": "emm_model_set (host sigma -> device) + emm_run(fixed_steps=K) (tables up, receivers back)"},
+                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+                "multi_gpu": "replicas only: every rank runs the whole workload, no collective on the data path"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--rd", type=int, default=0, help="override the FD half length (cfg4: 3 = 6th order as configs[3]; 2 = 4th order)")
+    ap.add_argument("--nf", type=int, default=0, help="cfg4: keep only the first nf frequencies")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the cell counts (debugging only)")
+    ap.add_argument("--aux-dx", type=float, default=0.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -143,6 +143,12 @@ int emm_run_enqueue(emm_grid *g, int n);
 int emm_run_end(emm_grid *g, double *out, int *nsteps);
 int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_out);
 
+/* Optional timing of the two fused update kernels: emm_profile(g,1) brackets every later launch of the
+ * E and H update kernel with CUDA events on the bound stream; emm_profile_read drains the stream and
+ * returns the summed durations ms[2] = {E kernel, H kernel} and launch counts, then resets.           */
+int emm_profile(emm_grid *g, int enable);
+int emm_profile_read(emm_grid *g, double *ms, int *counts);
+
 /* number of kernel launches issued by this library since the grid was created (bench evidence) */
 long long emm_launch_count(const emm_grid *g);
 

@@ -119,4 +119,8 @@ struct emm_grid {
   double vref[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // CPML reference speed per face [R5]
   emm::Run *run = nullptr;
   long long launches = 0;
+  // optional per-kernel timing of the two fused update kernels (CUDA events on the bound stream)
+  bool prof = false;
+  std::vector<cudaEvent_t> prof_ev;      // pairs: start, stop
+  std::vector<int> prof_kind;            // 0 = E kernel, 1 = H kernel
 };

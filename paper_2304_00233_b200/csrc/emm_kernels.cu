@@ -403,6 +403,11 @@ int launch_update(emm_grid *g, const DevState &s, int is_h) {
   dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
   if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
   cudaStream_t st = g->stream;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (g->prof) {
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(EMM_ECUDA, "cudaEventCreate failed");
+    cudaEventRecord(e0, st);
+  }
   if (is_h) {
     if (dg.r == 1) launch_update_nf<1, true>(dg, s, grid, block, st, kc, nchunks);
     else if (dg.r == 2) launch_update_nf<2, true>(dg, s, grid, block, st, kc, nchunks);
@@ -411,6 +416,12 @@ int launch_update(emm_grid *g, const DevState &s, int is_h) {
     if (dg.r == 1) launch_update_nf<1, false>(dg, s, grid, block, st, kc, nchunks);
     else if (dg.r == 2) launch_update_nf<2, false>(dg, s, grid, block, st, kc, nchunks);
     else launch_update_nf<3, false>(dg, s, grid, block, st, kc, nchunks);
+  }
+  if (g->prof) {
+    cudaEventRecord(e1, st);
+    g->prof_ev.push_back(e0);
+    g->prof_ev.push_back(e1);
+    g->prof_kind.push_back(is_h);
   }
   EMM_LAUNCH_CHECK(g, is_h ? "k_update<H>" : "k_update<E>");
   return 0;

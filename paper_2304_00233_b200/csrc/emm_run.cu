@@ -146,6 +146,7 @@ using namespace emm;
 extern "C" void emm_grid_destroy(emm_grid *g) {
   if (!g) return;
   free_run(g);
+  for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
   if (g->have_plans) {
     if (g->plan_fwd) cufftDestroy(g->plan_fwd);
     if (g->plan_inv_e) cufftDestroy(g->plan_inv_e);
@@ -692,4 +693,31 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
     return 0;
   }
   return fail(EMM_EINVAL, "emm_get: unknown item %d", what);
+}
+
+// ---- optional per-kernel timing (bench evidence for the roofline of the dominant kernel) ----
+extern "C" int emm_profile(emm_grid *g, int enable) {
+  if (!g) return fail(EMM_EINVAL, "emm_profile: null grid");
+  for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
+  g->prof_ev.clear();
+  g->prof_kind.clear();
+  g->prof = enable != 0;
+  return 0;
+}
+
+extern "C" int emm_profile_read(emm_grid *g, double *ms, int *counts) {
+  if (!g || !ms || !counts) return fail(EMM_EINVAL, "emm_profile_read: null argument");
+  CU(cudaStreamSynchronize(g->stream));
+  ms[0] = ms[1] = 0.0;
+  counts[0] = counts[1] = 0;
+  for (size_t q = 0; q < g->prof_kind.size(); ++q) {
+    float t = 0.f;
+    CU(cudaEventElapsedTime(&t, g->prof_ev[2 * q], g->prof_ev[2 * q + 1]));
+    ms[g->prof_kind[q]] += t;
+    counts[g->prof_kind[q]]++;
+  }
+  for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
+  g->prof_ev.clear();
+  g->prof_kind.clear();
+  return 0;
 }

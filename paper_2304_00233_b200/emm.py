@@ -27,7 +27,8 @@ _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "
 # every symbol include/emm.h declares (tests check that the library exports all of them)
 SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
            "emm_grid_fdcoef", "emm_workspace_bytes", "emm_bind_device", "emm_model_set", "emm_run", "emm_run_begin",
-           "emm_run_steps", "emm_run_enqueue", "emm_run_end", "emm_get", "emm_launch_count", "emm_last_error")
+           "emm_run_steps", "emm_run_enqueue", "emm_run_end", "emm_get", "emm_profile", "emm_profile_read",
+           "emm_launch_count", "emm_last_error")
 
 
 def build(force=False, verbose=False):
@@ -92,6 +93,8 @@ def lib():
         L.emm_run_enqueue.argtypes = [vp, C.c_int]
         L.emm_run_end.argtypes = [vp, dp, ip]
         L.emm_get.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+        L.emm_profile.argtypes = [vp, C.c_int]
+        L.emm_profile_read.argtypes = [vp, dp, ip]
         L.emm_launch_count.argtypes = [vp]
         L.emm_launch_count.restype = C.c_longlong
         _lib = L
@@ -288,6 +291,15 @@ class Grid:
             out = np.zeros(self.shape, dtype=np.float32)
         _chk(lib().emm_get(self._h, isrc, code, ifreq, out.ctypes.data_as(C.c_void_p)))
         return out
+
+    def profile(self, enable=True):
+        _chk(lib().emm_profile(self._h, int(enable)))
+
+    def profile_read(self):
+        ms = np.zeros(2)
+        cnt = np.zeros(2, dtype=np.int32)
+        _chk(lib().emm_profile_read(self._h, _dptr(ms), cnt.ctypes.data_as(C.POINTER(C.c_int))))
+        return {"E": (float(ms[0]), int(cnt[0])), "H": (float(ms[1]), int(cnt[1]))}
 
     def launch_count(self):
         return int(lib().emm_launch_count(self._h))
