@@ -13,6 +13,7 @@
 // neighbours come through L1/L2 (rows are 128-byte aligned).  The DTFT accumulators are streamed with
 // evict-first loads/stores: they are the dominant HBM traffic (96*nf of 84+96*nf bytes per node-step).
 #include <cstdio>
+#include <cstdlib>
 
 #include "emm_kernels.cuh"
 
@@ -100,8 +101,58 @@ __device__ __forceinline__ void dtft4_rt(float2 *F0, size_t fstride, float4 u, c
   }
 }
 
+#ifndef EMM_MINB
+#define EMM_MINB 3
+#endif
+#ifndef EMM_PF
+#define EMM_PF 1
+#endif
+#ifndef EMM_CPA
+#define EMM_CPA 1
+#endif
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// 16-byte asynchronous global->shared copy (LDGSTS): no register is held while it is in flight.  `.ca` on purpose:
+// the two 16-byte halves of a thread's 32-byte accumulator quad are fetched by two instructions that touch the
+// same sectors; through L1 the second one hits, with `.cg` (L1 bypass) every sector is pulled from L2 twice
+// (measured on cfg4: 6.03 ms/step with .cg vs 5.02 ms/step with .ca).
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Accumulators of one plane staged in shared memory: slot j of thread t sits at sm[j*128 + t] (conflict-free
+// LDS.128).  Each thread only ever touches its own slots, so no block barrier is needed: the thread waits for
+// its own cp.async group.  Slot order: ((c*NF + f)*2 + h), h = first / second pair of nodes of the quad.
+template <int NF>
+__device__ __forceinline__ void stage_plane(float4 *sm, const float2 *Fk, size_t fstride, size_t cstride) {
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const float *p = reinterpret_cast<const float *>(Fk + c * cstride + f * fstride);
+      cp_async16(sm + ((c * NF + f) * 2 + 0) * 128, p);
+      cp_async16(sm + ((c * NF + f) * 2 + 1) * 128, p + 4);
+    }
+}
+
+// DTFT of one component from the staged accumulators: F[f] += u * tw[f], result streamed back to global
+template <int NF>
+__device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0, size_t fstride, float4 u,
+                                             const float2 (&tw)[NF > 0 ? NF : 1]) {
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    float4 a0 = sm[((c * NF + f) * 2 + 0) * 128], a1 = sm[((c * NF + f) * 2 + 1) * 128];
+    a0.x = fmaf(u.x, tw[f].x, a0.x); a0.y = fmaf(u.x, tw[f].y, a0.y); a0.z = fmaf(u.y, tw[f].x, a0.z); a0.w = fmaf(u.y, tw[f].y, a0.w);
+    a1.x = fmaf(u.z, tw[f].x, a1.x); a1.y = fmaf(u.z, tw[f].y, a1.y); a1.z = fmaf(u.w, tw[f].x, a1.z); a1.w = fmaf(u.w, tw[f].y, a1.w);
+    float *p = reinterpret_cast<float *>(F0 + f * fstride);
+    stcs4(p, a0);
+    stcs4(p + 4, a1);
+  }
+}
+
 template <int R, int NF, bool IS_H>
-__global__ void __launch_bounds__(128) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks) {
+__global__ void __launch_bounds__(128, EMM_MINB) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
   const int src = blockIdx.z / nchunks, chunk = blockIdx.z - src * nchunks;
   if (s.done[src]) return;
@@ -169,8 +220,35 @@ __global__ void __launch_bounds__(128) k_update(const DevGrid g, const DevState 
     q2[m] = ld4(A2 + o);
   }
 
+  constexpr bool STAGED = (EMM_CPA != 0) && (NF > 0);
+  extern __shared__ float4 smF_all[];
+  float4 *smF = smF_all + (threadIdx.y * blockDim.x + threadIdx.x);
+  const size_t cstride = (size_t)g.NZB * g.PS;
+  if constexpr (STAGED) {
+    if (dft_xy && kbeg >= g.blo[2] && kbeg <= g.bhi[2])
+      stage_plane<NF>(smF, Fsrc + (size_t)(kbeg - g.blo[2]) * g.PS + row, fstride, cstride);
+    cp_async_commit();
+  }
+
   for (int k = kbeg; k < kend; ++k) {
     const size_t c0 = (size_t)k * g.PS + row;
+#if EMM_PF
+    // pull the next plane's streaming operands into L2 while this plane is being worked on (no registers held)
+    if (k + 1 < kend) {
+      const size_t c1 = c0 + g.PS;
+      prefetch_l2(U1 + c1); prefetch_l2(U2 + c1); prefetch_l2(U3 + c1);
+      if (!IS_H) { prefetch_l2(g.ce[0] + c1); prefetch_l2(g.ce[1] + c1); prefetch_l2(g.ce[2] + c1); }
+      prefetch_l2(A3 + c1);
+      prefetch_l2(A1 + (size_t)(k + R + O) * g.PS + row); prefetch_l2(A2 + (size_t)(k + R + O) * g.PS + row);
+      if (!STAGED && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) {
+        const float2 *Fn = Fsrc + (size_t)(k + 1 - g.blo[2]) * g.PS + row;
+        const size_t cs = (size_t)g.NZB * g.PS;
+        for (int f = 0; f < nf; ++f) {
+          prefetch_l2(Fn + f * fstride); prefetch_l2(Fn + f * fstride + cs); prefetch_l2(Fn + f * fstride + 2 * cs);
+        }
+      }
+    }
+#endif
 #pragma unroll
     for (int m = 0; m < 2 * R - 1; ++m) { q1[m] = q1[m + 1]; q2[m] = q2[m + 1]; }
     {
@@ -242,11 +320,12 @@ __global__ void __launch_bounds__(128) k_update(const DevGrid g, const DevState 
     float4 u1 = ld4(U1 + c0), u2 = ld4(U2 + c0), u3 = ld4(U3 + c0);
     const bool dft = dft_xy && k >= g.blo[2] && k <= g.bhi[2];
     float2 *Fk = Fsrc + (size_t)(k - g.blo[2]) * g.PS + row;
-    const size_t cstride = (size_t)g.NZB * g.PS;
+    if constexpr (STAGED) cp_async_wait_all();        // this thread's copies of plane k have landed
 
     if (IS_H) {
       if (dft) {        // old H sits at t = it*dt, the time level of J (Eq. 8; [R6])
-        if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
+        if constexpr (STAGED) { dtft4_staged<NF>(smF, 0, Fk, fstride, u1, tw); dtft4_staged<NF>(smF, 1, Fk + cstride, fstride, u2, tw); dtft4_staged<NF>(smF, 2, Fk + 2 * cstride, fstride, u3, tw); }
+        else if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
         else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
       }
       const float m0 = upd[0] ? g.dtmu : 0.f, m1 = upd[1] ? g.dtmu : 0.f, m2 = upd[2] ? g.dtmu : 0.f, m3 = upd[3] ? g.dtmu : 0.f;
@@ -261,9 +340,14 @@ __global__ void __launch_bounds__(128) k_update(const DevGrid g, const DevState 
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
       if (dft) {        // new E sits at t = (it+1/2)*dt [R6]
-        if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
+        if constexpr (STAGED) { dtft4_staged<NF>(smF, 0, Fk, fstride, u1, tw); dtft4_staged<NF>(smF, 1, Fk + cstride, fstride, u2, tw); dtft4_staged<NF>(smF, 2, Fk + 2 * cstride, fstride, u3, tw); }
+        else if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
         else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
       }
+    }
+    if constexpr (STAGED) {   // the slots are free again: start fetching the next plane's accumulators
+      if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) stage_plane<NF>(smF, Fk + g.PS, fstride, cstride);
+      cp_async_commit();
     }
   }
 }
@@ -376,15 +460,27 @@ __global__ void k_gather(const DevGrid g, const DevState s, const int *__restric
     (g)->launches++;                                                                   \
   } while (0)
 
+// unrolled-NF instantiations stage one plane of accumulators per thread in dynamic shared memory
+template <int R, int NF, bool IS_H>
+static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks) {
+  const size_t smem = EMM_CPA ? (size_t)3 * NF * 2 * 128 * sizeof(float4) : 0;
+  static bool configured = false;
+  if (!configured && smem > 48 * 1024) {
+    cudaFuncSetAttribute(k_update<R, NF, IS_H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = true;
+  }
+  k_update<R, NF, IS_H><<<grid, block, smem, st>>>(dg, s, kc, nchunks);
+}
+
 template <int R, bool IS_H>
 static void launch_update_nf(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks) {
   switch (s.nf) {
     case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
-    case 1: k_update<R, 1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
-    case 2: k_update<R, 2, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
-    case 3: k_update<R, 3, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
-    case 4: k_update<R, 4, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
-    case 5: k_update<R, 5, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
+    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
+    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
+    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
+    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
     default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
   }
 }
@@ -396,9 +492,17 @@ int launch_update(emm_grid *g, const DevState &s, int is_h) {
   int TX = 16;
   if (((quads + 31) / 32) * 32 <= ((quads + 15) / 16) * 16) TX = 32;
   if (quads <= 8) TX = 8;
+  {
+    static const char *env_tx = getenv("EMM_TX");        // tuning knob: quads per block row (8, 16, 32)
+    if (env_tx && atoi(env_tx) > 0) TX = atoi(env_tx);
+  }
   const int TY = 128 / TX;
   const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
   int kc = 16;
+  {
+    static const char *env_kc = getenv("EMM_KC");        // tuning knob: planes per z chunk
+    if (env_kc && atoi(env_kc) > 0) kc = atoi(env_kc);
+  }
   const int nchunks = (nk + kc - 1) / kc;
   dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
   if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");

@@ -11,7 +11,7 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libemm_b200.so")
+_SO = os.environ.get("EMM_B200_LIB") or os.path.join(_HERE, "libemm_b200.so")   # override: kernel-variant experiments
 _SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_air.cu", "emm_run.cu")]
 _HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
@@ -34,6 +34,8 @@ SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_grid_create", "emm_grid_destroy"
 def build(force=False, verbose=False):
     """nvcc -> libemm_b200.so in-tree, sm_100a only."""
     deps = _SRC + _HDR
+    if os.environ.get("EMM_B200_LIB"):
+        return _SO                       # an explicitly chosen (experiment) library is used as it is
     if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(os.path.getmtime(p) for p in deps):
         return _SO
     cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
