@@ -234,9 +234,9 @@ def run_gpu(args):
     g.profile(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
-    e0.record()
+    e0.record(g.stream)            # the library's stream (a torch stream owned by the binding)
     g.run_enqueue(K)
-    e1.record()
+    e1.record(g.stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     prof = g.profile_read()

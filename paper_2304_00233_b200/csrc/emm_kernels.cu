@@ -498,7 +498,13 @@ int launch_update(emm_grid *g, const DevState &s, int is_h) {
   }
   const int TY = 128 / TX;
   const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
+  // planes per z chunk: 16 on large grids; fewer on small ones so that the grid still holds ~8 blocks per SM
+  // (each block marches its planes one after the other, so a sparse grid is latency-bound)
   int kc = 16;
+  {
+    const long long xy = (long long)((quads + TX - 1) / TX) * ((dg.N2 + TY - 1) / TY) * s.nsrc;
+    while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 8) kc /= 2;
+  }
   {
     static const char *env_kc = getenv("EMM_KC");        // tuning knob: planes per z chunk
     if (env_kc && atoi(env_kc) > 0) kc = atoi(env_kc);

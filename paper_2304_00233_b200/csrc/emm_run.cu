@@ -2,6 +2,7 @@
 // Host code only prepares tables (fp64) and enqueues kernels; no field arithmetic happens on the host.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "emm_kernels.cuh"
@@ -24,6 +25,12 @@ struct Run {
   DevState ds{};
   DevRun dr{};
   int nrec_nodes = 0;
+  // one CUDA graph = check_every consecutive steps (captured once, replayed; the kernels read the step index
+  // from device memory, so replays need no parameter update)
+  cudaGraphExec_t chunk_graph = nullptr;
+  bool graph_failed = false;
+  long long kernels_per_chunk = 0;
+  ~Run() { if (chunk_graph) cudaGraphExecDestroy(chunk_graph); }
 };
 
 #define CU(call)                                                                                   \
@@ -359,7 +366,7 @@ static void cpml_tables(const emm_grid *g, int a, double fmax, std::vector<float
   }
 }
 
-static int enqueue_steps(emm_grid *g, int n) {
+static int enqueue_steps_raw(emm_grid *g, int n) {
   Run *R = g->run;
   int rc;
   for (int q = 0; q < n; ++q) {
@@ -374,6 +381,49 @@ static int enqueue_steps(emm_grid *g, int n) {
         (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
     if ((rc = launch_step_end(g, R->ds))) return rc;
     R->it_host++;
+  }
+  return 0;
+}
+
+// Whole chunks of check_every steps go through a CUDA graph (launch-bound on small grids: ~10 launches per
+// step); the first chunk (first-use set-up of the kernels), the ragged rest, and everything while per-kernel
+// profiling is on, are launched directly.
+static int enqueue_steps(emm_grid *g, int n) {
+  Run *R = g->run;
+  int rc;
+  static const bool no_graph = getenv("EMM_NO_GRAPH") != nullptr;
+  while (n > 0) {
+    const int ce = R->check_every;
+    const bool whole = !no_graph && !g->prof && !R->graph_failed && R->it_host >= ce && R->it_host % ce == 0 && n >= ce && R->it_host + ce <= R->table_steps;
+    if (!whole) {
+      const int m = std::min(n, ce - R->it_host % ce);
+      if ((rc = enqueue_steps_raw(g, m))) return rc;
+      n -= m;
+      continue;
+    }
+    if (!R->chunk_graph) {
+      cudaGraph_t graph = nullptr;
+      const int it_save = R->it_host;
+      const long long launches_save = g->launches;
+      if (cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); R->graph_failed = true; continue; }
+      rc = enqueue_steps_raw(g, ce);
+      const cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
+      R->it_host = it_save;
+      R->kernels_per_chunk = g->launches - launches_save;
+      g->launches = launches_save;
+      if (rc || e != cudaSuccess || !graph || cudaGraphInstantiate(&R->chunk_graph, graph, 0) != cudaSuccess) {
+        cudaGetLastError();
+        if (graph) cudaGraphDestroy(graph);
+        R->chunk_graph = nullptr;
+        R->graph_failed = true;          // fall back to direct launches (same kernels, same order)
+        continue;
+      }
+      cudaGraphDestroy(graph);
+    }
+    if (cudaGraphLaunch(R->chunk_graph, g->stream) != cudaSuccess) return fail(EMM_ECUDA, "cudaGraphLaunch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    g->launches += R->kernels_per_chunk;
+    R->it_host += ce;
+    n -= ce;
   }
   return 0;
 }

@@ -216,7 +216,11 @@ class Grid:
         n = self.workspace_bytes(nsrc, nfreq, max_steps, nrec)
         self._ws = None
         self._ws = torch.empty(n, dtype=torch.uint8, device=device)
-        stream = torch.cuda.current_stream(device).cuda_stream
+        torch.cuda.synchronize(device)
+        if getattr(self, "stream", None) is None:
+            # a torch stream of its own: the legacy default stream cannot be captured into CUDA graphs
+            self.stream = torch.cuda.Stream(device=device)
+        stream = self.stream.cuda_stream
         _chk(lib().emm_bind_device(self._h, C.c_void_p(self._ws.data_ptr()), n, C.c_void_p(stream)))
         self._plan = plan
 

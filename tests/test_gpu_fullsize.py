@@ -1,0 +1,193 @@
+"""GPU checks at BASELINE.json's FULL sizes, in the launch configuration bench.py times (`-m gpu`).
+
+The oracle cannot step a 43 M-node grid for thousands of steps inside a test, so at full size:
+  * configs[1] (cfg2) is compared with the oracle's converged result stored by tests/golden/make_goldens.py
+    (oracle only): step count exact, receivers within 1e-3;
+  * configs[3] (cfg4, the bench workload) is checked through properties that hold at any size, on sampled
+    nodes chosen on tile / chunk / quad boundaries of the launch configuration: one time step reproduces the
+    definition of the update (Eq. 8, 13, 14 with the library's own tables, fp64) and the fused DTFT equals the
+    sum of Eq. 25 over the steps taken;
+  * configs[4] (cfg5): the batched launch is bit-identical to running the sources one after the other.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from helpers import MU0, make_grid
+from paper_2304_00233_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def emm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2304_00233_b200 import emm as m
+    m.build()
+    return m
+
+
+def test_cfg2_full_size_converged_matches_oracle_golden(emm):
+    path = os.path.join(HERE, "golden", "cfg2_converged.json")
+    gold = json.load(open(path))
+    w = W.cfg2()
+    g = make_grid(emm, w)
+    info = g.info()
+    for k in ("N1", "N2", "N3", "k0"):
+        assert info[k] == gold["info"][k]
+    assert abs(info["dt"] / gold["info"]["dt"] - 1) < 1e-12
+    out, ns = g.run(w["sources"], w["freqs"], w["receivers"], w["run"])
+    ref = np.array(gold["receivers_re"]) + 1j * np.array(gold["receivers_im"])
+    assert int(ns[0]) == gold["nsteps"]                       # integer output: exact
+    for sl in (slice(0, 3), slice(3, 6)):
+        A, B = out[0][..., sl], ref[..., sl]
+        big = np.abs(B) > 1e-3 * np.abs(B).max()
+        assert (np.abs(A - B)[big] / np.abs(B)[big]).max() < 1e-3
+    # mirror symmetry of the layered model: Ex(+x) = Ex(-x) (free check)
+    ex = out[0, :, :, 0]
+    assert np.abs(ex - ex[:, ::-1]).max() < 1e-3 * np.abs(ex).max()
+
+
+def _sample_nodes(info, rd, rng, src, n=400, reach=44):
+    """interior nodes within `reach` cells of the source (where the young wave field lives), outside the CPML
+    slabs, biased to the boundaries of the launch tiles: 64-node x tiles / 4-node quads, 8-row y tiles,
+    16-plane z chunks"""
+    lo = np.array([info["box_lo3"] + rd + 1, info["box_lo2"] + rd, info["box_lo1"] + rd])
+    hi = np.array([info["box_hi3"] - rd, info["box_hi2"] - rd, info["box_hi1"] - rd])
+    lo, hi = np.maximum(lo, src - reach), np.minimum(hi, src + reach)
+    pts = rng.integers(lo, hi + 1, size=(n, 3))
+    edge_i = np.array([64 * m + d for m in range(1, info["N1"] // 64 + 1) for d in (-1, 0, 3, 4)])
+    edge_j = np.array([8 * m + d for m in range(2, info["N2"] // 8) for d in (-1, 0)])
+    edge_k = np.array([rd + 16 * m + d for m in range(1, (info["N3"] - 2 * rd) // 16 + 1) for d in (-1, 0)])
+    for col, edges, part in ((2, edge_i, slice(0, n // 4)), (1, edge_j, slice(n // 4, n // 2)), (0, edge_k, slice(n // 2, 3 * n // 4))):
+        ok = edges[(edges >= lo[col]) & (edges <= hi[col])]
+        assert len(ok) > 0
+        pts[part, col] = rng.choice(ok, n // 4)
+    return pts
+
+
+def _source_node(g):
+    return np.array([np.searchsorted(g.coords(2), 950.0), np.searchsorted(g.coords(1), 0.0), np.searchsorted(g.coords(0), 0.0)])
+
+
+def _curl(A, tabs, r, off, k, j, i):
+    """(D2A3 - D3A2, D3A1 - D1A3, D1A2 - D2A1) at node (k,j,i) in fp64, and the sum of |terms| of each component
+    (the scale of the fp32 rounding error); off = 0 for D-, 1 for D+ (Eq. 13-14)"""
+    def d(a, axis):
+        c = tabs[axis][(i, j, k)[axis]]
+        acc, mag = 0.0, 0.0
+        for m in range(2 * r):
+            o = m - r + off
+            kk, jj, ii = k + (o if axis == 2 else 0), j + (o if axis == 1 else 0), i + (o if axis == 0 else 0)
+            t = c[m] * float(a[kk, jj, ii])
+            acc += t
+            mag += abs(t)
+        return acc, mag
+    pairs = ((d(A[2], 1), d(A[1], 2)), (d(A[0], 2), d(A[2], 0)), (d(A[1], 0), d(A[0], 1)))
+    return [p[0] - q[0] for p, q in pairs], [p[1] + q[1] for p, q in pairs]
+
+
+@pytest.fixture(scope="module")
+def cfg4_run(emm):
+    """cfg4 at full size with a short wavelet so that the field is far from zero after ~100 steps"""
+    w = W.cfg4(emm.emm_nugrid)
+    g = make_grid(emm, w)
+    info = g.info()
+    fmax = 30.0                                       # wavelet centred on t0 = pi/30 s (~500 steps), still resolved by the grid
+    g.run_begin(w["sources"], w["freqs"], w["receivers"], dict(fixed_steps=1000, fmax=fmax))
+    g.run_steps(700)
+    return w, g, info
+
+
+def test_cfg4_full_size_one_step_equals_definition(emm, cfg4_run):
+    w, g, info = cfg4_run
+    r = w["grid"]["rd"]
+    names = ("E1", "E2", "E3", "H1", "H2", "H3")
+    old = {c: g.get(c) for c in names}
+    g.run_steps(1)
+    new = {c: g.get(c) for c in names}
+    ce = [g.get("CE%d" % (c + 1)) for c in range(3)]
+    tm = [g.fdcoef(a, 0) for a in range(3)]
+    tp = [g.fdcoef(a, 1) for a in range(3)]
+    dtmu = info["dt"] / MU0
+    rng = np.random.default_rng(11)
+    src = _source_node(g)
+    pts = _sample_nodes(info, r, rng, src)
+    # keep away from the source stencil (the injected term is checked by the small-grid parity tests)
+    pts = pts[np.abs(pts - src).max(axis=1) > 2 * r + 3]
+    Hold, Eold, Enew, Hnew = [old[c] for c in names[3:]], [old[c] for c in names[:3]], [new[c] for c in names[:3]], [new[c] for c in names[3:]]
+    checked, worst = 0, 0.0
+    for (k, j, i) in pts:
+        cH, mH = _curl(Hold, tm, r, 0, k, j, i)
+        cE, mE = _curl(Enew, tp, r, 1, k, j, i)
+        for c in range(3):
+            cec = float(ce[c][k, j, i])
+            e_ref, e_mag = float(Eold[c][k, j, i]) + cec * cH[c], abs(float(Eold[c][k, j, i])) + cec * mH[c]
+            h_ref, h_mag = float(Hold[c][k, j, i]) - dtmu * cE[c], abs(float(Hold[c][k, j, i])) + dtmu * mE[c]
+            for got, ref, mag in ((float(Enew[c][k, j, i]), e_ref, e_mag), (float(Hnew[c][k, j, i]), h_ref, h_mag)):
+                if mag > 1e-30:                          # the node carries signal (fp32 normal range)
+                    checked += 1
+                    worst = max(worst, abs(got - ref) / mag)
+    assert checked > 300, checked                        # (beyond the young wave front the field is still exactly 0)
+    # fp32 evaluation of a sum of ~4r+1 terms: error <= a few eps * sum|terms|  (eps = 6e-8)
+    assert worst < 2e-6, worst
+
+
+def test_cfg4_full_size_fused_dtft_equals_eq25(emm, cfg4_run):
+    w, g, info = cfg4_run
+    r = w["grid"]["rd"]
+    rng = np.random.default_rng(12)
+    pts = _sample_nodes(info, r, rng, _source_node(g), n=200)
+    kk, jj, ii = pts[:, 0], pts[:, 1], pts[:, 2]
+    comps = ("E1", "E3", "H2", "H3")
+    freqs = (0, 4)
+    ns, _ = g.run_steps(0)
+    it0 = int(ns[0])
+    before = {(c, f): g.get("F_" + c, ifreq=f)[kk, jj, ii].astype(np.complex128) for c in comps for f in freqs}
+    acc = {key: np.zeros(len(pts), dtype=np.complex128) for key in before}
+    w0 = 2 * np.pi * 1.0
+    nstep = 6
+    for q in range(nstep):
+        it = it0 + q
+        Hold = {c: g.get(c)[kk, jj, ii].astype(np.float64) for c in comps if c[0] == "H"}   # H before the step, t = it dt
+        g.run_steps(1)
+        Enew = {c: g.get(c)[kk, jj, ii].astype(np.float64) for c in comps if c[0] == "E"}   # E after the step, t = (it+1/2) dt
+        for f in freqs:
+            wp = (1 + 1j) * np.sqrt(2 * np.pi * w["freqs"][f] * w0)
+            for c in comps:
+                if c[0] == "H":
+                    acc[(c, f)] += Hold[c] * np.exp(1j * wp * it * info["dt"])
+                else:
+                    acc[(c, f)] += Enew[c] * np.exp(1j * wp * (it + 0.5) * info["dt"])
+    for (c, f), b in before.items():
+        after = g.get("F_" + c, ifreq=f)[kk, jj, ii].astype(np.complex128)
+        inc = after - b
+        sc = np.abs(acc[(c, f)]).max()
+        assert sc > 0
+        # fp32 accumulators: the increment is resolved to ~1e-7 of the accumulator itself
+        tol = 2e-6 * np.abs(after).max() + 1e-5 * sc
+        assert np.abs(inc - acc[(c, f)]).max() < tol, (c, f, np.abs(inc - acc[(c, f)]).max(), tol)
+
+
+def test_cfg5_full_size_batched_equals_sequential(emm):
+    w = W.cfg5(emm.emm_nugrid)
+    srcs = w["sources"][:4]
+    g = make_grid(emm, w)
+    rec = w["receivers"][::20]
+    fmax = np.pi / (60 * g.info()["dt"])
+    opts = dict(fixed_steps=150, fmax=fmax)
+    g.run_begin(srcs, w["freqs"], rec, dict(opts, batched=1))
+    ns, done = g.run_steps(150)
+    assert list(ns) == [150] * 4 and done
+    bat = [(g.get("E1", isrc=s), g.get("H2", isrc=s), g.get("F_E1", isrc=s, ifreq=1)) for s in range(4)]
+    for s in range(4):
+        assert np.abs(bat[s][0]).max() > 0 and np.all(np.isfinite(bat[s][2]))
+        g.run_begin(srcs[s:s + 1], w["freqs"], rec, dict(opts, batched=0))
+        g.run_steps(150)
+        for a, b in zip(bat[s], (g.get("E1"), g.get("H2"), g.get("F_E1", ifreq=1))):
+            assert np.array_equal(a, b)               # same kernels, same arithmetic: bit-identical
+    assert not np.array_equal(bat[0][0], bat[1][0])   # and the sources really differ
