@@ -39,8 +39,10 @@ def build_workload(args, nugrid):
         if args.aux_dx:
             kw["aux_dx"] = args.aux_dx
         w = W.build(args.workload, nugrid, **kw)
-        if args.workload == "cfg4" and args.nf:
-            w["freqs"] = w["freqs"][: args.nf]
+        if args.nf:
+            w["freqs"] = w["freqs"][: max(args.nf, 0)]       # --nf -1: pure update (no DTFT)
+            if args.nf < 0:
+                w["receivers"] = np.zeros((0, 3))
     else:
         w = W.build(args.workload, None, **({"rd": args.rd} if args.rd else {}))
     return w
@@ -251,6 +253,20 @@ def run_gpu(args):
     g.run_steps(1)
     for c in ("E1", "H2"):
         assert np.all(np.isfinite(g.get(c)))
+    batched = None
+    if nsrc > 1:
+        # configs[4]: the same K steps for ONE source alone = what running the sources one after the other costs
+        g.run_begin(srcs[:1], w["freqs"], w["receivers"], dict(fixed_steps=K + Wm + 4))
+        g.run_enqueue(Wm)
+        torch.cuda.synchronize()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(g.stream)
+        g.run_enqueue(K)
+        s1.record(g.stream)
+        torch.cuda.synchronize()
+        ms1 = s0.elapsed_time(s1)
+        batched = {"nsrc": nsrc, "ms_per_step_per_source_batched": ms / K / nsrc, "ms_per_step_per_source_sequential": ms1 / K,
+                   "speedup_vs_sequential": (ms1 / K) / (ms / K / nsrc)}
 
     if rank == 0:
         value = world * nsrc * N * K / (ms * 1e-3) / 1e9
@@ -281,7 +297,7 @@ def run_gpu(args):
                 "e2e": {"value": world * nsrc * N * K / t_e2e / 1e9, "unit": "Gcell-updates/s", "h2d_bytes_per_step": h2d / K,
                         "d2h_bytes_per_step": d2h / K, "seconds": t_e2e,
                         "what": "emm_model_set (host sigma -> device) + emm_run(fixed_steps=K) (tables up, receivers back)"},
-                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched,
                 "multi_gpu": "replicas only: every rank runs the whole workload, no collective on the data path"}
         print(json.dumps(line))
     if world > 1:
@@ -296,7 +312,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--rd", type=int, default=0, help="override the FD half length (cfg4: 3 = 6th order as configs[3]; 2 = 4th order)")
-    ap.add_argument("--nf", type=int, default=0, help="cfg4: keep only the first nf frequencies")
+    ap.add_argument("--nf", type=int, default=0, help="keep only the first nf frequencies; -1 = none (pure E/H update, no DTFT)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the cell counts (debugging only)")
     ap.add_argument("--aux-dx", type=float, default=0.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

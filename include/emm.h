@@ -128,7 +128,8 @@ int emm_model_set(emm_grid *g, const float *sigma_h, const float *sigma_v);
 
 /* One call: every source stepped to convergence (or fixed_steps).
  * out:    double complex [nsrc][nfreq][nrec][6] as (re,im) pairs: Green's functions Ex,Ey,Ez,Hx,Hy,Hz
- *         per unit dipole moment (Eq. 7); nsteps: [nsrc] steps executed.                             */
+ *         per unit dipole moment (Eq. 7); nsteps: [nsrc] steps executed.
+ * nfreq = 0 (pure time stepping, no DTFT) is accepted with fixed_steps > 0 and nrec = 0 (timing runs).  */
 int emm_run(emm_grid *g, const emm_src *src, int nsrc, const double *freqs_hz, int nfreq,
             const double *rec_xyz, int nrec, const emm_run_opts *opts, double *out, int *nsteps);
 

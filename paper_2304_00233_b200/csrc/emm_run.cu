@@ -377,7 +377,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
     if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                  // check-set part of L483
     if ((rc = launch_update(g, R->ds, 1))) return rc;                         // H part of L483 + L486-489
     if (g->top == EMM_TOP_AIR && (rc = launch_air(g, R->ds, R->dr, 1))) return rc;   // L491
-    if ((R->it_host + 1) % R->check_every == 0 &&
+    if (R->nf > 0 && (R->it_host + 1) % R->check_every == 0 &&
         (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
     if ((rc = launch_step_end(g, R->ds))) return rc;
     R->it_host++;
@@ -449,7 +449,9 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
   if (!g || !src || !freqs || !o || (nrec > 0 && !rec)) return fail(EMM_EINVAL, "emm_run_begin: null argument");
   if (!g->bound) return fail(EMM_ECUDA, "emm_run_begin: no device workspace bound");
   if (!g->have_model) return fail(EMM_EINVAL, "emm_run_begin: emm_model_set not called");
-  if (nsrc < 1 || nf < 1 || nrec < 0) return fail(EMM_EINVAL, "emm_run_begin: bad counts");
+  if (nsrc < 1 || nf < 0 || nrec < 0) return fail(EMM_EINVAL, "emm_run_begin: bad counts");
+  if (nf == 0 && (o->fixed_steps <= 0 || nrec > 0))   // pure time stepping (no DTFT): nothing to converge on or to return
+    return fail(EMM_EINVAL, "emm_run_begin: nfreq = 0 needs fixed_steps > 0 and no receivers");
   free_run(g);
   Run *R = new (std::nothrow) Run();
   if (!R) return fail(EMM_ENOMEM, "emm_run_begin: out of memory");
@@ -473,6 +475,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
       fhi = std::max(fhi, freqs[f]);
       if (freqs[f] < freqs[R->fmin]) R->fmin = f;
     }
+    if (nf == 0) fhi = 1.0;
     R->fmax = o->fmax > 0 ? o->fmax : 4.0 * std::sqrt(fhi * g->f0);         // [R8]
     R->beta = kPi * R->fmax * R->fmax;
     R->t0 = kPi / R->fmax;
@@ -497,6 +500,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     }
     // check set [R9]
     std::vector<int> chk;
+    if (nf > 0)
     for (int k = g->blo[2]; k <= g->bhi[2]; ++k) for (int j = g->blo[1]; j <= g->bhi[1]; ++j) for (int i = g->blo[0]; i <= g->bhi[0]; ++i) {
       const bool ei = i == g->blo[0] || i == g->bhi[0], ej = j == g->blo[1] || j == g->bhi[1], ek = k == g->blo[2] || k == g->bhi[2];
       const bool take = R->check_set == EMM_CHECK_FULL ? true : R->check_set == EMM_CHECK_FACES ? (ei || ej || ek) : (ei && ej && ek);

@@ -309,3 +309,32 @@ class Grid:
 
     def launch_count(self):
         return int(lib().emm_launch_count(self._h))
+
+
+# ---- multi-GPU: replicas only -------------------------------------------------------
+def shard_sources(nsrc, rank, world):
+    """Sources are independent problems (one source per MPI rank, no messages): source s runs on
+    rank s mod world."""
+    return list(range(rank, nsrc, world))
+
+
+def run_replicated(grid, sources, freqs, receivers, opts=None, group=None):
+    """Every rank runs its share of the sources on its own GPU through `grid.run`; the per-source results are
+    gathered on the host (all_gather_object).  No collective touches the data path."""
+    import torch.distributed as dist
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    mine = shard_sources(len(sources), rank, world)
+    out, ns = (grid.run([sources[s] for s in mine], freqs, receivers, opts) if mine
+               else (np.zeros((0, len(freqs), len(np.reshape(receivers, (-1, 3))), 6), np.complex128), np.zeros(0, np.int32)))
+    parts = [None] * world
+    if world > 1:
+        dist.all_gather_object(parts, (mine, out, ns), group=group)
+    else:
+        parts = [(mine, out, ns)]
+    full = np.zeros((len(sources),) + out.shape[1:], dtype=np.complex128)
+    steps = np.zeros(len(sources), dtype=np.int32)
+    for idx, o, n in parts:
+        for q, s in enumerate(idx):
+            full[s], steps[s] = o[q], n[q]
+    return full, steps
