@@ -102,10 +102,13 @@ __device__ __forceinline__ void dtft4_rt(float2 *F0, size_t fstride, float4 u, c
 }
 
 #ifndef EMM_MINB
-#define EMM_MINB 3
+#define EMM_MINB 0   /* 0 = choose per instantiation, see update_min_blocks */
 #endif
 #ifndef EMM_PF
 #define EMM_PF 1
+#endif
+#ifndef EMM_HOIST
+#define EMM_HOIST 1
 #endif
 #ifndef EMM_CPA
 #define EMM_CPA 1
@@ -151,8 +154,13 @@ __device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0
   }
 }
 
+// Blocks per SM the register allocation is aimed at.  Measured on B200 (profiles/r1_kernel_experiments.md): with
+// many frequencies (>= 4: 48+ KB of staged accumulators per block) two fat blocks per SM win -- no register cap,
+// and the unified L1 keeps ~100 KB for the neighbour rows; with fewer frequencies three blocks win.
+template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_MINB : (NF >= 4 ? 2 : 3); }
+
 template <int R, int NF, bool IS_H>
-__global__ void __launch_bounds__(128, EMM_MINB) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks) {
+__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
   const int src = blockIdx.z / nchunks, chunk = blockIdx.z - src * nchunks;
   if (s.done[src]) return;
@@ -259,6 +267,13 @@ __global__ void __launch_bounds__(128, EMM_MINB) k_update(const DevGrid g, const
     float cz[2 * R];
 #pragma unroll
     for (int m = 0; m < 2 * R; ++m) cz[m] = __ldg(tz + (size_t)k * 2 * R + m);
+#if EMM_HOIST
+    // issue the loads of the fields being updated (and dt/eps) together with the stencil loads: one dependent
+    // memory round trip per plane instead of two
+    float4 u1 = ld4(U1 + c0), u2 = ld4(U2 + c0), u3 = ld4(U3 + c0);
+    float4 e1 = zero4(), e2 = zero4(), e3 = zero4();
+    if (!IS_H) { e1 = ld4(g.ce[0] + c0); e2 = ld4(g.ce[1] + c0); e3 = ld4(g.ce[2] + c0); }
+#endif
     const float4 a1c = q1[R - O], a2c = q2[R - O];      // plane k of A1, A2
     const float4 a3c = ld4(A3 + c0);
 
@@ -317,7 +332,11 @@ __global__ void __launch_bounds__(128, EMM_MINB) k_update(const DevGrid g, const
 
     // curl (L338-346)
     const float4 c1 = sub4(D2A3, D3A2), c2 = sub4(D3A1, D1A3), c3 = sub4(D1A2, D2A1);
+#if !EMM_HOIST
     float4 u1 = ld4(U1 + c0), u2 = ld4(U2 + c0), u3 = ld4(U3 + c0);
+    float4 e1 = zero4(), e2 = zero4(), e3 = zero4();
+    if (!IS_H) { e1 = ld4(g.ce[0] + c0); e2 = ld4(g.ce[1] + c0); e3 = ld4(g.ce[2] + c0); }   // 0 where not updated
+#endif
     const bool dft = dft_xy && k >= g.blo[2] && k <= g.bhi[2];
     float2 *Fk = Fsrc + (size_t)(k - g.blo[2]) * g.PS + row;
     if constexpr (STAGED) cp_async_wait_all();        // this thread's copies of plane k have landed
@@ -334,7 +353,6 @@ __global__ void __launch_bounds__(128, EMM_MINB) k_update(const DevGrid g, const
       u3 = make_float4(fmaf(-m0, c3.x, u3.x), fmaf(-m1, c3.y, u3.y), fmaf(-m2, c3.z, u3.z), fmaf(-m3, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
     } else {
-      const float4 e1 = ld4(g.ce[0] + c0), e2 = ld4(g.ce[1] + c0), e3 = ld4(g.ce[2] + c0);   // 0 where not updated
       u1 = make_float4(fmaf(e1.x, c1.x, u1.x), fmaf(e1.y, c1.y, u1.y), fmaf(e1.z, c1.z, u1.z), fmaf(e1.w, c1.w, u1.w));
       u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
