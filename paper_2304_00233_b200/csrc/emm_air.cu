@@ -155,7 +155,7 @@ __global__ void k_air_filter_H(const AirArgs a, const float *__restrict__ kx, co
     (g)->launches++;                                                                   \
   } while (0)
 
-int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h) {
+int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st) {
   const int R = g->r;
   const int nlev = is_h ? R : R - 1;
   if (nlev <= 0) return 0;
@@ -172,7 +172,6 @@ int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h) {
   // writes Hx (node,half) + Hy (half,node)
   const int lat_in1[2] = {is_h ? 1 : 1, is_h ? 1 : 0}, lat_in2[2] = {0, 1};
   const int lat_out1[2] = {is_h ? 0 : 1, is_h ? 1 : 0}, lat_out2[2] = {is_h ? 1 : 0, is_h ? 0 : 1};
-  cudaStream_t st = g->stream;
   float2 *A = r.air, *B = r.air + (size_t)g->M1 * g->M2;
   const dim3 blk(128, 1, 1);
   const dim3 gM((g->M1 + 127) / 128, g->M2, 1), gN((g->N[0] + 127) / 128, g->N[1], nlev);

@@ -109,6 +109,8 @@ struct emm_grid {
   void *d_ws = nullptr;
   size_t ws_bytes = 0;
   cudaStream_t stream = nullptr;
+  cudaStream_t stream_b = nullptr;       // helper stream of the air-water boundary (created by emm_bind_device)
+  cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // fork/join events between the two streams
   bool bound = false;
   size_t fixed_bytes = 0;                // arena offset after the per-grid (model) region
   emm::DevGrid dg{};

@@ -13,6 +13,7 @@
 // neighbours come through L1/L2 (rows are 128-byte aligned).  The DTFT accumulators are streamed with
 // evict-first loads/stores: they are the dominant HBM traffic (96*nf of 84+96*nf bytes per node-step).
 #include <cstdio>
+#include <algorithm>
 #include <cstdlib>
 
 #include "emm_kernels.cuh"
@@ -160,9 +161,9 @@ __device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0
 template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_MINB : (NF >= 4 ? 2 : 3); }
 
 template <int R, int NF, bool IS_H>
-__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks) {
+__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
-  const int src = blockIdx.z / nchunks, chunk = blockIdx.z - src * nchunks;
+  const int src = blockIdx.z / nchunks, chunk = chunk0 + blockIdx.z - src * nchunks;   // this launch covers chunks [chunk0, chunk0 + nchunks)
   if (s.done[src]) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -480,30 +481,32 @@ __global__ void k_gather(const DevGrid g, const DevState s, const int *__restric
 
 // unrolled-NF instantiations stage one plane of accumulators per thread in dynamic shared memory
 template <int R, int NF, bool IS_H>
-static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks) {
+static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0) {
   const size_t smem = EMM_CPA ? (size_t)3 * NF * 2 * 128 * sizeof(float4) : 0;
   static bool configured = false;
   if (!configured && smem > 48 * 1024) {
     cudaFuncSetAttribute(k_update<R, NF, IS_H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
-  k_update<R, NF, IS_H><<<grid, block, smem, st>>>(dg, s, kc, nchunks);
+  k_update<R, NF, IS_H><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0);
 }
 
 template <int R, bool IS_H>
-static void launch_update_nf(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks) {
+static void launch_update_nf(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0) {
   switch (s.nf) {
-    case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
-    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
-    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
-    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
-    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
-    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks); break;
-    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks); break;
+    case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0); break;
+    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
+    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
+    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
+    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
+    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
+    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0); break;
   }
 }
 
-int launch_update(emm_grid *g, const DevState &s, int is_h) {
+// part: 0 = every z chunk, 1 = only the chunks next to the air-water plane (their stencils read the ghost planes),
+// 2 = all the others.  Parts 1 and 2 can run on different streams (emm_run.cu overlaps the boundary with part 2).
+int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st) {
   const DevGrid &dg = g->dg;
   const int quads = dg.P1 / 4;
   // block: TX quads wide (64 or 128 nodes), 128 threads; pick the width that wastes fewer lanes
@@ -527,23 +530,26 @@ int launch_update(emm_grid *g, const DevState &s, int is_h) {
     static const char *env_kc = getenv("EMM_KC");        // tuning knob: planes per z chunk
     if (env_kc && atoi(env_kc) > 0) kc = atoi(env_kc);
   }
-  const int nchunks = (nk + kc - 1) / kc;
+  const int nall = (nk + kc - 1) / kc;
+  const int nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);        // chunks whose stencils reach the ghost planes
+  const int chunk0 = part == 2 ? nsurf : 0;
+  const int nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
+  if (nchunks <= 0) return 0;
   dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
   if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
-  cudaStream_t st = g->stream;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (g->prof) {
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(EMM_ECUDA, "cudaEventCreate failed");
     cudaEventRecord(e0, st);
   }
   if (is_h) {
-    if (dg.r == 1) launch_update_nf<1, true>(dg, s, grid, block, st, kc, nchunks);
-    else if (dg.r == 2) launch_update_nf<2, true>(dg, s, grid, block, st, kc, nchunks);
-    else launch_update_nf<3, true>(dg, s, grid, block, st, kc, nchunks);
+    if (dg.r == 1) launch_update_nf<1, true>(dg, s, grid, block, st, kc, nchunks, chunk0);
+    else if (dg.r == 2) launch_update_nf<2, true>(dg, s, grid, block, st, kc, nchunks, chunk0);
+    else launch_update_nf<3, true>(dg, s, grid, block, st, kc, nchunks, chunk0);
   } else {
-    if (dg.r == 1) launch_update_nf<1, false>(dg, s, grid, block, st, kc, nchunks);
-    else if (dg.r == 2) launch_update_nf<2, false>(dg, s, grid, block, st, kc, nchunks);
-    else launch_update_nf<3, false>(dg, s, grid, block, st, kc, nchunks);
+    if (dg.r == 1) launch_update_nf<1, false>(dg, s, grid, block, st, kc, nchunks, chunk0);
+    else if (dg.r == 2) launch_update_nf<2, false>(dg, s, grid, block, st, kc, nchunks, chunk0);
+    else launch_update_nf<3, false>(dg, s, grid, block, st, kc, nchunks, chunk0);
   }
   if (g->prof) {
     cudaEventRecord(e1, st);

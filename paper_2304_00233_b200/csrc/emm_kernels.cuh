@@ -28,14 +28,14 @@ struct DevRun {
 };
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
-int launch_update(emm_grid *g, const DevState &s, int is_h);
+int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st);
 int launch_inject(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);
 int launch_step_end(emm_grid *g, const DevState &s);
 int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nrec_nodes);
 // air-water boundary (Eq. 17-21): ghost planes of Ex,Ey (is_h=0) or Hx,Hy (is_h=1)
-int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h);
+int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
 // model: effective medium (Eq. 26) -> min sigma (for Eq. 15) and dt/eps
 int launch_sigma_min(emm_grid *g, const float *d_sh, const float *d_sv, double *d_min);
 int launch_make_ce(emm_grid *g, const float *d_sh, const float *d_sv, double scale);

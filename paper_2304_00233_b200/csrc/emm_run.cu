@@ -154,6 +154,8 @@ extern "C" void emm_grid_destroy(emm_grid *g) {
   if (!g) return;
   free_run(g);
   for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
+  for (cudaEvent_t e : g->ev) if (e) cudaEventDestroy(e);
+  if (g->stream_b) cudaStreamDestroy(g->stream_b);
   if (g->have_plans) {
     if (g->plan_fwd) cufftDestroy(g->plan_fwd);
     if (g->plan_inv_e) cufftDestroy(g->plan_inv_e);
@@ -190,6 +192,14 @@ extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, voi
   g->d_ws = d_workspace;
   g->ws_bytes = bytes;
   g->stream = static_cast<cudaStream_t>(cuda_stream);
+  if (!g->stream_b) {
+    // highest priority: the boundary chain is short and on the critical path of the step; its blocks must get the
+    // next free SM slots while the bulk update (thousands of blocks on the main stream) is draining
+    int prio_lo = 0, prio_hi = 0;
+    CU(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    CU(cudaStreamCreateWithPriority(&g->stream_b, cudaStreamNonBlocking, prio_hi));
+    for (cudaEvent_t &e : g->ev) CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
   Arena A;
   A.base = static_cast<char *>(d_workspace);
   A.cap = bytes;
@@ -226,7 +236,7 @@ extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, voi
     const int batch[3] = {1, g->r - 1, g->r};
     for (int q = 0; q < 3; ++q) {
       if (batch[q] < 1) continue;
-      if (cufftSetStream(pl[q], g->stream) != CUFFT_SUCCESS || cufftSetWorkArea(pl[q], g->T.fft_ws[q]) != CUFFT_SUCCESS)
+      if (cufftSetStream(pl[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(pl[q], g->T.fft_ws[q]) != CUFFT_SUCCESS)
         return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
     }
   }
@@ -369,14 +379,44 @@ static void cpml_tables(const emm_grid *g, int a, double fmax, std::vector<float
 static int enqueue_steps_raw(emm_grid *g, int n) {
   Run *R = g->run;
   int rc;
+  static const bool no_overlap = getenv("EMM_NO_OVERLAP") != nullptr;
   for (int q = 0; q < n; ++q) {
     if (R->it_host >= R->table_steps) return fail(EMM_EINVAL, "run: step %d beyond the twiddle table (max_steps)", R->it_host);
+    cudaStream_t M = g->stream, B = g->stream_b;
     if ((rc = launch_inject(g, R->ds, R->dr))) return rc;                     // Alg. 1 L477 (before the update: same sum)
-    if ((rc = launch_update(g, R->ds, 0))) return rc;                         // L476-479 + E part of L483
-    if (g->top == EMM_TOP_AIR && (rc = launch_air(g, R->ds, R->dr, 0))) return rc;   // L481
-    if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                  // check-set part of L483
-    if ((rc = launch_update(g, R->ds, 1))) return rc;                         // H part of L483 + L486-489
-    if (g->top == EMM_TOP_AIR && (rc = launch_air(g, R->ds, R->dr, 1))) return rc;   // L491
+    if (g->top != EMM_TOP_AIR) {
+      if ((rc = launch_update(g, R->ds, 0, 0, M))) return rc;                 // L476-479 + E part of L483
+      if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                // check-set part of L483
+      if ((rc = launch_update(g, R->ds, 1, 0, M))) return rc;                 // H part of L483 + L486-489
+    } else if (g->prof || no_overlap) {
+      // one thing after the other (per-kernel timing, or EMM_NO_OVERLAP): the boundary still runs on its own stream
+      if ((rc = launch_update(g, R->ds, 0, 0, M))) return rc;
+      CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));
+      if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
+      CU(cudaEventRecord(g->ev[1], B)); CU(cudaStreamWaitEvent(M, g->ev[1], 0));
+      if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
+      if ((rc = launch_update(g, R->ds, 1, 0, M))) return rc;
+      CU(cudaEventRecord(g->ev[2], M)); CU(cudaStreamWaitEvent(B, g->ev[2], 0));
+      if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
+      CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));
+    } else {
+      // The boundary only feeds the z chunks next to the surface: those chunks and the FFT boundary form a short
+      // chain on the helper stream while the bulk of the grid is updated on the main stream (fork/join per step).
+      CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));      // fork (after the injection)
+      if ((rc = launch_update(g, R->ds, 0, 1, B))) return rc;                 // E, surface chunks
+      CU(cudaEventRecord(g->ev[1], B));
+      if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
+      if ((rc = launch_update(g, R->ds, 0, 2, M))) return rc;                 // E, bulk
+      CU(cudaEventRecord(g->ev[2], M));
+      CU(cudaStreamWaitEvent(M, g->ev[1], 0));                                // H bulk and the check set read surface-chunk E
+      if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
+      CU(cudaEventRecord(g->ev[4], M));
+      if ((rc = launch_update(g, R->ds, 1, 2, M))) return rc;                 // H, bulk
+      CU(cudaStreamWaitEvent(B, g->ev[2], 0)); CU(cudaStreamWaitEvent(B, g->ev[4], 0));
+      if ((rc = launch_update(g, R->ds, 1, 1, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
+      if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
+      CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));      // join
+    }
     if (R->nf > 0 && (R->it_host + 1) % R->check_every == 0 &&
         (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
     if ((rc = launch_step_end(g, R->ds))) return rc;
