@@ -40,33 +40,34 @@ __global__ void k_air_unpack(const AirArgs a, float *__restrict__ f1, float *__r
 // ---- non-uniform x-y: 4x4-point Lagrange interpolation to / from the auxiliary plane ----
 struct AuxTabs { const int *sx1, *sy1, *sx2, *sy2; const float *wx1, *wy1, *wx2, *wy2; };
 
-__global__ void k_air_toaux(const AirArgs a, const AuxTabs t, const float *__restrict__ f1, const float *__restrict__ f2,
-                            float2 *__restrict__ A) {
+// lattice -> auxiliary plane in two separable passes (4 taps each instead of 16 per point): x pass on the few
+// lattice rows (T[j][m], both packed components), then y pass over the whole plane, coalesced along m.
+__global__ void k_air_toaux_x(const AirArgs a, const AuxTabs t, const float *__restrict__ f1, const float *__restrict__ f2,
+                              float2 *__restrict__ T) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (m >= a.M1) return;
+  const float *p1 = f1 + (size_t)a.k0 * a.PS + (size_t)j * a.P1;
+  const float4 w1 = *reinterpret_cast<const float4 *>(t.wx1 + 4 * m);
+  const int i1 = t.sx1[m];
+  float v1 = fmaf(w1.x, p1[i1], fmaf(w1.y, p1[i1 + 1], fmaf(w1.z, p1[i1 + 2], w1.w * p1[i1 + 3]))), v2 = 0.f;
+  if (f2) {
+    const float *p2 = f2 + (size_t)a.k0 * a.PS + (size_t)j * a.P1;
+    const float4 w2 = *reinterpret_cast<const float4 *>(t.wx2 + 4 * m);
+    const int i2 = t.sx2[m];
+    v2 = fmaf(w2.x, p2[i2], fmaf(w2.y, p2[i2 + 1], fmaf(w2.z, p2[i2 + 2], w2.w * p2[i2 + 3])));
+  }
+  T[(size_t)j * a.M1 + m] = make_float2(v1, v2);
+}
+
+__global__ void k_air_toaux_y(const AirArgs a, const AuxTabs t, const float2 *__restrict__ T, float2 *__restrict__ A) {
   const int m = blockIdx.x * blockDim.x + threadIdx.x, n = blockIdx.y;
   if (m >= a.M1) return;
-  const float *p1 = f1 + (size_t)a.k0 * a.PS;
-  float v1 = 0.f, v2 = 0.f;
-  {
-    const int ix = t.sx1[m], iy = t.sy1[n];
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      float acc = 0.f;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) acc = fmaf(t.wx1[4 * m + c], p1[(size_t)(iy + b) * a.P1 + ix + c], acc);
-      v1 = fmaf(t.wy1[4 * n + b], acc, v1);
-    }
-  }
-  if (f2) {
-    const float *p2 = f2 + (size_t)a.k0 * a.PS;
-    const int ix = t.sx2[m], iy = t.sy2[n];
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      float acc = 0.f;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) acc = fmaf(t.wx2[4 * m + c], p2[(size_t)(iy + b) * a.P1 + ix + c], acc);
-      v2 = fmaf(t.wy2[4 * n + b], acc, v2);
-    }
-  }
+  const float4 w1 = *reinterpret_cast<const float4 *>(t.wy1 + 4 * n), w2 = *reinterpret_cast<const float4 *>(t.wy2 + 4 * n);
+  const int j1 = t.sy1[n], j2 = t.sy2[n];
+  const float v1 = fmaf(w1.x, T[(size_t)j1 * a.M1 + m].x, fmaf(w1.y, T[(size_t)(j1 + 1) * a.M1 + m].x,
+                   fmaf(w1.z, T[(size_t)(j1 + 2) * a.M1 + m].x, w1.w * T[(size_t)(j1 + 3) * a.M1 + m].x)));
+  const float v2 = fmaf(w2.x, T[(size_t)j2 * a.M1 + m].y, fmaf(w2.y, T[(size_t)(j2 + 1) * a.M1 + m].y,
+                   fmaf(w2.z, T[(size_t)(j2 + 2) * a.M1 + m].y, w2.w * T[(size_t)(j2 + 3) * a.M1 + m].y)));
   A[(size_t)n * a.M1 + m] = make_float2(v1, v2);
 }
 
@@ -102,16 +103,25 @@ __global__ void k_air_fromaux(const AirArgs a, const AuxTabs t, float *__restric
 }
 
 // ---- spectral filters ----
+// One thread filters 4 bins (independent loads in flight), bins are numbered row-major over the whole plane.
 // E: Laplace E = 0 above the surface (Eq. 21): level m is e^{-k_h h_m} times the surface spectrum.
 __global__ void k_air_filter_E(const AirArgs a, const float *__restrict__ kx, const float *__restrict__ ky,
                                const float2 *__restrict__ A, float2 *__restrict__ B) {
-  const int n1 = blockIdx.x * blockDim.x + threadIdx.x, n2 = blockIdx.y;
-  if (n1 >= a.M1) return;
-  const float kh = sqrtf(kx[n1] * kx[n1] + ky[n2] * ky[n2]);
-  const float2 v = A[(size_t)n2 * a.M1 + n1];
-  for (int m = 0; m < a.nlev; ++m) {
-    const float e = expf(-kh * a.h[m]) * a.scale;
-    B[(size_t)m * a.M1 * a.M2 + (size_t)n2 * a.M1 + n1] = make_float2(v.x * e, v.y * e);
+  const size_t MM = (size_t)a.M1 * a.M2, T = (size_t)gridDim.x * blockDim.x;
+  const size_t n0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float2 v[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) v[q] = n0 + q * T < MM ? A[n0 + q * T] : make_float2(0.f, 0.f);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const size_t n = n0 + q * T;
+    if (n >= MM) break;
+    const int n2 = (int)(n / a.M1), n1 = (int)(n - (size_t)n2 * a.M1);
+    const float kh = sqrtf(kx[n1] * kx[n1] + ky[n2] * ky[n2]);
+    for (int m = 0; m < a.nlev; ++m) {
+      const float e = expf(-kh * a.h[m]) * a.scale;
+      B[(size_t)m * MM + n] = make_float2(v[q].x * e, v[q].y * e);
+    }
   }
 }
 
@@ -120,31 +130,38 @@ __global__ void k_air_filter_E(const AirArgs a, const float *__restrict__ kx, co
 // Output plane = spectrum of Hx + i Hy.
 __global__ void k_air_filter_H(const AirArgs a, const float *__restrict__ kx, const float *__restrict__ ky,
                                const float2 *__restrict__ A, float2 *__restrict__ B) {
-  const int n1 = blockIdx.x * blockDim.x + threadIdx.x, n2 = blockIdx.y;
-  if (n1 >= a.M1) return;
-  const float qx = kx[n1], qy = ky[n2];
-  const float kh = sqrtf(qx * qx + qy * qy);
-  const bool nyx = ((a.M1 & 1) == 0) && n1 == a.M1 / 2, nyy = ((a.M2 & 1) == 0) && n2 == a.M2 / 2;
-  float2 gx = make_float2(0.f, 0.f), gy = make_float2(0.f, 0.f);   // i k/k_h [* e^{-i k d/2}]
-  if (kh > 0.f) {
-    if (!nyx) {
-      float sn = 0.f, cs = 1.f;
-      if (a.uniform) sincosf(-0.5f * qx * a.dx, &sn, &cs);
-      gx = make_float2(-sn * qx / kh, cs * qx / kh);
+  const size_t MM = (size_t)a.M1 * a.M2, T = (size_t)gridDim.x * blockDim.x;
+  const size_t n0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float2 v[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) v[q] = n0 + q * T < MM ? A[n0 + q * T] : make_float2(0.f, 0.f);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const size_t n = n0 + q * T;
+    if (n >= MM) break;
+    const int n2 = (int)(n / a.M1), n1 = (int)(n - (size_t)n2 * a.M1);
+    const float qx = kx[n1], qy = ky[n2];
+    const float kh = sqrtf(qx * qx + qy * qy);
+    const bool nyx = ((a.M1 & 1) == 0) && n1 == a.M1 / 2, nyy = ((a.M2 & 1) == 0) && n2 == a.M2 / 2;
+    float2 gx = make_float2(0.f, 0.f), gy = make_float2(0.f, 0.f);   // i k/k_h [* e^{-i k d/2}]
+    if (kh > 0.f) {
+      if (!nyx) {
+        float sn = 0.f, cs = 1.f;
+        if (a.uniform) sincosf(-0.5f * qx * a.dx, &sn, &cs);
+        gx = make_float2(-sn * qx / kh, cs * qx / kh);
+      }
+      if (!nyy) {
+        float sn = 0.f, cs = 1.f;
+        if (a.uniform) sincosf(-0.5f * qy * a.dy, &sn, &cs);
+        gy = make_float2(-sn * qy / kh, cs * qy / kh);
+      }
     }
-    if (!nyy) {
-      float sn = 0.f, cs = 1.f;
-      if (a.uniform) sincosf(-0.5f * qy * a.dy, &sn, &cs);
-      gy = make_float2(-sn * qy / kh, cs * qy / kh);
+    const float2 G = make_float2(gx.x - gy.y, gx.y + gy.x);             // gx + i gy
+    const float2 vg = make_float2(v[q].x * G.x - v[q].y * G.y, v[q].x * G.y + v[q].y * G.x);
+    for (int m = 0; m < a.nlev; ++m) {
+      const float e = expf(-kh * a.h[m]) * a.scale;
+      B[(size_t)m * MM + n] = make_float2(vg.x * e, vg.y * e);
     }
-  }
-  // G = gx + i gy
-  const float2 G = make_float2(gx.x - gy.y, gx.y + gy.x);
-  const float2 v = A[(size_t)n2 * a.M1 + n1];
-  const float2 vg = make_float2(v.x * G.x - v.y * G.y, v.x * G.y + v.y * G.x);
-  for (int m = 0; m < a.nlev; ++m) {
-    const float e = expf(-kh * a.h[m]) * a.scale;
-    B[(size_t)m * a.M1 * a.M2 + (size_t)n2 * a.M1 + n1] = make_float2(vg.x * e, vg.y * e);
   }
 }
 
@@ -188,12 +205,16 @@ int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaSt
       t.sy1 = g->T.ta_start[1][lat_in1[1]]; t.wy1 = g->T.ta_w[1][lat_in1[1]];
       t.sx2 = g->T.ta_start[0][lat_in2[0]]; t.wx2 = g->T.ta_w[0][lat_in2[0]];
       t.sy2 = g->T.ta_start[1][lat_in2[1]]; t.wy2 = g->T.ta_w[1][lat_in2[1]];
-      k_air_toaux<<<gM, blk, 0, st>>>(a, t, f_in1, f_in2, A);
+      float2 *Tx = r.air + (size_t)(1 + R) * g->M1 * g->M2;        // [N2][M1] x-interpolated lattice rows
+      k_air_toaux_x<<<dim3((g->M1 + 127) / 128, g->N[1], 1), blk, 0, st>>>(a, t, f_in1, f_in2, Tx);
+      EMM_LAUNCH_CHECK(g, "k_air_toaux_x");
+      k_air_toaux_y<<<gM, blk, 0, st>>>(a, t, Tx, A);
     }
     EMM_LAUNCH_CHECK(g, "k_air_pack");
     if (cufftExecC2C(g->plan_fwd, A, A, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C forward failed");
-    if (is_h) k_air_filter_H<<<gM, blk, 0, st>>>(a, g->T.kx, g->T.ky, A, B);
-    else k_air_filter_E<<<gM, blk, 0, st>>>(a, g->T.kx, g->T.ky, A, B);
+    const unsigned gF = (unsigned)(((size_t)g->M1 * g->M2 + 4 * 256 - 1) / (4 * 256));
+    if (is_h) k_air_filter_H<<<gF, 256, 0, st>>>(a, g->T.kx, g->T.ky, A, B);
+    else k_air_filter_E<<<gF, 256, 0, st>>>(a, g->T.kx, g->T.ky, A, B);
     EMM_LAUNCH_CHECK(g, "k_air_filter");
     if (cufftExecC2C(is_h ? g->plan_inv_h : g->plan_inv_e, B, B, CUFFT_INVERSE) != CUFFT_SUCCESS)
       return fail(EMM_ECUDA, "cufftExecC2C inverse failed");

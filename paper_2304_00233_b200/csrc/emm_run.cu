@@ -130,7 +130,8 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps,
   r.status = A.take<int>(nsrc);
   r.rec_idx = A.take<int>((size_t)6 * nrec * np3);
   r.rec_val = A.take<float2>((size_t)nsrc * nf * 6 * nrec * np3);
-  if (g->top == EMM_TOP_AIR) r.air = A.take<float2>((size_t)(1 + g->r) * g->M1 * g->M2);
+  if (g->top == EMM_TOP_AIR)   // FFT planes [1 + r][M2][M1] + (non-uniform x-y) the x-interpolated rows [N2][M1]
+    r.air = A.take<float2>((size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
 }
 
 template <class T>
