@@ -65,6 +65,11 @@ typedef struct {
   double fmax;     /* source wavelet parameter; <=0 => 4*sqrt(max f * f0)                              */
   int batched;     /* 1: advance all sources in one launch per kernel (they share grid and
                       coefficients); 0: one source after the other                                     */
+  int dtft_every;  /* m > 1: DTFT decimation -- only every m-th term of the sums of Eq. 25 is taken for the fields
+                      and J' (the small check set keeps every term: the stopping rule does not depend on m).  The fictitious wave field is band-limited far below 1/(2 m dt)
+                      (dt is set by the fastest cell, L251-260), so G = F/J' changes by ~1e-9 while the dominant
+                      accumulator traffic drops by (1 - 1/m).  0, 1: every step, as the paper does (L454);
+                      < 0: the largest safe m = floor(1/(dt (3 fmax + 2 sqrt(max f * f0))))                      */
 } emm_run_opts;
 
 /* integer grid facts for emm_grid_info(): */

@@ -182,7 +182,7 @@ typedef struct {
   double *freqs; cplx *wp;         /* omega' = (1+i) sqrt(omega omega0), Eq. 4                  */
   int fmin;                        /* index of the lowest frequency (L387)                      */
   double fmax, beta, t0;
-  int max_steps, fixed_steps, check_every, check_set, sparse; double tol;
+  int max_steps, fixed_steps, check_every, check_set, sparse, dtft_every; double tol;
   size_t ndft; size_t *dft_idx;    /* sorted node indices carrying DFT accumulators             */
   size_t nchk; size_t *chk_idx;
   int np;                          /* interpolation points per axis, max(2r,4) (c-6)            */
@@ -555,6 +555,7 @@ int emmo_run_begin(emmo_grid *g, const emmo_src *src, int nsrc, const double *fr
   R->tol = o->tol > 0 ? o->tol : 1e-6;
   R->check_every = o->check_every > 0 ? o->check_every : 100;
   R->check_set = o->check_set; R->sparse = o->sparse_dft;
+  R->dtft_every = o->dtft_every > 1 ? o->dtft_every : 1;      /* < 0: automatic, set once fmax is known */
   if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMMO_EINVAL, "run_begin: bad check_set"); }
   R->freqs = (double *)malloc(sizeof(double) * nf); R->wp = (cplx *)malloc(sizeof(cplx) * nf);
   if (!R->freqs || !R->wp) { free_run(g); return fail(EMMO_ENOMEM, "run_begin: out of memory"); }
@@ -568,6 +569,11 @@ int emmo_run_begin(emmo_grid *g, const emmo_src *src, int nsrc, const double *fr
   }
   R->fmax = o->fmax > 0 ? o->fmax : 4.0 * sqrt(fhi * g->f0);        /* [R8] */
   R->beta = M_PI * R->fmax * R->fmax; R->t0 = M_PI / R->fmax;
+  if (o->dtft_every < 0) {  /* largest m whose sampling rate 1/(m dt) still clears the wavelet band (3 fmax) plus the
+                               band the DTFT looks at (sqrt(f f0)) twice over: aliasing below ~1e-9 */
+    double m = floor(1.0 / (g->dt * (3.0 * R->fmax + 2.0 * sqrt(fhi * g->f0))));
+    R->dtft_every = m > 1 ? (m > 1000 ? 1000 : (int)m) : 1;
+  }
   R->np = 2 * r > 4 ? 2 * r : 4;
   /* CPML tables; v_ref per face = fastest padded cell inside that slab [R5] */
   for (int a = 0; a < 3; a++) {
@@ -873,12 +879,14 @@ static int airwave_bc_update_H(const emmo_grid *g, srcstate *S) {
 /* ---- DTFT (Eq. 25, listing L361-381) with the time levels of [R6] ---- */
 static void dtft_emf(const emmo_grid *g, const runstate *R, srcstate *S, int it, double st) {
   const int nf = R->nf;
+  const int fields = (it % R->dtft_every) == 0;   /* decimation: fields and J' take every m-th term; the check set
+                                                     (cheap) takes every term so that the stopping rule is unchanged */
   for (int f = 0; f < nf; f++) {
     cplx twH = cexp(I * R->wp[f] * ((double)it * g->dt));          /* H and J at t = it dt       */
     cplx twE = cexp(I * R->wp[f] * (((double)it + 0.5) * g->dt));  /* updated E at (it+1/2) dt   */
-    S->Jw[f] += st * twH;
+    if (fields) S->Jw[f] += st * twH;
 #pragma omp parallel for schedule(static)
-    for (size_t p = 0; p < R->ndft; p++) {
+    for (size_t p = 0; p < (fields ? R->ndft : 0); p++) {
       size_t t = R->dft_idx[p];
       for (int c = 0; c < 3; c++) {
         S->F[((size_t)c * nf + f) * R->ndft + p] += S->E[c][t] * twE;

@@ -61,6 +61,9 @@ typedef struct {
   int check_set;    /* EMMO_CHECK_*                                             */
   double fmax;      /* wavelet parameter; <=0 => 4*sqrt(max f * f0)             */
   int sparse_dft;   /* 1: accumulate only on receiver stencils (+check set)     */
+  int dtft_every;   /* m > 1: take only every m-th term of the DTFT sums (Eq. 25) of the fields and of J'; the
+                       check set keeps every term, so the stopping rule does not depend on m; 0, 1: every step;
+                       < 0: the largest safe m = floor(1/(dt (3 fmax + 2 sqrt(max f * f0))))                   */
 } emmo_run_opts;
 
 /* grid info indices for emmo_grid_info(): ints */

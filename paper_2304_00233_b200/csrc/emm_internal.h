@@ -70,6 +70,7 @@ struct DevState {              // per run; arrays carry a leading source dimensi
   int *it;                     // device step counter
   int *done;                   // [nsrc]
   int nf, nsrc;
+  int dft_every;               // DTFT decimation: accumulate only when it % dft_every == 0 (1 = every step)
 };
 
 struct DevTables {             // device pointers of the per-grid region

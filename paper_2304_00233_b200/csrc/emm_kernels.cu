@@ -211,7 +211,8 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 
   // DTFT bookkeeping
   const int nf = s.nf;
-  const bool dft_xy = (nf > 0) && (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);
+  const bool dft_xy = (nf > 0) && (it % s.dft_every == 0) &&        // DTFT decimation: this step contributes or not
+                      (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);
   const size_t fstride = (size_t)6 * g.NZB * g.PS;      // float2 elements between frequencies
   float2 *Fsrc = s.F + (size_t)src * nf * fstride + (size_t)(IS_H ? 3 : 0) * g.NZB * g.PS;
   const float2 *twp = (IS_H ? s.twH : s.twE) + (size_t)it * nf;

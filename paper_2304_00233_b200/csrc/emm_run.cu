@@ -18,7 +18,7 @@ struct Run {
   int fmin = 0;
   double fmax = 0, beta = 0, t0 = 0, tol = 1e-6;
   int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
-  int it_min = 0, it_host = 0, table_steps = 0;
+  int it_min = 0, it_host = 0, table_steps = 0, dtft_every = 1;
   std::vector<double> wav;                  // s(it*dt) rounded to fp32 (what the device injects)
   std::vector<Stencil1> rst;                // [nrec][6][3]
   std::vector<int> nsteps, done, status;
@@ -506,6 +506,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     R->tol = o->tol > 0 ? o->tol : 1e-6;
     R->check_every = o->check_every > 0 ? o->check_every : 100;
     R->check_set = o->check_set;
+    R->dtft_every = o->dtft_every > 1 ? o->dtft_every : 1;
     if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
     R->table_steps = (R->fixed_steps ? R->fixed_steps : R->max_steps) + 1;
     double fhi = 0;
@@ -518,6 +519,10 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     }
     if (nf == 0) fhi = 1.0;
     R->fmax = o->fmax > 0 ? o->fmax : 4.0 * std::sqrt(fhi * g->f0);         // [R8]
+    if (o->dtft_every < 0) {   // automatic: the largest m whose sampling rate clears the wavelet band
+      const double m = std::floor(1.0 / (g->dt * (3.0 * R->fmax + 2.0 * std::sqrt(fhi * g->f0))));
+      R->dtft_every = m > 1 ? (m > 1000 ? 1000 : (int)m) : 1;
+    }
     R->beta = kPi * R->fmax * R->fmax;
     R->t0 = kPi / R->fmax;
     R->np = std::max(2 * r, 4);
@@ -551,6 +556,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     Arena A;
     A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
     layout_run(g, A, nsrc, nf, R->table_steps, nrec, chk.size(), R->ds, R->dr);
+    R->ds.dft_every = R->dtft_every;
     if (A.overflow) { size_t need = A.off; free_run(g); return fail(EMM_ENOMEM, "emm_run_begin: workspace too small (%zu bytes needed)", need); }
     // zero the whole run region (fields, psi, accumulators, flags)
     CU(cudaMemsetAsync(static_cast<char *>(g->d_ws) + g->fixed_bytes, 0, A.off - g->fixed_bytes, g->stream));
@@ -694,7 +700,7 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
   for (int s = 0; s < R->nsrc; ++s)
     for (int f = 0; f < nf; ++f) {
       std::complex<double> Jw = 0;                                             // J'(omega') = sum s[it] e^{i w' it dt}
-      for (int it = 0; it < R->nsteps[s]; ++it) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
+      for (int it = 0; it < R->nsteps[s]; it += R->dtft_every) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
       const std::complex<double> sc = std::sqrt(-I * 2.0 * kPi * R->freqs[f] / (2 * g->w0));   // Eq. 7a, principal root
       for (int q = 0; q < R->nrec; ++q)
         for (int c = 0; c < 6; ++c) {
@@ -777,7 +783,7 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
     const std::complex<double> I(0, 1);
     for (int f = 0; f < R->nf; ++f) {
       std::complex<double> Jw = 0;
-      for (int it = 0; it < R->nsteps[isrc]; ++it) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
+      for (int it = 0; it < R->nsteps[isrc]; it += R->dtft_every) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
       o[f] = Jw;
     }
     return 0;

@@ -40,7 +40,7 @@ def _group_errors(ga, gb, s):
     return d, n, grp
 
 
-def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, batched=0):
+def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, batched=0, dtft_every=0):
     """Field parity at four checkpoints up to `nsteps` (200 in north_star).
 
     Tolerance: relative L2 <= 1e-5 per field wherever the field still
@@ -49,7 +49,7 @@ def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, bat
     curl-free residual of ~1e-8 of the peak that never radiates away, while on these small test grids the
     wave itself has left through the CPML long before step 200."""
     sources = sources or w["sources"]
-    opts = dict(fixed_steps=nsteps, batched=batched)
+    opts = dict(fixed_steps=nsteps, batched=batched, dtft_every=dtft_every)
     ga, gb = make_grid(emm, w), make_grid(oracle, w)
     assert abs(ga.info()["dt"] / gb.info()["dt"] - 1) < 1e-12
     for c in ("CE1", "CE2", "CE3"):
@@ -131,6 +131,21 @@ def test_fields_batched_sources(emm, oracle):
     srcs = [((-180.0 + 170.0 * i, 40.0 * i, 950.0), (1.0, 0.3 * i, 0.1)) for i in range(3)]
     w["receivers"] = _small_receivers()
     _field_parity(emm, oracle, w, 120, sources=srcs, batched=1)
+
+
+@pytest.mark.parametrize("m", [3, -1])
+def test_dtft_decimation_matches_oracle(emm, oracle, m):
+    """SURVEY 8f rank 1: only every m-th term of Eq. 25 is accumulated (m = -1: the automatic safe value);
+    fields, accumulators, J', receivers and the converged step count follow the oracle's identical rule."""
+    w = W.cfg2(nx=36, nz=24, dx=100.0, rd=2, nb=8)
+    _field_parity(emm, oracle, w, 200, dtft_every=m)
+    opts = dict(tol=1e-6, check_every=100, dtft_every=m)
+    ga, gb = make_grid(emm, w), make_grid(oracle, w)
+    oa, nsa = ga.run(w["sources"], w["freqs"], w["receivers"], opts)
+    ob, nsb = gb.run(w["sources"], w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
+    assert list(nsa) == list(nsb) and nsa[0] > 0
+    big = np.abs(ob) > 1e-3 * np.abs(ob).max()
+    assert (np.abs(oa - ob)[big] / np.abs(ob)[big]).max() < 1e-3
 
 
 def test_converged_run_matches_oracle_steps_and_receivers(emm, oracle):

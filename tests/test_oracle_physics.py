@@ -278,3 +278,29 @@ def test_convergence_rule(oracle):
     # sparse-DFT mode gives pointwise identical receivers
     out5, ns5 = g.run(w["sources"], w["freqs"], rec, dict(tol=1e-6, check_every=50, sparse_dft=1))
     assert ns5[0] == ns[0] and np.array_equal(out5, out)
+
+
+# ---- DTFT decimation -----------------------------------
+def test_dtft_decimation_leaves_green_functions_unchanged(oracle, small_ws):
+    """Taking only every m-th term of the sums of Eq. 25 (for the fields AND J') aliases the spectrum at multiples
+    of 1/(m dt); the wavelet has nothing there (Gaussian, fmax << 1/(m dt)), so G = F/J' moves by ~1e-9 while
+    the work of the DTFT drops m-fold.  A careless version (decimating F but not J', or forgetting the
+    half-step of E) would be off by O(1) or by |w'| dt / 2."""
+    w, rec, ref, base = small_ws
+    # dt = 0.0132 s, fmax = 4 Hz: the automatic rule floor(1/(dt (3 fmax + 2 sqrt(f f0)))) gives m = 5
+    for m, bound in ((2, 1e-9), (5, 1e-9), (-1, 1e-9), (16, None)):
+        o, ns = make_grid(oracle, w).run(w["sources"], w["freqs"], rec, dict(fixed_steps=500, dtft_every=m))
+        assert ns[0] == 500
+        err = np.abs(o[0, 0] - base).max() / np.abs(base).max()
+        if bound:
+            assert err < bound, (m, err)
+        else:
+            assert err > 1e-2, (m, err)     # sampling at 4.7 Hz aliases the 4 Hz wavelet: the rule matters
+    # a marine model with the air boundary, run to convergence with and without decimation
+    wm = W.cfg2(nx=24, nz=16, dx=100.0, rd=2, nb=8)
+    g = make_grid(oracle, wm)
+    a, na = g.run(wm["sources"], wm["freqs"], wm["receivers"], dict(tol=1e-6, check_every=100, sparse_dft=1))
+    b, nb_ = g.run(wm["sources"], wm["freqs"], wm["receivers"], dict(tol=1e-6, check_every=100, sparse_dft=1, dtft_every=4))
+    big = np.abs(a) > 1e-3 * np.abs(a).max()
+    assert (np.abs(a - b)[big] / np.abs(a)[big]).max() < 1e-4      # both stop at ~1e-6 relative change
+    assert abs(int(na[0]) - int(nb_[0])) <= 100
