@@ -124,6 +124,7 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_2() { asm volatile("cp.async.wait_group 2;" ::: "memory"); }
 
 // Accumulators of one plane staged in shared memory: slot j of thread t sits at sm[j*128 + t] (conflict-free
 // LDS.128).  Each thread only ever touches its own slots, so no block barrier is needed: the thread waits for
@@ -138,6 +139,17 @@ __device__ __forceinline__ void stage_plane(float4 *sm, const float2 *Fk, size_t
       cp_async16(sm + ((c * NF + f) * 2 + 0) * 128, p);
       cp_async16(sm + ((c * NF + f) * 2 + 1) * 128, p + 4);
     }
+}
+
+// one component only (the three components are separate commit groups, see the kernel)
+template <int NF>
+__device__ __forceinline__ void stage_component(float4 *sm, int c, const float2 *Fkc, size_t fstride) {
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    const float *p = reinterpret_cast<const float *>(Fkc + f * fstride);
+    cp_async16(sm + ((c * NF + f) * 2 + 0) * 128, p);
+    cp_async16(sm + ((c * NF + f) * 2 + 1) * 128, p + 4);
+  }
 }
 
 // DTFT of one component from the staged accumulators: F[f] += u * tw[f], result streamed back to global
@@ -234,10 +246,16 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   extern __shared__ float4 smF_all[];
   float4 *smF = smF_all + (threadIdx.y * blockDim.x + threadIdx.x);
   const size_t cstride = (size_t)g.NZB * g.PS;
+  // The accumulators of the three components are three commit groups, consumed in issue order and re-issued for
+  // the next plane as soon as their slots are free: every copy gets almost a whole plane of lead time, and
+  // `cp.async.wait_group 2` before each use leaves exactly the two younger groups pending.
   if constexpr (STAGED) {
-    if (dft_xy && kbeg >= g.blo[2] && kbeg <= g.bhi[2])
-      stage_plane<NF>(smF, Fsrc + (size_t)(kbeg - g.blo[2]) * g.PS + row, fstride, cstride);
-    cp_async_commit();
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      if (dft_xy && kbeg >= g.blo[2] && kbeg <= g.bhi[2])
+        stage_component<NF>(smF, c, Fsrc + (size_t)(kbeg - g.blo[2]) * g.PS + row + c * cstride, fstride);
+      cp_async_commit();
+    }
   }
 
   for (int k = kbeg; k < kend; ++k) {
@@ -341,12 +359,20 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 #endif
     const bool dft = dft_xy && k >= g.blo[2] && k <= g.bhi[2];
     float2 *Fk = Fsrc + (size_t)(k - g.blo[2]) * g.PS + row;
-    if constexpr (STAGED) cp_async_wait_all();        // this thread's copies of plane k have landed
+    // one component: wait for its staged accumulators, add u * twiddle, stream out, refill the slots for plane k+1
+    auto dtft_staged_component = [&](int c, float4 u) {
+      cp_async_wait_2();
+      if (dft) dtft4_staged<NF>(smF, c, Fk + c * cstride, fstride, u, tw);
+      if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2])
+        stage_component<NF>(smF, c, Fk + g.PS + c * cstride, fstride);
+      cp_async_commit();
+    };
 
     if (IS_H) {
-      if (dft) {        // old H sits at t = it*dt, the time level of J (Eq. 8; [R6])
-        if constexpr (STAGED) { dtft4_staged<NF>(smF, 0, Fk, fstride, u1, tw); dtft4_staged<NF>(smF, 1, Fk + cstride, fstride, u2, tw); dtft4_staged<NF>(smF, 2, Fk + 2 * cstride, fstride, u3, tw); }
-        else if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
+      // old H sits at t = it*dt, the time level of J (Eq. 8; [R6])
+      if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
+      else if (dft) {
+        if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
         else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
       }
       const float m0 = upd[0] ? g.dtmu : 0.f, m1 = upd[1] ? g.dtmu : 0.f, m2 = upd[2] ? g.dtmu : 0.f, m3 = upd[3] ? g.dtmu : 0.f;
@@ -359,15 +385,12 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
-      if (dft) {        // new E sits at t = (it+1/2)*dt [R6]
-        if constexpr (STAGED) { dtft4_staged<NF>(smF, 0, Fk, fstride, u1, tw); dtft4_staged<NF>(smF, 1, Fk + cstride, fstride, u2, tw); dtft4_staged<NF>(smF, 2, Fk + 2 * cstride, fstride, u3, tw); }
-        else if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
+      // new E sits at t = (it+1/2)*dt [R6]
+      if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
+      else if (dft) {
+        if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
         else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
       }
-    }
-    if constexpr (STAGED) {   // the slots are free again: start fetching the next plane's accumulators
-      if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) stage_plane<NF>(smF, Fk + g.PS, fstride, cstride);
-      cp_async_commit();
     }
   }
 }

@@ -6,7 +6,7 @@ in these files comes from the CUDA path.  The oracle runs in sparse-DFT mode (ac
 receiver stencils and the check set: pointwise identical values, see test_convergence_rule).
 
     python tests/golden/make_goldens.py cfg2            # ~15 min on 8 cores
-    python tests/golden/make_goldens.py cfg3 [max_steps]  # hours
+    python tests/golden/make_goldens.py cfg3 0 100        # configs[2] with aux_dx = 100 m, to convergence: ~2 h
 
 Output: tests/golden/<name>_converged.json with the inputs' SHA-256, nsteps, delta and the complex receivers.
 """
@@ -41,6 +41,9 @@ def main():
     name = sys.argv[1]
     kw = {}
     fixed = int(sys.argv[2]) if len(sys.argv) > 2 else 0
+    aux_dx = float(sys.argv[3]) if len(sys.argv) > 3 else 0.0
+    if aux_dx:
+        kw["aux_dx"] = aux_dx          # coarser auxiliary plane: the oracle's plain FFT makes the 25 m default take ~10 h on cfg3
     w = W.build(name, O.nugrid, **kw)
     g = O.Grid(w["x"], w["y"], w["z"], **w["grid"])
     g.model_set(w["sigma_h"], w.get("sigma_v"))
@@ -60,7 +63,7 @@ def main():
            "delta": [float(v) for v in g.get("DELTA")], "seconds": time.time() - t,
            "receivers_re": out[0].real.tolist(), "receivers_im": out[0].imag.tolist(),
            "written_by": "tests/golden/make_goldens.py %s (oracle only)" % " ".join(sys.argv[1:])}
-    suffix = "_converged" if not fixed else "_%dsteps" % fixed
+    suffix = ("_converged" if not fixed else "_%dsteps" % fixed) + ("_aux%g" % aux_dx if aux_dx else "")
     with open(os.path.join(HERE, name + suffix + ".json"), "w") as f:
         json.dump(res, f)
     print("wrote", name + suffix + ".json", "nsteps", res["nsteps"])
