@@ -52,7 +52,10 @@ typedef struct {
 
 typedef struct {
   double pos[3]; /* x,y,z of the point dipole (anywhere inside the model, L640)                        */
-  double dir[3]; /* polarisation of the electric current J (normalised internally)                     */
+  double dir[3]; /* polarisation of the dipole (normalised internally)                                 */
+  int type;      /* 0: electric dipole J (Eq. 8, inject_electric_src_fwd L457); 1: magnetic dipole M
+                    (Eq. 8, inject_magnetic_src_fwd).  Outputs for type 1 are G^EM = E/M and G^HM = H/M
+                    (same transformation as Eq. 7: E' = E, M' = M, H' = sqrt(-i w/2 w0) H, Eq. 4)            */
 } emm_src;
 
 typedef struct {

@@ -168,6 +168,7 @@ typedef struct {           /* one source's time-stepping state */
                               0:D1H3 1:D1H2 (x slabs) 2:D2H3 3:D2H1 (y) 4:D3H2 5:D3H1 (z)       */
   double *psiH[6];         /* of the 6 E-derivatives: 0:D1E3 1:D1E2 2:D2E3 3:D2E1 4:D3E2 5:D3E1 */
   int nsn[3]; size_t *sidx[3]; double *sw[3]; /* source nodes and weights W_c (c-6)            */
+  int magnetic;            /* 1: the weights live on the H lattices and M is injected into H   */
   cplx *F;                 /* [(c*nf+f)*ndft + p], c = 0..5 (E1..H3)                            */
   cplx *Jw;                /* [nf] J'(omega')                                                   */
   cplx *Cnow, *Cprev;      /* [6][nchk] check-set accumulators, lowest frequency               */
@@ -659,12 +660,15 @@ int emmo_run_begin(emmo_grid *g, const emmo_src *src, int nsrc, const double *fr
     /* source weights W_c = dir_c * wx wy wz / V_node on the component's own lattice [R7] */
     double dn = sqrt(src[s].dir[0] * src[s].dir[0] + src[s].dir[1] * src[s].dir[1] + src[s].dir[2] * src[s].dir[2]);
     if (!(dn > 0) || !isfinite(dn)) { free_run(g); return fail(EMMO_EINVAL, "run_begin: source %d has zero direction", s); }
+    S->magnetic = src[s].type == 1;
+    if (src[s].type != 0 && src[s].type != 1) { free_run(g); return fail(EMMO_EINVAL, "run_begin: source %d has an unknown type", s); }
     for (int c = 0; c < 3; c++) {
+      const int cl = c + (S->magnetic ? 3 : 0);         /* lattice of E_c or of H_c */
       S->nsn[c] = 0;
       if (src[s].dir[c] == 0.0) continue;
       stencil1 st[3];
       for (int a = 0; a < 3; a++) {
-        const double *L = LAT[c][a] ? g->xh[a] : g->xn[a];
+        const double *L = LAT[cl][a] ? g->xh[a] : g->xn[a];
         int lo_ok = (a == 2) ? g->klo : r;
         if (src[s].pos[a] < g->xn[a][g->lo[a]] || src[s].pos[a] > g->xn[a][g->lo[a] + g->nc[a]] ||
             lattice_stencil(L, g->N[a], src[s].pos[a], R->np, lo_ok, &st[a]) || st[a].start + R->np - 1 > g->N[a] - 1 - r) {
@@ -677,7 +681,7 @@ int emmo_run_begin(emmo_grid *g, const emmo_src *src, int nsrc, const double *fr
       int n = 0;
       for (int c3 = 0; c3 < R->np; c3++) for (int c2 = 0; c2 < R->np; c2++) for (int c1 = 0; c1 < R->np; c1++) {
         int i = st[0].start + c1, j = st[1].start + c2, k = st[2].start + c3;
-        double V = node_width(g, 0, LAT[c][0], i) * node_width(g, 1, LAT[c][1], j) * node_width(g, 2, LAT[c][2], k);
+        double V = node_width(g, 0, LAT[cl][0], i) * node_width(g, 1, LAT[cl][1], j) * node_width(g, 2, LAT[cl][2], k);
         S->sidx[c][n] = IDX(g, i, j, k);
         S->sw[c][n] = src[s].dir[c] / dn * st[0].w[c1] * st[1].w[c2] * st[2].w[c3] / V;
         n++;
@@ -732,7 +736,7 @@ static void update_E(const emmo_grid *g, const runstate *R, srcstate *S, double 
     }
   }
   /* source term -dt/eps * J, J = s(t) W  (Eq. 8) */
-  for (int c = 0; c < 3; c++)
+  if (!S->magnetic) for (int c = 0; c < 3; c++)
     for (int n = 0; n < S->nsn[c]; n++) S->E[c][S->sidx[c][n]] -= g->ce[c][S->sidx[c][n]] * st * S->sw[c][n];
 }
 
@@ -884,7 +888,8 @@ static void dtft_emf(const emmo_grid *g, const runstate *R, srcstate *S, int it,
   for (int f = 0; f < nf; f++) {
     cplx twH = cexp(I * R->wp[f] * ((double)it * g->dt));          /* H and J at t = it dt       */
     cplx twE = cexp(I * R->wp[f] * (((double)it + 0.5) * g->dt));  /* updated E at (it+1/2) dt   */
-    if (fields) S->Jw[f] += st * twH;
+    /* source spectrum: J sits at t = it dt; M is centred in the H update, at (it+1/2) dt [R6] */
+    if (fields) S->Jw[f] += S->magnetic ? wavelet(R, ((double)it + 0.5) * g->dt) * twE : st * twH;
 #pragma omp parallel for schedule(static)
     for (size_t p = 0; p < (fields ? R->ndft : 0); p++) {
       size_t t = R->dft_idx[p];
@@ -938,6 +943,11 @@ int emmo_run_steps(emmo_grid *g, int n, int *nsteps, int *all_done) {
       dtft_emf(g, R, S, it, st);                                          /* L483 */
       update_H(g, R, S);                                                  /* L486-489 */
       if (g->top == EMMO_TOP_AIR && airwave_bc_update_H(g, S)) return fail(EMMO_ENOMEM, "run_steps: out of memory");
+      if (S->magnetic) {                                                  /* inject_magnetic_src_fwd (L488): -dt/mu * M^{n+1/2} */
+        const double sm = wavelet(R, ((double)it + 0.5) * g->dt);
+        for (int c = 0; c < 3; c++)
+          for (int n = 0; n < S->nsn[c]; n++) S->H[c][S->sidx[c][n]] -= g->dt / MU0 * sm * S->sw[c][n];
+      }
       S->nsteps = it + 1;
       if ((it + 1) % R->check_every == 0) {                               /* L493-498, [R9] */
         int cv = check_convergence(g, R, S, it);
@@ -975,8 +985,12 @@ int emmo_run_end(emmo_grid *g, double *out_, int *nsteps) {
         if (p < 0) return fail(EMMO_EINVAL, "run_end: receiver %d stencil leaves the DFT box", q);
         acc += st[0].w[c1] * st[1].w[c2] * st[2].w[c3] * S->F[((size_t)c * nf + f) * R->ndft + (size_t)p];
       }
-      cplx G = acc / S->Jw[f];                                           /* Eq. 7b */
-      if (c < 3) G *= csqrt(-I * 2 * M_PI * R->freqs[f] / (2 * g->w0));  /* Eq. 7a, principal root */
+      /* Eq. 4 + Eq. 7: E' = E, M' = M, H' = sq H, J' = sq J with sq = sqrt(-i w / 2 w0) (principal root):
+         electric source G^EE = sq F_E/J', G^HE = F_H/J'; magnetic source G^EM = F_E/M', G^HM = F_H/(sq M') */
+      cplx G = acc / S->Jw[f];
+      const cplx sq = csqrt(-I * 2 * M_PI * R->freqs[f] / (2 * g->w0));
+      if (!S->magnetic && c < 3) G *= sq;
+      if (S->magnetic && c >= 3) G /= sq;
       out[(((size_t)s * nf + f) * R->nrec + q) * 6 + c] = G;
     }
   }

@@ -51,7 +51,10 @@ typedef struct {
   double aux_dx;   /* auxiliary uniform plane spacing for NU x-y; <=0 => min    */
 } emmo_grid_opts;
 
-typedef struct { double pos[3]; double dir[3]; } emmo_src;
+typedef struct {
+  double pos[3]; double dir[3];
+  int type;        /* 0: electric dipole J (Eq. 8); 1: magnetic dipole M (Eq. 8, inject_magnetic_src_fwd L457) */
+} emmo_src;
 
 typedef struct {
   int max_steps;    /* hard cap; <=0 => 100000                                  */

@@ -40,7 +40,7 @@ class GridOpts(C.Structure):
 
 
 class Src(C.Structure):
-    _fields_ = [("pos", C.c_double * 3), ("dir", C.c_double * 3)]
+    _fields_ = [("pos", C.c_double * 3), ("dir", C.c_double * 3), ("type", C.c_int)]
 
 
 class RunOpts(C.Structure):
@@ -117,9 +117,10 @@ def fft2(a, sign):
 
 def _srcs(sources):
     arr = (Src * len(sources))()
-    for s, (pos, d) in zip(arr, sources):
-        s.pos[:] = [float(v) for v in pos]
-        s.dir[:] = [float(v) for v in d]
+    for s, src in zip(arr, sources):       # (pos, dir) = electric dipole; (pos, dir, "M") = magnetic dipole
+        s.pos[:] = [float(v) for v in src[0]]
+        s.dir[:] = [float(v) for v in src[1]]
+        s.type = 1 if len(src) > 2 and str(src[2]).upper().startswith("M") else 0
     return arr
 
 

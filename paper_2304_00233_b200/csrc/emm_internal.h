@@ -66,7 +66,9 @@ struct DevState {              // per run; arrays carry a leading source dimensi
   float *psz[2][2];            // z-slab psi [nsrc][2nb][N2][P1]
   float2 *F;                   // [nsrc][nf][6][NZB][N2][P1]
   const float2 *twE, *twH;     // [max_steps][nf]
-  const float *wav;            // [max_steps]
+  const float *wav;            // [max_steps] s(it dt): electric sources
+  const float *wavh;           // [max_steps] s((it+1/2) dt): magnetic sources
+  const int *src_mag;          // [nsrc] 1 = magnetic dipole
   int *it;                     // device step counter
   int *done;                   // [nsrc]
   int nf, nsrc;

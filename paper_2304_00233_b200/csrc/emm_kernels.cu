@@ -395,15 +395,16 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   }
 }
 
-// ---- source injection: E_c[node] -= s(it*dt) * (dt/eps * W_c)[node]  (Eq. 8, [R7]) ----
+// ---- source injection (Eq. 8, [R7]): electric dipoles E_c[node] -= s(it dt) * (dt/eps W_c)[node] before the E
+// update; magnetic dipoles H_c[node] -= s((it+1/2) dt) * (dt/mu W_c)[node] after the H update and its boundary ----
 __global__ void k_inject(const DevGrid g, const DevState s, const int *__restrict__ off, const int *__restrict__ idx,
-                         const float *__restrict__ w) {
+                         const float *__restrict__ w, const int magnetic) {
   const int src = blockIdx.x;
-  if (s.done[src]) return;
-  const float st = s.wav[*s.it];
+  if (s.done[src] || s.src_mag[src] != magnetic) return;
+  const float st = magnetic ? s.wavh[*s.it] : s.wav[*s.it];
   for (int c = 0; c < 3; ++c) {
-    float *E = s.E[c] + (size_t)src * g.VS;
-    for (int n = off[src * 3 + c] + threadIdx.x; n < off[src * 3 + c + 1]; n += blockDim.x) E[idx[n]] -= st * w[n];
+    float *U = (magnetic ? s.H[c] : s.E[c]) + (size_t)src * g.VS;
+    for (int n = off[src * 3 + c] + threadIdx.x; n < off[src * 3 + c + 1]; n += blockDim.x) U[idx[n]] -= st * w[n];
   }
 }
 
@@ -585,8 +586,8 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream
   return 0;
 }
 
-int launch_inject(emm_grid *g, const DevState &s, const DevRun &r) {
-  k_inject<<<s.nsrc, 128, 0, g->stream>>>(g->dg, s, r.src_off, r.src_idx, r.src_w);
+int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic) {
+  k_inject<<<s.nsrc, 128, 0, g->stream>>>(g->dg, s, r.src_off, r.src_idx, r.src_w, magnetic);
   EMM_LAUNCH_CHECK(g, "k_inject");
   return 0;
 }

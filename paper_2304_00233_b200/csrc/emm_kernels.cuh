@@ -29,7 +29,7 @@ struct DevRun {
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st);
-int launch_inject(emm_grid *g, const DevState &s, const DevRun &r);
+int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);
 int launch_step_end(emm_grid *g, const DevState &s);

@@ -19,7 +19,9 @@ struct Run {
   double fmax = 0, beta = 0, t0 = 0, tol = 1e-6;
   int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
   int it_min = 0, it_host = 0, table_steps = 0, dtft_every = 1;
-  std::vector<double> wav;                  // s(it*dt) rounded to fp32 (what the device injects)
+  std::vector<double> wav, wavh;            // s(it dt), s((it+1/2) dt) rounded to fp32 (what the device injects)
+  std::vector<int> mag;                     // [nsrc] 1 = magnetic dipole
+  bool any_mag = false, any_el = false;
   std::vector<Stencil1> rst;                // [nrec][6][3]
   std::vector<int> nsteps, done, status;
   DevState ds{};
@@ -111,6 +113,8 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps,
   s.twE = A.take<float2>((size_t)table_steps * nf);
   s.twH = A.take<float2>((size_t)table_steps * nf);
   s.wav = A.take<float>(table_steps);
+  s.wavh = A.take<float>(table_steps);
+  s.src_mag = A.take<int>(nsrc);
   s.it = A.take<int>(1);
   s.done = A.take<int>(nsrc);
   s.nf = nf;
@@ -377,6 +381,17 @@ static void cpml_tables(const emm_grid *g, int a, double fmax, std::vector<float
   }
 }
 
+// source spectrum of Eq. 7: J'(w') = sum s(it dt) e^{i w' it dt}; a magnetic source is centred in the H update,
+// M'(w') = sum s((it+1/2) dt) e^{i w' (it+1/2) dt} [R6]; only the terms the DTFT took (decimation)
+static std::complex<double> source_spectrum(const emm_grid *g, const Run *R, int s, int f) {
+  const std::complex<double> I(0, 1);
+  std::complex<double> J = 0;
+  for (int it = 0; it < R->nsteps[s]; it += R->dtft_every)
+    J += R->mag[s] ? R->wavh[it] * std::exp(I * R->wp[f] * (((double)it + 0.5) * g->dt))
+                   : R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
+  return J;
+}
+
 static int enqueue_steps_raw(emm_grid *g, int n) {
   Run *R = g->run;
   int rc;
@@ -384,7 +399,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
   for (int q = 0; q < n; ++q) {
     if (R->it_host >= R->table_steps) return fail(EMM_EINVAL, "run: step %d beyond the twiddle table (max_steps)", R->it_host);
     cudaStream_t M = g->stream, B = g->stream_b;
-    if ((rc = launch_inject(g, R->ds, R->dr))) return rc;                     // Alg. 1 L477 (before the update: same sum)
+    if (R->any_el && (rc = launch_inject(g, R->ds, R->dr, 0))) return rc;     // Alg. 1 L477 (before the update: same sum)
     if (g->top != EMM_TOP_AIR) {
       if ((rc = launch_update(g, R->ds, 0, 0, M))) return rc;                 // L476-479 + E part of L483
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                // check-set part of L483
@@ -418,6 +433,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));      // join
     }
+    if (R->any_mag && (rc = launch_inject(g, R->ds, R->dr, 1))) return rc;    // L488, after the H update and its boundary
     if (R->nf > 0 && (R->it_host + 1) % R->check_every == 0 &&
         (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
     if ((rc = launch_step_end(g, R->ds))) return rc;
@@ -567,10 +583,15 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     std::vector<float2> twE((size_t)T * nf), twH((size_t)T * nf);
     std::vector<double2> twE64(T), twH64(T);
     R->wav.resize(T);
+    R->wavh.resize(T);
+    std::vector<float> wavh(T);
     for (int it = 0; it < T; ++it) {
       const double t = (double)it * g->dt, u = t - R->t0;
       wav[it] = (float)(-2.0 * R->beta * u * std::sqrt(R->beta / kPi) * std::exp(-R->beta * u * u));
       R->wav[it] = (double)wav[it];
+      const double uh = t + 0.5 * g->dt - R->t0;
+      wavh[it] = (float)(-2.0 * R->beta * uh * std::sqrt(R->beta / kPi) * std::exp(-R->beta * uh * uh));
+      R->wavh[it] = (double)wavh[it];
       for (int f = 0; f < nf; ++f) {
         const std::complex<double> I(0, 1);
         const std::complex<double> h = std::exp(I * R->wp[f] * t), e = std::exp(I * R->wp[f] * (((double)it + 0.5) * g->dt));
@@ -579,6 +600,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
         if (f == R->fmin) { twH64[it] = make_double2(h.real(), h.imag()); twE64[it] = make_double2(e.real(), e.imag()); }
       }
     }
+    if ((rc = upload(g, const_cast<float *>(R->ds.wavh), wavh))) { free_run(g); return rc; }
     if ((rc = upload(g, const_cast<float *>(R->ds.wav), wav)) || (rc = upload(g, const_cast<float2 *>(R->ds.twE), twE)) ||
         (rc = upload(g, const_cast<float2 *>(R->ds.twH), twH)) || (rc = upload(g, R->dr.twE64, twE64)) ||
         (rc = upload(g, R->dr.twH64, twH64)) || (rc = upload(g, R->dr.chk_idx, chk))) { free_run(g); return rc; }
@@ -602,14 +624,19 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     std::vector<float> sw;
     for (int s = 0; s < nsrc; ++s) {
       const double *dir = src[s].dir, *pos = src[s].pos;
+      if (src[s].type != 0 && src[s].type != 1) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: source %d has an unknown type", s); }
+      const bool mag = src[s].type == 1;
+      R->mag.push_back(mag ? 1 : 0);
+      (mag ? R->any_mag : R->any_el) = true;
       const double dn = std::sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
       if (!(dn > 0) || !std::isfinite(dn)) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: source %d has zero direction", s); }
       for (int c = 0; c < 3; ++c) {
         soff[s * 3 + c] = (int)sidx.size();
         if (dir[c] == 0.0) continue;
+        const int cl = c + (mag ? 3 : 0);                 // lattice of E_c or of H_c
         Stencil1 st[3];
         for (int a = 0; a < 3; ++a) {
-          const double *S = kLat[c][a] ? g->xh[a].data() : g->xn[a].data();
+          const double *S = kLat[cl][a] ? g->xh[a].data() : g->xn[a].data();
           if (pos[a] < g->xn[a][g->lo[a]] || pos[a] > g->xn[a][g->lo[a] + g->nc[a]] ||
               !make_stencil(S, g->N[a], pos[a], np, a == 2 ? g->klo : r, g->N[a] - 1 - r, false, &st[a])) {
             free_run(g); return fail(EMM_EINVAL, "emm_run_begin: source %d outside the interior", s);
@@ -617,9 +644,9 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
         }
         for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1) {
           const int i = st[0].start + c1, j = st[1].start + c2, k = st[2].start + c3;
-          const double V = node_width(g, 0, kLat[c][0], i) * node_width(g, 1, kLat[c][1], j) * node_width(g, 2, kLat[c][2], k);
+          const double V = node_width(g, 0, kLat[cl][0], i) * node_width(g, 1, kLat[cl][1], j) * node_width(g, 2, kLat[cl][2], k);
           const double W = dir[c] / dn * st[0].w[c1] * st[1].w[c2] * st[2].w[c3] / V;
-          const double ce = g->dt * 2 * g->w0 / sigma_bar_host(g, c, i, j, k);
+          const double ce = mag ? g->dt / kMu0 : g->dt * 2 * g->w0 / sigma_bar_host(g, c, i, j, k);   // dt/mu or dt/eps
           sidx.push_back((int)(((size_t)k * g->N[1] + j) * g->P1 + i));
           sw.push_back((float)(ce * W));
         }
@@ -628,6 +655,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     }
     for (int s = 0; s < nsrc; ++s) for (int c = 0; c < 3; ++c) if (soff[s * 3 + c + 1] < soff[s * 3 + c]) soff[s * 3 + c + 1] = soff[s * 3 + c];
     (void)np3;
+    if ((rc = upload(g, const_cast<int *>(R->ds.src_mag), R->mag))) { free_run(g); return rc; }
     if ((rc = upload(g, R->dr.src_off, soff)) || (rc = upload(g, R->dr.src_idx, sidx)) || (rc = upload(g, R->dr.src_w, sw))) { free_run(g); return rc; }
 
     // receiver gather list
@@ -699,8 +727,7 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
   const std::complex<double> I(0, 1);
   for (int s = 0; s < R->nsrc; ++s)
     for (int f = 0; f < nf; ++f) {
-      std::complex<double> Jw = 0;                                             // J'(omega') = sum s[it] e^{i w' it dt}
-      for (int it = 0; it < R->nsteps[s]; it += R->dtft_every) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
+      const std::complex<double> Jw = source_spectrum(g, R, s, f);
       const std::complex<double> sc = std::sqrt(-I * 2.0 * kPi * R->freqs[f] / (2 * g->w0));   // Eq. 7a, principal root
       for (int q = 0; q < R->nrec; ++q)
         for (int c = 0; c < 6; ++c) {
@@ -711,7 +738,8 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
           for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1, ++n)
             acc += st[0].w[c1] * st[1].w[c2] * st[2].w[c3] * std::complex<double>(v[n].x, v[n].y);
           std::complex<double> G = acc / Jw;                                   // Eq. 7b
-          if (c < 3) G *= sc;
+          if (!R->mag[s] && c < 3) G *= sc;                                    // electric source: G^EE = sc F_E/J'
+          if (R->mag[s] && c >= 3) G /= sc;                                    // magnetic source: G^HM = F_H/(sc M')
           out[(((size_t)s * nf + f) * R->nrec + q) * 6 + c] = G;
         }
     }
@@ -781,11 +809,7 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
     if (rc) return rc;
     std::complex<double> *o = static_cast<std::complex<double> *>(host_out);
     const std::complex<double> I(0, 1);
-    for (int f = 0; f < R->nf; ++f) {
-      std::complex<double> Jw = 0;
-      for (int it = 0; it < R->nsteps[isrc]; it += R->dtft_every) Jw += R->wav[it] * std::exp(I * R->wp[f] * ((double)it * g->dt));
-      o[f] = Jw;
-    }
+    for (int f = 0; f < R->nf; ++f) o[f] = source_spectrum(g, R, isrc, f);
     return 0;
   }
   if (what == EMM_GET_DELTA) {

@@ -148,6 +148,15 @@ def test_dtft_decimation_matches_oracle(emm, oracle, m):
     assert (np.abs(oa - ob)[big] / np.abs(ob)[big]).max() < 1e-3
 
 
+def test_magnetic_and_mixed_sources_match_oracle(emm, oracle):
+    """a magnetic dipole (injected into H at the half step), alone and batched together with
+    an electric dipole; fields, accumulators and receivers against the oracle."""
+    w = W.cfg2(nx=36, nz=24, dx=100.0, rd=2, nb=8)
+    srcs = [((-130.0, 60.0, 870.0), (0.2, 1.0, 0.4), "M"), ((210.0, -40.0, 930.0), (1.0, 0.0, 0.3))]
+    _field_parity(emm, oracle, w, 160, sources=srcs[:1])
+    _field_parity(emm, oracle, w, 120, sources=srcs, batched=1)
+
+
 def test_converged_run_matches_oracle_steps_and_receivers(emm, oracle):
     """configs[1] scaled, run to convergence: integer step count exact, receivers within 1e-3."""
     w = W.cfg2(nx=40, nz=28, dx=100.0, rd=2, nb=8)
