@@ -151,6 +151,19 @@ def oracle_rate(w_full, budget_s, steps, warmup, args):
     t = time.perf_counter()
     g.run_steps(steps)
     el = time.perf_counter() - t
+    # the same sample on ONE host thread (1 thread and all cores), one step is enough
+    one = None
+    try:
+        import ctypes
+        gomp = ctypes.CDLL("libgomp.so.1")
+        gomp.omp_set_num_threads(1)
+        t = time.perf_counter()
+        g.run_steps(1)
+        one = n / (time.perf_counter() - t) / 1e9
+        gomp.omp_set_num_threads(ncores)
+    except OSError:
+        pass
+    oracle_rate.one_thread = one
     g.close()
     desc = ("%s recipe at %dx%dx%d cells (padded %dx%dx%d, nf=%d, full-box DTFT), %d steps after %d warm-up, fp64, "
             "gcc -O2 -fopenmp" % (w["name"], len(w["x"]) - 1, len(w["y"]) - 1, len(w["z"]) - 1, i["N1"], i["N2"], i["N3"],
@@ -173,7 +186,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "Gcell-updates/s", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": describe(w_full, gi, 1),
-            "cpu_baseline": {"value": val, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "cpu_baseline": {"value": val, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc,
+                             "value_one_thread": getattr(oracle_rate, "one_thread", None)},
             "e2e": {"value": val, "unit": "Gcell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -305,7 +319,8 @@ def run_gpu(args):
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             v, cms, cores, desc = oracle_rate(w, 20.0, 3, 1, args)
-            cpu = {"value": v, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc, "ms_per_step": cms}
+            cpu = {"value": v, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc, "ms_per_step": cms,
+                   "value_one_thread": getattr(oracle_rate, "one_thread", None)}
         line = {"metric": METRIC, "value": value, "unit": "Gcell-updates/s", "n_gpus": world, "steps": K, "warmup": Wm,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                 "data": "synthetic", "config": describe(w, info, nsrc), "clocks": clocks,

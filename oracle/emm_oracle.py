@@ -147,7 +147,10 @@ class Grid:
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().emmo_grid_destroy(self._h)
+            try:
+                lib().emmo_grid_destroy(self._h)
+            except TypeError:          # interpreter shutdown: module globals are already gone
+                pass
             self._h = None
 
     __del__ = close

@@ -168,7 +168,10 @@ class Grid:
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().emm_grid_destroy(self._h)
+            try:
+                lib().emm_grid_destroy(self._h)
+            except TypeError:          # interpreter shutdown: module globals are already gone
+                pass
             self._h = None
         self._ws = None
 
