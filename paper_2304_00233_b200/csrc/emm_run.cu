@@ -563,11 +563,18 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     // check set [R9]
     std::vector<int> chk;
     if (nf > 0)
-    for (int k = g->blo[2]; k <= g->bhi[2]; ++k) for (int j = g->blo[1]; j <= g->bhi[1]; ++j) for (int i = g->blo[0]; i <= g->bhi[0]; ++i) {
-      const bool ei = i == g->blo[0] || i == g->bhi[0], ej = j == g->blo[1] || j == g->bhi[1], ek = k == g->blo[2] || k == g->bhi[2];
-      const bool take = R->check_set == EMM_CHECK_FULL ? true : R->check_set == EMM_CHECK_FACES ? (ei || ej || ek) : (ei && ej && ek);
-      if (take) chk.push_back((int)(((size_t)k * g->N[1] + j) * g->P1 + i));
-    }
+      for (int k = g->blo[2]; k <= g->bhi[2]; ++k) for (int j = g->blo[1]; j <= g->bhi[1]; ++j) {
+        const bool ej = j == g->blo[1] || j == g->bhi[1], ek = k == g->blo[2] || k == g->bhi[2];
+        const size_t rowbase = ((size_t)k * g->N[1] + j) * g->P1;
+        // whole row when the row lies on a face (or for the full set); otherwise only its two end nodes can qualify
+        const bool whole = R->check_set == EMM_CHECK_FULL || (R->check_set == EMM_CHECK_FACES && (ej || ek));
+        if (whole) {
+          for (int i = g->blo[0]; i <= g->bhi[0]; ++i) chk.push_back((int)(rowbase + i));
+        } else if (R->check_set == EMM_CHECK_FACES || (ej && ek)) {      // corners: only rows with ej && ek
+          chk.push_back((int)(rowbase + g->blo[0]));
+          if (g->bhi[0] != g->blo[0]) chk.push_back((int)(rowbase + g->bhi[0]));
+        }
+      }
     // workspace layout
     Arena A;
     A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
