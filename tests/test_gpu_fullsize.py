@@ -191,3 +191,32 @@ def test_cfg5_full_size_batched_equals_sequential(emm):
         for a, b in zip(bat[s], (g.get("E1"), g.get("H2"), g.get("F_E1", ifreq=1))):
             assert np.array_equal(a, b)               # same kernels, same arithmetic: bit-identical
     assert not np.array_equal(bat[0][0], bat[1][0])   # and the sources really differ
+
+
+def _compare_with_golden(emm, path, build, fixed=0):
+    gold = json.load(open(path))
+    w = build()
+    g = make_grid(emm, w)
+    info = g.info()
+    for k in ("N1", "N2", "N3", "k0", "aux_M1", "aux_M2"):
+        assert info[k] == gold["info"][k], k
+    assert abs(info["dt"] / gold["info"]["dt"] - 1) < 1e-12
+    opts = dict(fixed_steps=fixed) if fixed else dict(w["run"])
+    opts.pop("batched", None)
+    out, ns = g.run(w["sources"][:1], w["freqs"], w["receivers"], opts)
+    ref = np.array(gold["receivers_re"]) + 1j * np.array(gold["receivers_im"])
+    assert int(ns[0]) == gold["nsteps"]                       # integer output: exact
+    for sl in (slice(0, 3), slice(3, 6)):
+        A, B = out[0][..., sl], ref[..., sl]
+        big = np.abs(B) > 1e-3 * np.abs(B).max()
+        assert big.sum() > 10
+        assert (np.abs(A - B)[big] / np.abs(B)[big]).max() < 1e-3
+    return out, gold
+
+
+def test_cfg3_full_size_converged_matches_oracle_golden(emm):
+    """configs[2] at full size (200x200x120 non-uniform cells, random sediment + resistive block, VTI cell values),
+    run to convergence; the oracle's result was stored by `make_goldens.py cfg3 0 100` (auxiliary plane spacing
+    100 m instead of the default 25 m: with the oracle's plain FFT the default would take ~10 h)."""
+    _compare_with_golden(emm, os.path.join(HERE, "golden", "cfg3_converged_aux100.json"),
+                         lambda: W.cfg3(emm.emm_nugrid, aux_dx=100.0))
