@@ -173,7 +173,7 @@ __device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0
 template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_MINB : (NF >= 4 ? 2 : 3); }
 
 template <int R, int NF, bool IS_H>
-__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0) {
+__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0, const int sel) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
   const int src = blockIdx.z / nchunks, chunk = chunk0 + blockIdx.z - src * nchunks;   // this launch covers chunks [chunk0, chunk0 + nchunks)
   if (s.done[src]) return;
@@ -184,6 +184,9 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   const int kend = min(kbeg + kc, g.N3 - R);
   if (kbeg >= kend) return;
   const int it = *s.it;
+  // DTFT decimation runs two instances per pass: sel 1 = the accumulator-free one, for the steps that skip the DTFT;
+  // sel 2 = the DTFT one, for the steps that contribute; the instance whose turn it is not exits here (sel 0: no split)
+  if (sel && ((sel == 2) != (it % s.dft_every == 0))) return;
 
   const float *A1 = (IS_H ? s.E[0] : s.H[0]) + (size_t)src * g.VS;
   const float *A2 = (IS_H ? s.E[1] : s.H[1]) + (size_t)src * g.VS;
@@ -223,7 +226,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 
   // DTFT bookkeeping
   const int nf = s.nf;
-  const bool dft_xy = (nf > 0) && (it % s.dft_every == 0) &&        // DTFT decimation: this step contributes or not
+  const bool dft_xy = (sel != 1) && (nf > 0) && (it % s.dft_every == 0) &&        // DTFT decimation: this step contributes or not
                       (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);
   const size_t fstride = (size_t)6 * g.NZB * g.PS;      // float2 elements between frequencies
   float2 *Fsrc = s.F + (size_t)src * nf * fstride + (size_t)(IS_H ? 3 : 0) * g.NZB * g.PS;
@@ -506,26 +509,26 @@ __global__ void k_gather(const DevGrid g, const DevState s, const int *__restric
 
 // unrolled-NF instantiations stage one plane of accumulators per thread in dynamic shared memory
 template <int R, int NF, bool IS_H>
-static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0) {
+static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
   const size_t smem = EMM_CPA ? (size_t)3 * NF * 2 * 128 * sizeof(float4) : 0;
   static bool configured = false;
   if (!configured && smem > 48 * 1024) {
     cudaFuncSetAttribute(k_update<R, NF, IS_H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
-  k_update<R, NF, IS_H><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0);
+  k_update<R, NF, IS_H><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel);
 }
 
 template <int R, bool IS_H>
-static void launch_update_nf(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0) {
-  switch (s.nf) {
-    case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0); break;
-    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
-    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
-    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
-    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
-    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0); break;
-    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0); break;
+static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
+  switch (nf) {
+    case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0, sel); break;
+    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
+    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
+    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
+    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
+    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
+    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0, sel); break;
   }
 }
 
@@ -534,47 +537,61 @@ static void launch_update_nf(const DevGrid &dg, const DevState &s, dim3 grid, di
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st) {
   const DevGrid &dg = g->dg;
   const int quads = dg.P1 / 4;
-  // block: TX quads wide (64 or 128 nodes), 128 threads; pick the width that wastes fewer lanes
-  int TX = 16;
-  if (((quads + 31) / 32) * 32 <= ((quads + 15) / 16) * 16) TX = 32;
-  if (quads <= 8) TX = 8;
-  {
-    static const char *env_tx = getenv("EMM_TX");        // tuning knob: quads per block row (8, 16, 32)
-    if (env_tx && atoi(env_tx) > 0) TX = atoi(env_tx);
-  }
-  const int TY = 128 / TX;
   const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
-  // planes per z chunk: 16 on large grids; fewer on small ones so that the grid still holds ~8 blocks per SM
-  // (each block marches its planes one after the other, so a sparse grid is latency-bound)
-  int kc = 16;
-  {
-    const long long xy = (long long)((quads + TX - 1) / TX) * ((dg.N2 + TY - 1) / TY) * s.nsrc;
-    while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 8) kc /= 2;
-  }
-  {
-    static const char *env_kc = getenv("EMM_KC");        // tuning knob: planes per z chunk
-    if (env_kc && atoi(env_kc) > 0) kc = atoi(env_kc);
-  }
-  const int nall = (nk + kc - 1) / kc;
-  const int nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);        // chunks whose stencils reach the ghost planes
-  const int chunk0 = part == 2 ? nsurf : 0;
-  const int nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
-  if (nchunks <= 0) return 0;
-  dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
-  if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
+  // launch one instance (nf = accumulators it is compiled for) over the chunks of `part`
+  auto launch = [&](int nf, int sel) -> int {
+    // block: TX quads wide, 128 threads.  With accumulators: 16 or 32 quads, whichever wastes fewer lanes (long
+    // contiguous accumulator rows); without: 8 quads x 16 rows, more y reuse in L1 (profiles/r1_kernel_experiments.md)
+    int TX = 16;
+    if (((quads + 31) / 32) * 32 <= ((quads + 15) / 16) * 16) TX = 32;
+    if (nf == 0 || quads <= 8) TX = 8;
+    {
+      static const char *env_tx = getenv("EMM_TX");        // tuning knob: quads per block row (8, 16, 32)
+      if (env_tx && atoi(env_tx) > 0) TX = atoi(env_tx);
+    }
+    const int TY = 128 / TX;
+    // planes per z chunk: 16 on large grids; fewer on small ones so that the grid still holds ~8 blocks per SM
+    // (each block marches its planes one after the other, so a sparse grid is latency-bound)
+    int kc = 16;
+    {
+      const long long xy = (long long)((quads + TX - 1) / TX) * ((dg.N2 + TY - 1) / TY) * s.nsrc;
+      while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 8) kc /= 2;
+    }
+    {
+      static const char *env_kc = getenv("EMM_KC");        // tuning knob: planes per z chunk
+      if (env_kc && atoi(env_kc) > 0) kc = atoi(env_kc);
+    }
+    const int nall = (nk + kc - 1) / kc;
+    const int nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);        // chunks whose stencils reach the ghost planes
+    const int chunk0 = part == 2 ? nsurf : 0;
+    const int nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
+    if (nchunks <= 0) return 0;
+    dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
+    if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
+    if (is_h) {
+      if (dg.r == 1) launch_update_nf<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+      else if (dg.r == 2) launch_update_nf<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+      else launch_update_nf<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+    } else {
+      if (dg.r == 1) launch_update_nf<1, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+      else if (dg.r == 2) launch_update_nf<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+      else launch_update_nf<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+    }
+    EMM_LAUNCH_CHECK(g, is_h ? "k_update<H>" : "k_update<E>");
+    return 0;
+  };
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (g->prof) {
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(EMM_ECUDA, "cudaEventCreate failed");
     cudaEventRecord(e0, st);
   }
-  if (is_h) {
-    if (dg.r == 1) launch_update_nf<1, true>(dg, s, grid, block, st, kc, nchunks, chunk0);
-    else if (dg.r == 2) launch_update_nf<2, true>(dg, s, grid, block, st, kc, nchunks, chunk0);
-    else launch_update_nf<3, true>(dg, s, grid, block, st, kc, nchunks, chunk0);
+  int rc;
+  if (s.nf > 0 && s.dft_every > 1) {
+    // DTFT decimation: most steps take no accumulator at all.  Both instances are launched every step (the step index
+    // lives on the device, so that a captured graph can be replayed); the one whose turn it is not exits at once.
+    if ((rc = launch(0, 1)) || (rc = launch(s.nf, 2))) return rc;
   } else {
-    if (dg.r == 1) launch_update_nf<1, false>(dg, s, grid, block, st, kc, nchunks, chunk0);
-    else if (dg.r == 2) launch_update_nf<2, false>(dg, s, grid, block, st, kc, nchunks, chunk0);
-    else launch_update_nf<3, false>(dg, s, grid, block, st, kc, nchunks, chunk0);
+    if ((rc = launch(s.nf, 0))) return rc;
   }
   if (g->prof) {
     cudaEventRecord(e1, st);
@@ -582,7 +599,6 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream
     g->prof_ev.push_back(e1);
     g->prof_kind.push_back(is_h);
   }
-  EMM_LAUNCH_CHECK(g, is_h ? "k_update<H>" : "k_update<E>");
   return 0;
 }
 
