@@ -82,6 +82,7 @@ struct DevTables {             // device pointers of the per-grid region
   float *ta_w[2][2], *fa_w[2][2];
   float *kx, *ky;                          // signed wavenumbers of the FFT plane
   void *fft_ws[3];
+  void *sp_ws[8];                          // work areas of the separable route's 1-D plans
 };
 
 struct Run;
@@ -101,6 +102,7 @@ struct emm_grid {
   int P1 = 0, XS = 0;
   // air boundary
   int M1 = 0, M2 = 0;
+  bool sep_air = false;                  // non-uniform x-y: separable route (emm_air_sep.cu) instead of plane-sized 2-D transforms
   double dxa = 0, dya = 0;
   std::vector<emm::Stencil1> toaux[2][2], fromaux[2][2];
   // model
@@ -121,6 +123,8 @@ struct emm_grid {
   cufftHandle plan_fwd = 0, plan_inv_e = 0, plan_inv_h = 0;
   bool have_plans = false;
   size_t fft_ws[3] = {0, 0, 0};             // cuFFT work-area bytes: forward, inverse (E), inverse (H)
+  cufftHandle sp[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // separable route: batched 1-D plans (emm_air_sep.cu)
+  size_t sp_ws[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   double vref[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // CPML reference speed per face [R5]
   emm::Run *run = nullptr;
   long long launches = 0;

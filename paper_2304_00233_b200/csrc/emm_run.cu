@@ -46,6 +46,16 @@ static size_t vol(const emm_grid *g) { return (size_t)g->P1 * g->N[1] * g->N[2];
 // cuFFT plans of the air boundary; their work areas are carved from the caller's workspace
 static int ensure_plans(emm_grid *g) {
   if (g->top != EMM_TOP_AIR || g->have_plans) return 0;
+  // non-uniform x-y: separable route with batched 1-D transforms (EMM_AIR_PLANE=1 keeps the plane-sized 2-D
+  // transforms, for A/B measurements)
+  const char *force = std::getenv("EMM_AIR_PLANE");
+  g->sep_air = !g->uniform_xy && !(force && force[0] == '1');
+  if (g->sep_air) {
+    const int rc = sep_air_make_plans(g);
+    if (rc) return rc;
+    g->have_plans = true;
+    return 0;
+  }
   int n[2] = {g->M2, g->M1};
   cufftHandle *pl[3] = {&g->plan_fwd, &g->plan_inv_e, &g->plan_inv_h};
   const int batch[3] = {1, g->r - 1, g->r};
@@ -85,6 +95,8 @@ static void layout_fixed(emm_grid *g, Arena &A) {
           g->T.fa_w[a][l] = A.take<float>((size_t)4 * g->N[a]);
         }
     for (int q = 0; q < 3; ++q) g->T.fft_ws[q] = A.take<char>(g->fft_ws[q] + 256);
+    if (g->sep_air)
+      for (int q = 0; q < 8; ++q) g->T.sp_ws[q] = A.take<char>(g->sp_ws[q] + 256);
   }
 }
 
@@ -135,7 +147,7 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps,
   r.rec_idx = A.take<int>((size_t)6 * nrec * np3);
   r.rec_val = A.take<float2>((size_t)nsrc * nf * 6 * nrec * np3);
   if (g->top == EMM_TOP_AIR)   // FFT planes [1 + r][M2][M1] + (non-uniform x-y) the x-interpolated rows [N2][M1]
-    r.air = A.take<float2>((size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
+    r.air = A.take<float2>(g->sep_air ? sep_air_scratch(g) : (size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
 }
 
 template <class T>
@@ -165,6 +177,7 @@ extern "C" void emm_grid_destroy(emm_grid *g) {
     if (g->plan_fwd) cufftDestroy(g->plan_fwd);
     if (g->plan_inv_e) cufftDestroy(g->plan_inv_e);
     if (g->plan_inv_h) cufftDestroy(g->plan_inv_h);
+    for (cufftHandle h : g->sp) if (h) cufftDestroy(h);
   }
   delete g;
 }
@@ -239,8 +252,12 @@ extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, voi
     }
     cufftHandle pl[3] = {g->plan_fwd, g->plan_inv_e, g->plan_inv_h};
     const int batch[3] = {1, g->r - 1, g->r};
+    for (int q = 0; q < 8; ++q)
+      if (g->sep_air && g->sp[q] &&
+          (cufftSetStream(g->sp[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(g->sp[q], g->T.sp_ws[q]) != CUFFT_SUCCESS))
+        return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
     for (int q = 0; q < 3; ++q) {
-      if (batch[q] < 1) continue;
+      if (batch[q] < 1 || g->sep_air) continue;
       if (cufftSetStream(pl[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(pl[q], g->T.fft_ws[q]) != CUFFT_SUCCESS)
         return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
     }

@@ -12,7 +12,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.environ.get("EMM_B200_LIB") or os.path.join(_HERE, "libemm_b200.so")   # override: kernel-variant experiments
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_air.cu", "emm_run.cu")]
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu")]
 _HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
 
