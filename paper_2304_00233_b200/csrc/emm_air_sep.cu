@@ -29,8 +29,8 @@ namespace emm {
 namespace {
 
 struct SepArgs {
-  int N1, N2, P1, M1, M2, K1, k0, nlev, nrows_f, is_h;
-  long long PS;
+  int N1, N2, P1, M1, M2, K1, k0, nlev, nrows_f, is_h, nsrc;
+  long long PS, VS;
   float h[kMaxR];
   float scale;
 };
@@ -45,12 +45,13 @@ __device__ __forceinline__ float lag4(const float *__restrict__ p, int s, const 
 // E pass: complex row j = (Ex row j, Ey row j).  H pass: complex row jj = (Hz row 2jj, Hz row 2jj+1).
 __global__ void k_sep_xup(const SepArgs A, const float *__restrict__ fa, const float *__restrict__ fb, const Tab ta, const Tab tb,
                           float2 *__restrict__ XR) {
-  const int m = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
+  const int m = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y, src = blockIdx.z;
   if (m >= A.M1) return;
   const int ja = A.is_h ? 2 * row : row, jb = A.is_h ? 2 * row + 1 : row;
-  const float va = lag4(fa + (size_t)ja * A.P1, ta.s[m], ta.w + 4 * m);
-  const float vb = jb < A.N2 ? lag4(fb + (size_t)jb * A.P1, tb.s[m], tb.w + 4 * m) : 0.f;
-  XR[(size_t)row * A.M1 + m] = make_float2(va, vb);
+  const size_t so = (size_t)src * A.VS;
+  const float va = lag4(fa + so + (size_t)ja * A.P1, ta.s[m], ta.w + 4 * m);
+  const float vb = jb < A.N2 ? lag4(fb + so + (size_t)jb * A.P1, tb.s[m], tb.w + 4 * m) : 0.f;
+  XR[((size_t)src * A.nrows_f + row) * A.M1 + m] = make_float2(va, vb);
 }
 
 // XT[k][row] holds the transform of (a + i b); the transform of the real row a is (U(k) + conj U(-k)) / 2, of b
@@ -61,9 +62,11 @@ __device__ __forceinline__ float2 real_part_spectrum(const float2 *__restrict__ 
 }
 
 __global__ void k_sep_yup(const SepArgs A, const float2 *__restrict__ XT, const Tab t0, const Tab t1, float2 *__restrict__ V) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y, c = blockIdx.z;
+  const int ncomp = A.is_h ? 1 : 2;
+  const int n = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y, src = blockIdx.z / ncomp, c = blockIdx.z - src * ncomp;
   if (n >= A.M2) return;
   const Tab t = c ? t1 : t0;
+  const int nrows = A.nsrc * A.nrows_f, r0 = src * A.nrows_f;
   const int s = t.s[n];
   const float4 w = *reinterpret_cast<const float4 *>(t.w + 4 * n);
   const float wq[4] = {w.x, w.y, w.z, w.w};
@@ -71,22 +74,24 @@ __global__ void k_sep_yup(const SepArgs A, const float2 *__restrict__ XT, const 
 #pragma unroll
   for (int b = 0; b < 4; ++b) {
     const int j = s + b;
-    const float2 a = A.is_h ? real_part_spectrum(XT, A.nrows_f, A.M1, k1, j >> 1, j & 1) : real_part_spectrum(XT, A.nrows_f, A.M1, k1, j, c);
+    const float2 a = A.is_h ? real_part_spectrum(XT, nrows, A.M1, k1, r0 + (j >> 1), j & 1) : real_part_spectrum(XT, nrows, A.M1, k1, r0 + j, c);
     acc.x = fmaf(wq[b], a.x, acc.x);
     acc.y = fmaf(wq[b], a.y, acc.y);
   }
-  V[((size_t)c * A.K1 + k1) * A.M2 + n] = acc;
+  V[(((size_t)src * 2 + c) * A.K1 + k1) * A.M2 + n] = acc;
 }
 
 // E (Eq. 21): level m of component c is e^{-k_h h_m} times its surface spectrum.  H (Eq. 17-20): Hx^ = i kx/k_h
 // e^{-k_h h} Hz^, Hy^ likewise with ky; odd filters vanish at their Nyquist bin [R10].  W[o][lev][k1][n].
 __global__ void k_sep_filter(const SepArgs A, const float *__restrict__ kx, const float *__restrict__ ky, const float2 *__restrict__ V,
                              float2 *__restrict__ W) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y;
+  const int n = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y, src = blockIdx.z;
   if (n >= A.M2) return;
   const float qx = kx[k1], qy = ky[n];
   const float kh = sqrtf(qx * qx + qy * qy);
   const size_t plane = (size_t)A.K1 * A.M2, o0 = (size_t)k1 * A.M2 + n;
+  V += (size_t)src * 2 * plane;
+  W += (size_t)src * 2 * A.nlev * plane;
   if (!A.is_h) {
     const float2 v0 = V[o0], v1 = V[plane + o0];
     for (int m = 0; m < A.nlev; ++m) {
@@ -109,9 +114,10 @@ __global__ void k_sep_filter(const SepArgs A, const float *__restrict__ kx, cons
 // ZT[k][lev*N2 + j] = Za + i Zb for k = k1 and conj(Za) + i conj(Zb) for k = M1 - k1, with Za, Zb the columns of the
 // two output components interpolated back to their own y lattices.
 __global__ void k_sep_ydown(const SepArgs A, const float2 *__restrict__ W, const Tab t0, const Tab t1, float2 *__restrict__ ZT) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y, lev = blockIdx.z;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y, src = blockIdx.z / A.nlev, lev = blockIdx.z - src * A.nlev;
   if (j >= A.N2) return;
   const size_t plane = (size_t)A.K1 * A.M2;
+  W += (size_t)src * 2 * A.nlev * plane;
   const float2 *ra = W + (size_t)lev * plane + (size_t)k1 * A.M2, *rb = W + (size_t)(A.nlev + lev) * plane + (size_t)k1 * A.M2;
   const int sa = t0.s[j], sb = t1.s[j];
   const float4 wa = *reinterpret_cast<const float4 *>(t0.w + 4 * j), wb = *reinterpret_cast<const float4 *>(t1.w + 4 * j);
@@ -121,59 +127,64 @@ __global__ void k_sep_ydown(const SepArgs A, const float2 *__restrict__ W, const
                                 fmaf(wa.x, a0.y, fmaf(wa.y, a1.y, fmaf(wa.z, a2.y, wa.w * a3.y))));
   const float2 zb = make_float2(fmaf(wb.x, b0.x, fmaf(wb.y, b1.x, fmaf(wb.z, b2.x, wb.w * b3.x))),
                                 fmaf(wb.x, b0.y, fmaf(wb.y, b1.y, fmaf(wb.z, b2.y, wb.w * b3.y))));
-  const size_t nrows = (size_t)A.nlev * A.N2, col = (size_t)lev * A.N2 + j;
+  const size_t nrows = (size_t)A.nsrc * A.nlev * A.N2, col = ((size_t)src * A.nlev + lev) * A.N2 + j;
   ZT[(size_t)k1 * nrows + col] = make_float2(za.x - zb.y, za.y + zb.x);
   if (k1 > 0 && A.M1 - k1 != k1) ZT[(size_t)(A.M1 - k1) * nrows + col] = make_float2(za.x + zb.y, zb.x - za.y);
 }
 
 __global__ void k_sep_xdown(const SepArgs A, const float2 *__restrict__ XR, const Tab ta, const Tab tb, float *__restrict__ fa,
                             float *__restrict__ fb) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, lev = blockIdx.z;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, src = blockIdx.z / A.nlev, lev = blockIdx.z - src * A.nlev;
   if (i >= A.N1) return;
-  const float2 *p = XR + ((size_t)lev * A.N2 + j) * A.M1;
+  const float2 *p = XR + (((size_t)src * A.nlev + lev) * A.N2 + j) * A.M1;
   const int ia = ta.s[i], ib = tb.s[i];
   const float4 wa = *reinterpret_cast<const float4 *>(ta.w + 4 * i), wb = *reinterpret_cast<const float4 *>(tb.w + 4 * i);
-  const size_t o = (size_t)(A.k0 - 1 - lev) * A.PS + (size_t)j * A.P1 + i;
+  const size_t o = (size_t)src * A.VS + (size_t)(A.k0 - 1 - lev) * A.PS + (size_t)j * A.P1 + i;
   fa[o] = fmaf(wa.x, p[ia].x, fmaf(wa.y, p[ia + 1].x, fmaf(wa.z, p[ia + 2].x, wa.w * p[ia + 3].x)));
   fb[o] = fmaf(wb.x, p[ib].y, fmaf(wb.y, p[ib + 1].y, fmaf(wb.z, p[ib + 2].y, wb.w * p[ib + 3].y)));
 }
 
 }  // namespace
 
-// scratch (float2 elements): XR rows [r*N2][M1] | XT / ZT [M1][r*N2] | V [2][K1][M2] | W [2r][K1][M2]
-size_t sep_air_scratch(const emm_grid *g) {
+// scratch (float2 elements) per source: XR rows [r*N2][M1] | XT / ZT [M1][r*N2] | V [2][K1][M2] | W [2r][K1][M2];
+// every array carries a leading source dimension (all unfinished and finished sources go through one launch)
+size_t sep_air_scratch(const emm_grid *g, int nsrc) {
   const size_t K1 = (size_t)g->M1 / 2 + 1, rows = (size_t)g->r * g->N[1];
-  return 2 * rows * g->M1 + (size_t)(2 + 2 * g->r) * K1 * g->M2;
+  return (size_t)nsrc * (2 * rows * g->M1 + (size_t)(2 + 2 * g->r) * K1 * g->M2);
 }
 
-// 1-D batched plans: 0/1 x forward (E/H), 2/3 y forward, 4/5 y inverse, 6/7 x inverse.  The x plans write (forward) or
-// read (inverse) the transposed layout [k][row] through cuFFT's strided data layout.
-int sep_air_make_plans(emm_grid *g) {
+// 1-D batched plans for nsrc sources: 0/1 x forward (E/H), 2/3 y forward, 4/5 y inverse, 6/7 x inverse.  The x plans
+// write (forward) or read (inverse) the transposed layout [k][row] through cuFFT's strided data layout.
+int sep_air_make_plans(emm_grid *g, int nsrc) {
+  if (g->sp_nsrc == nsrc) return 0;
+  for (cufftHandle &h : g->sp) { if (h) cufftDestroy(h); h = 0; }
+  g->sp_nsrc = 0;
   const int M1 = g->M1, M2 = g->M2, N2 = g->N[1], K1 = M1 / 2 + 1, R = g->r;
   for (int q = 0; q < 8; ++q) {
     const int is_h = q & 1, nlev = is_h ? R : R - 1;
     g->sp_ws[q] = 0;
-    g->sp[q] = 0;
     int n[1], batch, istride = 1, idist, ostride = 1, odist;
     if (q < 2) {                       // x forward: rows [row][M1] -> XT[k][row]
-      batch = is_h ? (N2 + 1) / 2 : N2;
+      batch = nsrc * (is_h ? (N2 + 1) / 2 : N2);
       n[0] = M1; idist = M1; ostride = batch; odist = 1;
-    } else if (q < 4) {                // y forward, in place on V
-      batch = (is_h ? 1 : 2) * K1;
+    } else if (q < 4) {                // y forward, in place on V (two planes per source; the H pass fills one)
+      batch = nsrc * 2 * K1;
       n[0] = M2; idist = odist = M2;
     } else if (q < 6) {                // y inverse, in place on W
-      batch = 2 * nlev * K1;
+      batch = nsrc * 2 * nlev * K1;
       n[0] = M2; idist = odist = M2;
     } else {                           // x inverse: ZT[k][row] -> rows [row][M1]
-      batch = nlev * N2;
+      batch = nsrc * nlev * N2;
       n[0] = M1; istride = batch; idist = 1; odist = M1;
     }
     if (batch < 1) continue;
+    if (q == 3 && nsrc == 1) batch = K1;                                  // single source, H pass: only the first plane is live
     if (cufftCreate(&g->sp[q]) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftCreate failed (no CUDA device?)");
     cufftSetAutoAllocation(g->sp[q], 0);
     if (cufftMakePlanMany(g->sp[q], 1, n, n, istride, idist, n, ostride, odist, CUFFT_C2C, batch, &g->sp_ws[q]) != CUFFT_SUCCESS)
       return fail(EMM_ECUDA, "cufftMakePlanMany failed for %d transforms of length %d", batch, n[0]);
   }
+  g->sp_nsrc = nsrc;
   return 0;
 }
 
@@ -201,29 +212,31 @@ int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cu
   const int out_x[2] = {is_h ? 0 : 1, is_h ? 1 : 0}, out_y[2] = {is_h ? 1 : 0, is_h ? 0 : 1};
   auto ta = [&](int axis, int lat) { return Tab{g->T.ta_start[axis][lat], g->T.ta_w[axis][lat]}; };
   auto fa = [&](int axis, int lat) { return Tab{g->T.fa_start[axis][lat], g->T.fa_w[axis][lat]}; };
-  const size_t rows = (size_t)R * a.N2, plane = (size_t)a.K1 * a.M2;
-  float2 *XR = r.air, *XT = XR + rows * a.M1, *V = XT + rows * a.M1, *W = V + 2 * plane;
-  const int ncomp = is_h ? 1 : 2;
+  a.nsrc = s.nsrc;
+  a.VS = g->dg.VS;
+  if (g->sp_nsrc != s.nsrc) return fail(EMM_EINVAL, "air boundary: plans were made for %d sources, the run has %d", g->sp_nsrc, s.nsrc);
+  const size_t rows = (size_t)s.nsrc * R * a.N2, plane = (size_t)a.K1 * a.M2;
+  float2 *XR = r.air, *XT = XR + rows * a.M1, *V = XT + rows * a.M1, *W = V + (size_t)s.nsrc * 2 * plane;
+  const int ncomp = is_h ? 1 : 2, ns = s.nsrc;
   const dim3 blk(128, 1, 1);
-  for (int src = 0; src < s.nsrc; ++src) {
-    const size_t vo = (size_t)src * g->dg.VS, so = vo + (size_t)g->k0 * a.PS;
-    const float *f_a = (is_h ? s.H[2] : s.E[0]) + so, *f_b = (is_h ? s.H[2] : s.E[1]) + so;
-    k_sep_xup<<<dim3((a.M1 + 127) / 128, a.nrows_f, 1), blk, 0, st>>>(a, f_a, f_b, ta(0, in_x[0]), ta(0, in_x[1]), XR);
-    EMM_SEP_CHECK(g, "k_sep_xup");
-    if (cufftExecC2C(g->sp[0 + is_h], XR, XT, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x forward) failed");
-    k_sep_yup<<<dim3((a.M2 + 127) / 128, a.K1, ncomp), blk, 0, st>>>(a, XT, ta(1, in_y[0]), ta(1, in_y[1]), V);
-    EMM_SEP_CHECK(g, "k_sep_yup");
-    if (cufftExecC2C(g->sp[2 + is_h], V, V, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (y forward) failed");
-    k_sep_filter<<<dim3((a.M2 + 127) / 128, a.K1, 1), blk, 0, st>>>(a, g->T.kx, g->T.ky, V, W);
-    EMM_SEP_CHECK(g, "k_sep_filter");
-    if (cufftExecC2C(g->sp[4 + is_h], W, W, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (y inverse) failed");
-    k_sep_ydown<<<dim3((a.N2 + 127) / 128, a.K1, nlev), blk, 0, st>>>(a, W, fa(1, out_y[0]), fa(1, out_y[1]), XT);
-    EMM_SEP_CHECK(g, "k_sep_ydown");
-    if (cufftExecC2C(g->sp[6 + is_h], XT, XR, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x inverse) failed");
-    k_sep_xdown<<<dim3((a.N1 + 127) / 128, a.N2, nlev), blk, 0, st>>>(a, XR, fa(0, out_x[0]), fa(0, out_x[1]),
-                                                                        (is_h ? s.H[0] : s.E[0]) + vo, (is_h ? s.H[1] : s.E[1]) + vo);
-    EMM_SEP_CHECK(g, "k_sep_xdown");
-  }
+  // sources finished earlier keep their ghost planes: harmless, nothing reads them any more
+  const size_t so = (size_t)g->k0 * a.PS;
+  const float *f_a = (is_h ? s.H[2] : s.E[0]) + so, *f_b = (is_h ? s.H[2] : s.E[1]) + so;
+  k_sep_xup<<<dim3((a.M1 + 127) / 128, a.nrows_f, ns), blk, 0, st>>>(a, f_a, f_b, ta(0, in_x[0]), ta(0, in_x[1]), XR);
+  EMM_SEP_CHECK(g, "k_sep_xup");
+  if (cufftExecC2C(g->sp[0 + is_h], XR, XT, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x forward) failed");
+  k_sep_yup<<<dim3((a.M2 + 127) / 128, a.K1, ncomp * ns), blk, 0, st>>>(a, XT, ta(1, in_y[0]), ta(1, in_y[1]), V);
+  EMM_SEP_CHECK(g, "k_sep_yup");
+  if (cufftExecC2C(g->sp[2 + is_h], V, V, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (y forward) failed");
+  k_sep_filter<<<dim3((a.M2 + 127) / 128, a.K1, ns), blk, 0, st>>>(a, g->T.kx, g->T.ky, V, W);
+  EMM_SEP_CHECK(g, "k_sep_filter");
+  if (cufftExecC2C(g->sp[4 + is_h], W, W, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (y inverse) failed");
+  k_sep_ydown<<<dim3((a.N2 + 127) / 128, a.K1, nlev * ns), blk, 0, st>>>(a, W, fa(1, out_y[0]), fa(1, out_y[1]), XT);
+  EMM_SEP_CHECK(g, "k_sep_ydown");
+  if (cufftExecC2C(g->sp[6 + is_h], XT, XR, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x inverse) failed");
+  k_sep_xdown<<<dim3((a.N1 + 127) / 128, a.N2, nlev * ns), blk, 0, st>>>(a, XR, fa(0, out_x[0]), fa(0, out_x[1]), is_h ? s.H[0] : s.E[0],
+                                                                          is_h ? s.H[1] : s.E[1]);
+  EMM_SEP_CHECK(g, "k_sep_xdown");
   return 0;
 }
 

@@ -82,7 +82,6 @@ struct DevTables {             // device pointers of the per-grid region
   float *ta_w[2][2], *fa_w[2][2];
   float *kx, *ky;                          // signed wavenumbers of the FFT plane
   void *fft_ws[3];
-  void *sp_ws[8];                          // work areas of the separable route's 1-D plans
 };
 
 struct Run;
@@ -125,6 +124,7 @@ struct emm_grid {
   size_t fft_ws[3] = {0, 0, 0};             // cuFFT work-area bytes: forward, inverse (E), inverse (H)
   cufftHandle sp[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // separable route: batched 1-D plans (emm_air_sep.cu)
   size_t sp_ws[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  int sp_nsrc = 0;                       // number of sources the plans in sp[] are batched for
   double vref[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // CPML reference speed per face [R5]
   emm::Run *run = nullptr;
   long long launches = 0;

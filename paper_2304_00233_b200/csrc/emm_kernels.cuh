@@ -25,6 +25,7 @@ struct DevRun {
   int nrec_nodes = 0;
   // air boundary scratch: complex planes [1 + r][M2][M1] (plane route) or sep_air_scratch() elements (separable route)
   float2 *air = nullptr;
+  void *sp_ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // cuFFT work areas of the separable route
 };
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
@@ -38,8 +39,8 @@ int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nrec_node
 int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
 // separable route of the same boundary for non-uniform x-y (emm_air_sep.cu); launch_air dispatches to it when g->sep_air
 int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
-size_t sep_air_scratch(const emm_grid *g);
-int sep_air_make_plans(emm_grid *g);
+size_t sep_air_scratch(const emm_grid *g, int nsrc);
+int sep_air_make_plans(emm_grid *g, int nsrc);
 // model: effective medium (Eq. 26) -> min sigma (for Eq. 15) and dt/eps
 int launch_sigma_min(emm_grid *g, const float *d_sh, const float *d_sv, double *d_min);
 int launch_make_ce(emm_grid *g, const float *d_sh, const float *d_sv, double scale);

@@ -50,9 +50,7 @@ static int ensure_plans(emm_grid *g) {
   // transforms, for A/B measurements)
   const char *force = std::getenv("EMM_AIR_PLANE");
   g->sep_air = !g->uniform_xy && !(force && force[0] == '1');
-  if (g->sep_air) {
-    const int rc = sep_air_make_plans(g);
-    if (rc) return rc;
+  if (g->sep_air) {             // its plans are batched over the sources of a run: made by emm_workspace_bytes / emm_run_begin
     g->have_plans = true;
     return 0;
   }
@@ -95,8 +93,6 @@ static void layout_fixed(emm_grid *g, Arena &A) {
           g->T.fa_w[a][l] = A.take<float>((size_t)4 * g->N[a]);
         }
     for (int q = 0; q < 3; ++q) g->T.fft_ws[q] = A.take<char>(g->fft_ws[q] + 256);
-    if (g->sep_air)
-      for (int q = 0; q < 8; ++q) g->T.sp_ws[q] = A.take<char>(g->sp_ws[q] + 256);
   }
 }
 
@@ -147,7 +143,9 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps,
   r.rec_idx = A.take<int>((size_t)6 * nrec * np3);
   r.rec_val = A.take<float2>((size_t)nsrc * nf * 6 * nrec * np3);
   if (g->top == EMM_TOP_AIR)   // FFT planes [1 + r][M2][M1] + (non-uniform x-y) the x-interpolated rows [N2][M1]
-    r.air = A.take<float2>(g->sep_air ? sep_air_scratch(g) : (size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
+    r.air = A.take<float2>(g->sep_air ? sep_air_scratch(g, nsrc) : (size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
+  if (g->top == EMM_TOP_AIR && g->sep_air)
+    for (int q = 0; q < 8; ++q) r.sp_ws[q] = A.take<char>(g->sp_ws[q] + 256);
 }
 
 template <class T>
@@ -186,6 +184,7 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   emm_grid *g = const_cast<emm_grid *>(cg);
   if (!g || nsrc < 1 || nfreq < 0 || nrec < 0) { fail(EMM_EINVAL, "emm_workspace_bytes: bad arguments"); return 0; }
   if (ensure_plans(g)) return 0;
+  if (g->sep_air && sep_air_make_plans(g, nsrc)) return 0;
   if (max_steps <= 0) max_steps = 100000;
   const DevTables keep = g->T;       // dry-run layout: the live grid's pointers are restored below
   Arena A;
@@ -252,10 +251,6 @@ extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, voi
     }
     cufftHandle pl[3] = {g->plan_fwd, g->plan_inv_e, g->plan_inv_h};
     const int batch[3] = {1, g->r - 1, g->r};
-    for (int q = 0; q < 8; ++q)
-      if (g->sep_air && g->sp[q] &&
-          (cufftSetStream(g->sp[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(g->sp[q], g->T.sp_ws[q]) != CUFFT_SUCCESS))
-        return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
     for (int q = 0; q < 3; ++q) {
       if (batch[q] < 1 || g->sep_air) continue;
       if (cufftSetStream(pl[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(pl[q], g->T.fft_ws[q]) != CUFFT_SUCCESS)
@@ -593,9 +588,16 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
         }
       }
     // workspace layout
+    if (g->top == EMM_TOP_AIR && g->sep_air && (rc = sep_air_make_plans(g, nsrc))) { free_run(g); return rc; }
     Arena A;
     A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
     layout_run(g, A, nsrc, nf, R->table_steps, nrec, chk.size(), R->ds, R->dr);
+    if (g->top == EMM_TOP_AIR && g->sep_air && !A.overflow)
+      for (int q = 0; q < 8; ++q)
+        if (g->sp[q] && (cufftSetStream(g->sp[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(g->sp[q], R->dr.sp_ws[q]) != CUFFT_SUCCESS)) {
+          free_run(g);
+          return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
+        }
     R->ds.dft_every = R->dtft_every;
     if (A.overflow) { size_t need = A.off; free_run(g); return fail(EMM_ENOMEM, "emm_run_begin: workspace too small (%zu bytes needed)", need); }
     // zero the whole run region (fields, psi, accumulators, flags)
