@@ -73,6 +73,12 @@ typedef struct {
                       (dt is set by the fastest cell, L251-260), so G = F/J' changes by ~1e-9 while the dominant
                       accumulator traffic drops by (1 - 1/m).  0, 1: every step, as the paper does (L454);
                       < 0: the largest safe m = floor(1/(dt (3 fmax + 2 sqrt(max f * f0))))                      */
+  int sparse_dft;  /* 1: receivers-only DTFT -- the sums of Eq. 25 are kept only at the nodes of the receivers'
+                      interpolation stencils (fp64 accumulators fed by the fp32 fields) and on the check set; no
+                      full-grid accumulator exists (emm_get of EMM_GET_F_* fails with EMM_EINVAL), the update kernels
+                      run without the 96*nf B/node term.  Same sums at those nodes, so emm_run returns the same
+                      Green's functions and step counts; for runs that only want receiver data.
+                      0: accumulators for every frequency on the whole DTFT box, as the paper does (L454)            */
 } emm_run_opts;
 
 /* integer grid facts for emm_grid_info(): */

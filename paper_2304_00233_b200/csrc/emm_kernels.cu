@@ -427,6 +427,27 @@ __global__ void k_check_acc(const DevGrid g, const DevState s, const int *__rest
   a.y += u * t.y;
 }
 
+// ---- receivers-only DTFT: Eq. 25 at the nodes of the receivers' interpolation stencils only, fp64 sums of the fp32
+// fields, every frequency.  Runs where k_check_acc runs: after the E update (E at (it+1/2) dt) and before the H update
+// (H at it dt), [R6]. ----
+__global__ void k_rec_acc(const DevGrid g, const DevState s, const int *__restrict__ ridx, const int nn, const int nf,
+                          double2 *__restrict__ RA, const double2 *__restrict__ twE, const double2 *__restrict__ twH) {
+  const int src = blockIdx.z, c = blockIdx.y;
+  if (s.done[src]) return;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= nn) return;
+  const int it = *s.it;
+  if (it % s.dft_every != 0) return;
+  const float *fld = (c < 3 ? s.E[c] : s.H[c - 3]) + (size_t)src * g.VS;
+  const double u = (double)fld[ridx[(size_t)c * nn + p]];
+  const double2 *tw = (c < 3 ? twE : twH) + (size_t)it * nf;
+  for (int f = 0; f < nf; ++f) {
+    double2 &a = RA[(((size_t)src * nf + f) * 6 + c) * nn + p];
+    a.x += u * tw[f].x;
+    a.y += u * tw[f].y;
+  }
+}
+
 // relative change since the previous check: warp shuffle + block reduction + one atomic per block
 __global__ void k_check_reduce(const DevState s, const int nchk, const double2 *__restrict__ C, double2 *__restrict__ Cprev,
                                double *__restrict__ red) {
@@ -613,6 +634,14 @@ int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r) {
   dim3 grid((r.nchk + 255) / 256, 6, s.nsrc);
   k_check_acc<<<grid, 256, 0, g->stream>>>(g->dg, s, r.chk_idx, r.nchk, r.C, r.twE64, r.twH64);
   EMM_LAUNCH_CHECK(g, "k_check_acc");
+  return 0;
+}
+
+int launch_rec_acc(emm_grid *g, const DevState &s, const DevRun &r) {
+  if (r.nf_rec <= 0 || r.nrec_nodes <= 0) return 0;
+  dim3 grid((r.nrec_nodes + 255) / 256, 6, s.nsrc);
+  k_rec_acc<<<grid, 256, 0, g->stream>>>(g->dg, s, r.rec_idx, r.nrec_nodes, r.nf_rec, r.RA, r.twEf, r.twHf);
+  EMM_LAUNCH_CHECK(g, "k_rec_acc");
   return 0;
 }
 

@@ -23,6 +23,10 @@ struct DevRun {
   int *rec_idx = nullptr;      // [6][nrec*np^3]
   float2 *rec_val = nullptr;   // [nsrc][nf][6][nrec*np^3]
   int nrec_nodes = 0;
+  // receivers-only DTFT (emm_run_opts.sparse_dft): fp64 accumulators at the receiver stencil nodes
+  double2 *RA = nullptr;       // [nsrc][nf][6][nrec*np^3]
+  double2 *twEf = nullptr, *twHf = nullptr;   // [max_steps][nf] twiddles of every frequency, fp64
+  int nf_rec = 0;              // number of frequencies in RA (0: mode off)
   // air boundary scratch: complex planes [1 + r][M2][M1] (plane route) or sep_air_scratch() elements (separable route)
   float2 *air = nullptr;
   void *sp_ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // cuFFT work areas of the separable route
@@ -32,6 +36,7 @@ struct DevRun {
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st);
 int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
+int launch_rec_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);
 int launch_step_end(emm_grid *g, const DevState &s);
 int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nrec_nodes);

@@ -19,6 +19,7 @@ struct Run {
   double fmax = 0, beta = 0, t0 = 0, tol = 1e-6;
   int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
   int it_min = 0, it_host = 0, table_steps = 0, dtft_every = 1;
+  bool sparse = false;                   // receivers-only DTFT (emm_run_opts.sparse_dft)
   std::vector<double> wav, wavh;            // s(it dt), s((it+1/2) dt) rounded to fp32 (what the device injects)
   std::vector<int> mag;                     // [nsrc] 1 = magnetic dipole
   bool any_mag = false, any_el = false;
@@ -105,7 +106,8 @@ static size_t chk_count(const emm_grid *g, int check_set) {
 }
 
 // per-run region
-static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps, int nrec, size_t nchk, DevState &s, DevRun &r) {
+// nf = frequencies with full-grid accumulators, nf_rec = frequencies kept at the receiver stencils only (one of the two is 0)
+static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int table_steps, int nrec, size_t nchk, DevState &s, DevRun &r) {
   const size_t V = vol(g), PS = (size_t)g->P1 * g->N[1];
   const int np = std::max(2 * g->r, 4);
   const size_t np3 = (size_t)np * np * np;
@@ -142,6 +144,10 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int table_steps,
   r.status = A.take<int>(nsrc);
   r.rec_idx = A.take<int>((size_t)6 * nrec * np3);
   r.rec_val = A.take<float2>((size_t)nsrc * nf * 6 * nrec * np3);
+  r.nf_rec = nf_rec;
+  r.RA = A.take<double2>((size_t)nsrc * nf_rec * 6 * nrec * np3);
+  r.twEf = A.take<double2>((size_t)table_steps * nf_rec);
+  r.twHf = A.take<double2>((size_t)table_steps * nf_rec);
   if (g->top == EMM_TOP_AIR)   // FFT planes [1 + r][M2][M1] + (non-uniform x-y) the x-interpolated rows [N2][M1]
     r.air = A.take<float2>(g->sep_air ? sep_air_scratch(g, nsrc) : (size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
   if (g->top == EMM_TOP_AIR && g->sep_air)
@@ -192,7 +198,7 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   const size_t fixed = A.off;
   DevState s{};
   DevRun r{};
-  layout_run(g, A, nsrc, nfreq, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), s, r);
+  layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), s, r);   // the full-grid mode is the larger one
   g->T = keep;
   // emm_model_set stages the raw model in the run region: make sure it fits as well
   const size_t stage = fixed + 2 * ((size_t)g->nc[0] * g->nc[1] * g->nc[2] * sizeof(float) + 256) + 512;
@@ -415,6 +421,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
     if (g->top != EMM_TOP_AIR) {
       if ((rc = launch_update(g, R->ds, 0, 0, M))) return rc;                 // L476-479 + E part of L483
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                // check-set part of L483
+      if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
       if ((rc = launch_update(g, R->ds, 1, 0, M))) return rc;                 // H part of L483 + L486-489
     } else if (g->prof || no_overlap) {
       // one thing after the other (per-kernel timing, or EMM_NO_OVERLAP): the boundary still runs on its own stream
@@ -423,6 +430,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
       CU(cudaEventRecord(g->ev[1], B)); CU(cudaStreamWaitEvent(M, g->ev[1], 0));
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
+      if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
       if ((rc = launch_update(g, R->ds, 1, 0, M))) return rc;
       CU(cudaEventRecord(g->ev[2], M)); CU(cudaStreamWaitEvent(B, g->ev[2], 0));
       if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
@@ -438,6 +446,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       CU(cudaEventRecord(g->ev[2], M));
       CU(cudaStreamWaitEvent(M, g->ev[1], 0));                                // H bulk and the check set read surface-chunk E
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
+      if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
       CU(cudaEventRecord(g->ev[4], M));
       if ((rc = launch_update(g, R->ds, 1, 2, M))) return rc;                 // H, bulk
       CU(cudaStreamWaitEvent(B, g->ev[2], 0)); CU(cudaStreamWaitEvent(B, g->ev[4], 0));
@@ -535,6 +544,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     R->check_every = o->check_every > 0 ? o->check_every : 100;
     R->check_set = o->check_set;
     R->dtft_every = o->dtft_every > 1 ? o->dtft_every : 1;
+    R->sparse = o->sparse_dft != 0 && nf > 0;
     if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
     R->table_steps = (R->fixed_steps ? R->fixed_steps : R->max_steps) + 1;
     double fhi = 0;
@@ -591,7 +601,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     if (g->top == EMM_TOP_AIR && g->sep_air && (rc = sep_air_make_plans(g, nsrc))) { free_run(g); return rc; }
     Arena A;
     A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
-    layout_run(g, A, nsrc, nf, R->table_steps, nrec, chk.size(), R->ds, R->dr);
+    layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), R->ds, R->dr);
     if (g->top == EMM_TOP_AIR && g->sep_air && !A.overflow)
       for (int q = 0; q < 8; ++q)
         if (g->sp[q] && (cufftSetStream(g->sp[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(g->sp[q], R->dr.sp_ws[q]) != CUFFT_SUCCESS)) {
@@ -606,8 +616,9 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     // wavelet and twiddles (fp64 -> fp32), [R6]/[R8]
     const int T = R->table_steps;
     std::vector<float> wav(T);
-    std::vector<float2> twE((size_t)T * nf), twH((size_t)T * nf);
-    std::vector<double2> twE64(T), twH64(T);
+    const int nfg = R->sparse ? 0 : nf, nfr = R->sparse ? nf : 0;      // frequencies on the grid / at the receivers only
+    std::vector<float2> twE((size_t)T * nfg), twH((size_t)T * nfg);
+    std::vector<double2> twE64(T), twH64(T), twEf((size_t)T * nfr), twHf((size_t)T * nfr);
     R->wav.resize(T);
     R->wavh.resize(T);
     std::vector<float> wavh(T);
@@ -621,15 +632,21 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
       for (int f = 0; f < nf; ++f) {
         const std::complex<double> I(0, 1);
         const std::complex<double> h = std::exp(I * R->wp[f] * t), e = std::exp(I * R->wp[f] * (((double)it + 0.5) * g->dt));
-        twH[(size_t)it * nf + f] = make_float2((float)h.real(), (float)h.imag());
-        twE[(size_t)it * nf + f] = make_float2((float)e.real(), (float)e.imag());
+        if (R->sparse) {
+          twHf[(size_t)it * nf + f] = make_double2(h.real(), h.imag());
+          twEf[(size_t)it * nf + f] = make_double2(e.real(), e.imag());
+        } else {
+          twH[(size_t)it * nf + f] = make_float2((float)h.real(), (float)h.imag());
+          twE[(size_t)it * nf + f] = make_float2((float)e.real(), (float)e.imag());
+        }
         if (f == R->fmin) { twH64[it] = make_double2(h.real(), h.imag()); twE64[it] = make_double2(e.real(), e.imag()); }
       }
     }
     if ((rc = upload(g, const_cast<float *>(R->ds.wavh), wavh))) { free_run(g); return rc; }
     if ((rc = upload(g, const_cast<float *>(R->ds.wav), wav)) || (rc = upload(g, const_cast<float2 *>(R->ds.twE), twE)) ||
         (rc = upload(g, const_cast<float2 *>(R->ds.twH), twH)) || (rc = upload(g, R->dr.twE64, twE64)) ||
-        (rc = upload(g, R->dr.twH64, twH64)) || (rc = upload(g, R->dr.chk_idx, chk))) { free_run(g); return rc; }
+        (rc = upload(g, R->dr.twH64, twH64)) || (rc = upload(g, R->dr.chk_idx, chk)) ||
+        (rc = upload(g, R->dr.twEf, twEf)) || (rc = upload(g, R->dr.twHf, twHf))) { free_run(g); return rc; }
 
     // CPML tables
     DevGrid &d = g->dg;
@@ -687,6 +704,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     // receiver gather list
     std::vector<int> ridx((size_t)6 * nrec * np3);
     R->nrec_nodes = (int)(nrec * np3);
+    R->dr.nrec_nodes = R->nrec_nodes;
     for (int c = 0; c < 6; ++c) for (int q = 0; q < nrec; ++q) {
       const Stencil1 *st = &R->rst[((size_t)q * 6 + c) * 3];
       size_t n = 0;
@@ -745,10 +763,18 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
   if (!out_ || R->nrec == 0) return 0;
   const int nf = R->nf, np = R->np, nn = R->nrec_nodes;
   const size_t np3 = (size_t)np * np * np;
-  if ((rc = launch_gather(g, R->ds, R->dr, nn))) return rc;
-  std::vector<float2> val((size_t)R->nsrc * nf * 6 * nn);
-  CU(cudaMemcpyAsync(val.data(), R->dr.rec_val, val.size() * sizeof(float2), cudaMemcpyDeviceToHost, g->stream));
-  CU(cudaStreamSynchronize(g->stream));
+  // accumulators at the receiver stencil nodes: gathered from the full-grid F, or the fp64 sums of the receivers-only mode
+  std::vector<double2> val((size_t)R->nsrc * nf * 6 * nn);
+  if (R->sparse) {
+    CU(cudaMemcpyAsync(val.data(), R->dr.RA, val.size() * sizeof(double2), cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+  } else {
+    if ((rc = launch_gather(g, R->ds, R->dr, nn))) return rc;
+    std::vector<float2> v32(val.size());
+    CU(cudaMemcpyAsync(v32.data(), R->dr.rec_val, v32.size() * sizeof(float2), cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    for (size_t n = 0; n < val.size(); ++n) val[n] = make_double2((double)v32[n].x, (double)v32[n].y);
+  }
   std::complex<double> *out = reinterpret_cast<std::complex<double> *>(out_);
   const std::complex<double> I(0, 1);
   for (int s = 0; s < R->nsrc; ++s)
@@ -758,7 +784,7 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
       for (int q = 0; q < R->nrec; ++q)
         for (int c = 0; c < 6; ++c) {
           const Stencil1 *st = &R->rst[((size_t)q * 6 + c) * 3];
-          const float2 *v = &val[(((size_t)s * nf + f) * 6 + c) * nn + (size_t)q * np3];
+          const double2 *v = &val[(((size_t)s * nf + f) * 6 + c) * nn + (size_t)q * np3];
           std::complex<double> acc = 0;
           size_t n = 0;
           for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1, ++n)
@@ -816,6 +842,7 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
   }
   if (what >= EMM_GET_F_E1 && what <= EMM_GET_F_H3) {
     if (ifreq < 0 || ifreq >= R->nf) return fail(EMM_EINVAL, "emm_get: bad ifreq");
+    if (R->sparse) return fail(EMM_EINVAL, "emm_get: no full-grid accumulators in a receivers-only run (sparse_dft)");
     const int c = what - EMM_GET_F_E1;
     float2 *o = static_cast<float2 *>(host_out);
     std::memset(o, 0, sizeof(float2) * (size_t)N1 * N2 * N3);

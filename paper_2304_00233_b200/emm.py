@@ -58,7 +58,7 @@ class Src(C.Structure):
 class RunOpts(C.Structure):
     _fields_ = [("max_steps", C.c_int), ("fixed_steps", C.c_int), ("tol", C.c_double),
                 ("check_every", C.c_int), ("check_set", C.c_int), ("fmax", C.c_double), ("batched", C.c_int),
-                ("dtft_every", C.c_int)]
+                ("dtft_every", C.c_int), ("sparse_dft", C.c_int)]
 
 
 class EmmError(RuntimeError):
@@ -144,7 +144,7 @@ def _ropts(o):
     o = dict(o or {})
     r = RunOpts(int(o.pop("max_steps", 0)), int(o.pop("fixed_steps", 0)), float(o.pop("tol", 0)),
                 int(o.pop("check_every", 0)), int(o.pop("check_set", CHECK_FACES)), float(o.pop("fmax", 0)),
-                int(o.pop("batched", 0)), int(o.pop("dtft_every", 0)))
+                int(o.pop("batched", 0)), int(o.pop("dtft_every", 0)), int(o.pop("sparse_dft", 0)))
     o.pop("sparse_dft", None)
     if o:
         raise TypeError("unknown run options %s" % sorted(o))

@@ -148,6 +148,60 @@ def test_dtft_decimation_matches_oracle(emm, oracle, m):
     assert (np.abs(oa - ob)[big] / np.abs(ob)[big]).max() < 1e-3
 
 
+@pytest.mark.parametrize("m", [0, -1])
+def test_receivers_only_dtft_matches_full_grid_and_oracle(emm, oracle, m):
+    """SURVEY 8f rank 1, second half: sparse_dft keeps the sums of Eq. 25 only at the receivers' stencil nodes (fp64)
+    and on the check set.  Same receivers as the full-grid run and as the oracle, same converged step count, with
+    and without decimation, on the non-uniform grid with the auxiliary-plane air boundary and two batched sources."""
+    w = W.cfg3(oracle.nugrid, nx=36, nz=32, rd=2, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
+    w["receivers"] = _small_receivers()
+    srcs = [((-150.0, 30.0, 950.0), (1.0, 0.2, 0.1)), ((120.0, -60.0, 930.0), (0.1, 1.0, 0.3), "M")]
+    opts = dict(tol=1e-6, check_every=100, dtft_every=m, batched=1)
+    ga, gb = make_grid(emm, w), make_grid(oracle, w)
+    o_full, n_full = ga.run(srcs, w["freqs"], w["receivers"], opts)
+    o_sp, n_sp = ga.run(srcs, w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
+    o_or, n_or = gb.run(srcs, w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
+    assert list(n_sp) == list(n_full) == list(n_or) and min(n_sp) > 0          # integer outputs: exact
+    for s in range(2):
+        for sl in (slice(0, 3), slice(3, 6)):
+            ref = o_or[s][..., sl]
+            big = np.abs(ref) > 1e-3 * np.abs(ref).max()
+            assert big.sum() > 10
+            assert (np.abs(o_sp[s][..., sl] - ref)[big] / np.abs(ref)[big]).max() < 1e-3
+            assert (np.abs(o_full[s][..., sl] - ref)[big] / np.abs(ref)[big]).max() < 1e-3
+    # no full-grid accumulator exists in this mode
+    ga.run_begin(srcs[:1], w["freqs"], w["receivers"], dict(fixed_steps=5, sparse_dft=1))
+    ga.run_steps(5)
+    with pytest.raises(emm.EmmError) as e:
+        ga.get("F_E1")
+    assert e.value.code == emm.EINVAL
+    ga.run_end()
+
+
+def test_plane_and_separable_air_routes_agree(emm, oracle, monkeypatch):
+    """Non-uniform x-y: the separable route (batched 1-D transforms, default) and the plane-sized 2-D route
+    (EMM_AIR_PLANE=1) are the same linear map up to rounding order; both are within the field tolerance of the oracle."""
+    w = W.cfg4(oracle.nugrid, nx=40, nz=36, rd=3, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
+    w["receivers"] = _small_receivers()
+    fields = {}
+    for route in ("0", "1"):
+        monkeypatch.setenv("EMM_AIR_PLANE", route)
+        g = make_grid(emm, w)
+        g.run_begin(w["sources"], w["freqs"], w["receivers"], dict(fixed_steps=150))
+        g.run_steps(150)
+        fields[route] = [g.get(c) for c in ("E1", "E2", "E3", "H1", "H2", "H3")]
+        g.run_end()
+        g.close()
+    monkeypatch.delenv("EMM_AIR_PLANE")
+    for a, b in zip(fields["0"], fields["1"]):
+        assert np.abs(a).max() > 0
+    ne = np.sqrt(sum(np.sum(np.asarray(a, np.float64) ** 2) for a in fields["0"][:3]))
+    nh = np.sqrt(sum(np.sum(np.asarray(a, np.float64) ** 2) for a in fields["0"][3:]))
+    de = np.sqrt(sum(np.sum((np.asarray(a, np.float64) - b) ** 2) for a, b in zip(fields["0"][:3], fields["1"][:3])))
+    dh = np.sqrt(sum(np.sum((np.asarray(a, np.float64) - b) ** 2) for a, b in zip(fields["0"][3:], fields["1"][3:])))
+    assert de / ne < 1e-5 and dh / nh < 1e-5
+
+
 def test_magnetic_and_mixed_sources_match_oracle(emm, oracle):
     """a magnetic dipole (injected into H at the half step), alone and batched together with
     an electric dipole; fields, accumulators and receivers against the oracle."""
