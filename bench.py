@@ -296,6 +296,20 @@ def run_gpu(args):
         m_auto = max(1, min(1000, int(np.floor(1.0 / (g.info()["dt"] * (3.0 * fmax + 2.0 * np.sqrt(max(w["freqs"]) * 1.0)))))))
         decim = {"dtft_every": m_auto, "ms_per_step": msd / K, "value": world * nsrc * N * K / (msd * 1e-3) / 1e9,
                  "note": "only every m-th term of Eq. 25 (fields and J'); same converged step count; not the paper's every-step DTFT"}
+    # extra, not the headline: receivers-only DTFT (every term of Eq. 25, but only at the receivers' stencil nodes)
+    rec_only = None
+    if len(w["freqs"]) > 0 and len(w["receivers"]) > 0:
+        g.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=K + Wm + 4, batched=1 if nsrc > 1 else 0, sparse_dft=1))
+        g.run_enqueue(Wm)
+        torch.cuda.synchronize()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(g.stream)
+        g.run_enqueue(K)
+        d1.record(g.stream)
+        torch.cuda.synchronize()
+        msr = d0.elapsed_time(d1)
+        rec_only = {"ms_per_step": msr / K, "value": world * nsrc * N * K / (msr * 1e-3) / 1e9,
+                    "note": "sparse_dft=1: same receiver outputs and step counts, no full-grid frequency-domain fields"}
     batched = None
     if nsrc > 1:
         # configs[4]: the same K steps for ONE source alone = what running the sources one after the other costs
@@ -343,7 +357,7 @@ def run_gpu(args):
                 "e2e": {"value": world * nsrc * N * K / t_e2e / 1e9, "unit": "Gcell-updates/s", "h2d_bytes_per_step": h2d / K,
                         "d2h_bytes_per_step": d2h / K, "seconds": t_e2e,
                         "what": "emm_model_set (host sigma -> device) + emm_run(fixed_steps=K) (tables up, receivers back)"},
-                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched, "dtft_decimation": decim,
+                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched, "dtft_decimation": decim, "receivers_only_dtft": rec_only,
                 "multi_gpu": "replicas only: every rank runs the whole workload, no collective on the data path"}
         print(json.dumps(line))
     if world > 1:
