@@ -218,10 +218,13 @@ def run_gpu(args):
     N = info["N1"] * info["N2"] * info["N3"]
 
     # ---- end to end through the C ABI with host buffers (model upload + run + receiver read-back) ----
-    sh = np.ascontiguousarray(w["sigma_h"], np.float32)
-    sv = None if w.get("sigma_v") is None else np.ascontiguousarray(w["sigma_v"], np.float32)
-    g.model_set(sh, sv)                                        # warm-up of the whole path (plans, kernels)
-    g.run(srcs, w["freqs"], w["receivers"], dict(fixed_steps=3, batched=1 if nsrc > 1 else 0))
+    # host inputs in pinned memory (numpy views of pinned torch tensors): the library copies from whatever host pointer it gets
+    def pinned(a):
+        return torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory().numpy()
+    sh = pinned(w["sigma_h"])
+    sv = None if w.get("sigma_v") is None else pinned(w["sigma_v"])
+    g.model_set(sh, sv)                                        # warm-up of the whole path (plans, kernels, one graph capture)
+    g.run(srcs, w["freqs"], w["receivers"], dict(fixed_steps=min(K, 210), batched=1 if nsrc > 1 else 0))
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -232,8 +235,7 @@ def run_gpu(args):
     t_e2e = time.perf_counter() - t0
     assert int(ns[0]) == K and np.all(np.isfinite(out))
     h2d = sh.nbytes + (sv.nbytes if sv is not None else 0) + (K + 1) * (len(w["freqs"]) * 16 + 4 + 32)
-    npnt = max(2 * w["grid"]["rd"], 4) ** 3
-    d2h = nsrc * len(w["freqs"]) * 6 * len(w["receivers"]) * npnt * 8
+    d2h = nsrc * len(w["freqs"]) * len(w["receivers"]) * 6 * 16      # accumulators interpolated to the receivers on the device, complex fp64
     if world > 1:
         tt = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)

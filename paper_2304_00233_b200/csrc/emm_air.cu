@@ -297,6 +297,69 @@ __global__ void k_make_ce(const ModelArgs a, float *__restrict__ ce1, float *__r
   ce1[o] = v1; ce2[o] = v2; ce3[o] = v3;
 }
 
+// Raw model scan: validity (every cell finite and > 0) and the smallest conductivity inside each of the six CPML slabs
+// (reference speed of the profiles, [R5]).  out[0..5] = slab minima as ordered bit patterns of positive doubles
+// (axis-major, low side first), out[6] = number of invalid cells.
+struct ScanArgs { int nc[3]; int c0[3][2], c1[3][2]; const float *sh, *sv; };
+
+__global__ void k_model_scan(const ScanArgs a, unsigned long long *__restrict__ out) {
+  const size_t n = (size_t)a.nc[0] * a.nc[1] * a.nc[2];
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double m[6] = {inf, inf, inf, inf, inf, inf};
+  unsigned long long bad = 0;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+    const float h = a.sh[t], v = a.sv ? a.sv[t] : h;
+    if (!(h > 0.f) || !(v > 0.f) || isinf(h) || isinf(v)) { ++bad; continue; }
+    const int i = (int)(t % a.nc[0]), j = (int)((t / a.nc[0]) % a.nc[1]), k = (int)(t / ((size_t)a.nc[0] * a.nc[1]));
+    const int idx[3] = {i, j, k};
+    const double s = fmin((double)h, (double)v);
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax)
+#pragma unroll
+      for (int side = 0; side < 2; ++side)
+        if (idx[ax] >= a.c0[ax][side] && idx[ax] <= a.c1[ax][side]) m[2 * ax + side] = fmin(m[2 * ax + side], s);
+  }
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m[q] = fmin(m[q], __shfl_xor_sync(0xffffffffu, m[q], o));
+    if ((threadIdx.x & 31) == 0) atomicMin(out + q, (unsigned long long)__double_as_longlong(m[q]));
+  }
+  if (bad) atomicAdd(out + 6, bad);
+}
+
+// values of selected raw cells (idx < 0: air, 0); which[n] = 1 reads sigma_v
+__global__ void k_gather_cells(const float *__restrict__ sh, const float *__restrict__ sv, const long long *__restrict__ idx,
+                               const int *__restrict__ which, const int n, float *__restrict__ out) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  const long long t = idx[p];
+  out[p] = t < 0 ? 0.f : (which[p] ? sv : sh)[t];
+}
+
+int launch_model_scan(emm_grid *g, const float *d_sh, const float *d_sv, unsigned long long *d_out) {
+  ScanArgs a{};
+  for (int ax = 0; ax < 3; ++ax) {
+    a.nc[ax] = g->nc[ax];
+    for (int side = 0; side < 2; ++side) {
+      const int lo = side == 0 ? 0 : g->N[ax] - g->nb, hi = side == 0 ? g->nb - 1 : g->N[ax] - 1;   // padded cell range of the slab
+      a.c0[ax][side] = std::min(std::max(lo - g->lo[ax], 0), g->nc[ax] - 1);
+      a.c1[ax][side] = std::min(std::max(hi - g->lo[ax], 0), g->nc[ax] - 1);
+    }
+  }
+  a.sh = d_sh; a.sv = d_sv;
+  k_model_scan<<<148 * 8, 256, 0, g->stream>>>(a, d_out);
+  EMM_LAUNCH_CHECK(g, "k_model_scan");
+  return 0;
+}
+
+int launch_gather_cells(emm_grid *g, const float *d_sh, const float *d_sv, const long long *d_idx, const int *d_which, int n, float *d_out) {
+  if (n <= 0) return 0;
+  k_gather_cells<<<(n + 127) / 128, 128, 0, g->stream>>>(d_sh, d_sv, d_idx, d_which, n, d_out);
+  EMM_LAUNCH_CHECK(g, "k_gather_cells");
+  return 0;
+}
+
 static ModelArgs model_args(const emm_grid *g, const float *d_sh, const float *d_sv) {
   ModelArgs a{};
   a.N1 = g->N[0]; a.N2 = g->N[1]; a.N3 = g->N[2]; a.P1 = g->P1; a.r = g->r; a.klo = g->klo; a.air = g->top == EMM_TOP_AIR;

@@ -77,6 +77,7 @@ struct DevState {              // per run; arrays carry a leading source dimensi
 
 struct DevTables {             // device pointers of the per-grid region
   float *ce[3], *cm[3], *cp[3];
+  float *sig_h, *sig_v;        // raw per-cell model [nz][ny][nx] as given to emm_model_set (resident: effective medium at the source nodes)
   double *xn[3];
   int *ta_start[2][2], *fa_start[2][2];   // [axis][lattice]: lattice -> aux plane, aux plane -> lattice
   float *ta_w[2][2], *fa_w[2][2];
@@ -106,7 +107,6 @@ struct emm_grid {
   std::vector<emm::Stencil1> toaux[2][2], fromaux[2][2];
   // model
   bool have_model = false;
-  std::vector<float> sig_h, sig_v;       // raw per-cell model (kept for sigma_bar at source nodes, v_ref)
   bool vti = false;
   double dt = 0, smin = 0;
   // device

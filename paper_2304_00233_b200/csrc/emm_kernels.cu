@@ -509,15 +509,36 @@ __global__ void k_check_final(const DevState s, double *__restrict__ red, double
 
 __global__ void k_step_end(const DevState s) { *s.it += 1; }
 
-// receivers: gather accumulators on the interpolation stencils (Eq. 7 and the weights are applied on the host)
-__global__ void k_gather(const DevGrid g, const DevState s, const int *__restrict__ ridx, float2 *__restrict__ out, const int nn) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  const int c = blockIdx.y % 6, f = blockIdx.y / 6, src = blockIdx.z;
-  if (n >= nn) return;
-  const int t = ridx[(size_t)c * nn + n];              // node index in the padded volume
-  const int k = t / (int)g.PS, rem = t - k * (int)g.PS;
-  const float2 *F = s.F + ((((size_t)src * s.nf + f) * 6 + c) * g.NZB + (k - g.blo[2])) * g.PS + rem;
-  out[(((size_t)src * s.nf + f) * 6 + c) * nn + n] = *F;
+// receivers: interpolate the accumulators to the receiver positions, sum_n w_n F[node_n] in fp64 over the np^3 nodes of
+// each component's stencil (weights = tensor product of the 1-D weights, Eq. 9-12); one warp per (receiver, component,
+// frequency, source).  Reads the full-grid accumulators, or the receivers-only sums RA when nf_rec > 0.  Eq. 7 (the
+// division by the source spectrum) is applied on the host.
+__global__ void k_rec_interp(const DevGrid g, const DevState s, const int *__restrict__ ridx, const double *__restrict__ rw,
+                             const double2 *__restrict__ RA, const int nf, const int nrec, const int np3, const int sparse,
+                             double2 *__restrict__ out) {
+  const int q = blockIdx.x, c = blockIdx.y % 6, f = blockIdx.y / 6, src = blockIdx.z;
+  const size_t nn = (size_t)nrec * np3, base = (size_t)c * nn + (size_t)q * np3;
+  double ax = 0.0, ay = 0.0;
+  for (int n = threadIdx.x; n < np3; n += 32) {
+    double2 v;
+    if (sparse) {
+      v = RA[(((size_t)src * nf + f) * 6 + c) * nn + (size_t)q * np3 + n];
+    } else {
+      const int t = ridx[base + n];                      // node index in the padded volume
+      const int k = t / (int)g.PS, rem = t - k * (int)g.PS;
+      const float2 F = s.F[((((size_t)src * nf + f) * 6 + c) * g.NZB + (k - g.blo[2])) * g.PS + rem];
+      v = make_double2((double)F.x, (double)F.y);
+    }
+    const double w = rw[base + n];
+    ax += w * v.x;
+    ay += w * v.y;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ax += __shfl_xor_sync(0xffffffffu, ax, o);
+    ay += __shfl_xor_sync(0xffffffffu, ay, o);
+  }
+  if (threadIdx.x == 0) out[(((size_t)src * nf + f) * nrec + q) * 6 + c] = make_double2(ax, ay);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -663,11 +684,12 @@ int launch_step_end(emm_grid *g, const DevState &s) {
   return 0;
 }
 
-int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nn) {
-  if (nn <= 0) return 0;
-  dim3 grid((nn + 127) / 128, 6 * s.nf, s.nsrc);
-  k_gather<<<grid, 128, 0, g->stream>>>(g->dg, s, r.rec_idx, r.rec_val, nn);
-  EMM_LAUNCH_CHECK(g, "k_gather");
+int launch_rec_interp(emm_grid *g, const DevState &s, const DevRun &r, int nf, int nrec, int np3) {
+  if (nrec <= 0 || nf <= 0) return 0;
+  dim3 grid(nrec, 6 * nf, s.nsrc);
+  if (grid.y > 65535) return fail(EMM_EINVAL, "launch_rec_interp: too many frequencies");
+  k_rec_interp<<<grid, 32, 0, g->stream>>>(g->dg, s, r.rec_idx, r.rec_w, r.RA, nf, nrec, np3, r.nf_rec > 0 ? 1 : 0, r.rec_out);
+  EMM_LAUNCH_CHECK(g, "k_rec_interp");
   return 0;
 }
 

@@ -10,6 +10,9 @@ struct DevRun {
   int *src_off = nullptr;      // [nsrc*3+1] offsets into src_idx / src_w (component-major per source)
   int *src_idx = nullptr;      // node index inside one source's volume
   float *src_w = nullptr;      // dt/eps * W (c-6)
+  long long *cell_idx = nullptr;  // [nsrc*3*np^3*4] raw cells around the source nodes (effective medium at the sources)
+  int *cell_which = nullptr;
+  float *cell_val = nullptr;
   // check set
   int *chk_idx = nullptr;
   int nchk = 0;
@@ -21,7 +24,8 @@ struct DevRun {
   int *status = nullptr;       // [nsrc]
   // receivers
   int *rec_idx = nullptr;      // [6][nrec*np^3]
-  float2 *rec_val = nullptr;   // [nsrc][nf][6][nrec*np^3]
+  double *rec_w = nullptr;     // [6][nrec*np^3] interpolation weights (tensor products)
+  double2 *rec_out = nullptr;  // [nsrc][nf][nrec][6] accumulators interpolated to the receivers
   int nrec_nodes = 0;
   // receivers-only DTFT (emm_run_opts.sparse_dft): fp64 accumulators at the receiver stencil nodes
   double2 *RA = nullptr;       // [nsrc][nf][6][nrec*np^3]
@@ -39,7 +43,7 @@ int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_rec_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);
 int launch_step_end(emm_grid *g, const DevState &s);
-int launch_gather(emm_grid *g, const DevState &s, const DevRun &r, int nrec_nodes);
+int launch_rec_interp(emm_grid *g, const DevState &s, const DevRun &r, int nf, int nrec, int np3);
 // air-water boundary (Eq. 17-21): ghost planes of Ex,Ey (is_h=0) or Hx,Hy (is_h=1)
 int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
 // separable route of the same boundary for non-uniform x-y (emm_air_sep.cu); launch_air dispatches to it when g->sep_air
@@ -47,6 +51,8 @@ int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cu
 size_t sep_air_scratch(const emm_grid *g, int nsrc);
 int sep_air_make_plans(emm_grid *g, int nsrc);
 // model: effective medium (Eq. 26) -> min sigma (for Eq. 15) and dt/eps
+int launch_model_scan(emm_grid *g, const float *d_sh, const float *d_sv, unsigned long long *d_out /* [7] */);
+int launch_gather_cells(emm_grid *g, const float *d_sh, const float *d_sv, const long long *d_idx, const int *d_which, int n, float *d_out);
 int launch_sigma_min(emm_grid *g, const float *d_sh, const float *d_sv, double *d_min);
 int launch_make_ce(emm_grid *g, const float *d_sh, const float *d_sv, double scale);
 

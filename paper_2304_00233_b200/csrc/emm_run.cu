@@ -81,6 +81,8 @@ static void layout_fixed(emm_grid *g, Arena &A) {
     g->T.xn[a] = A.take<double>((size_t)g->N[a] + 1);
   }
   for (int c = 0; c < 3; ++c) g->T.ce[c] = A.take<float>(vol(g));
+  g->T.sig_h = A.take<float>((size_t)g->nc[0] * g->nc[1] * g->nc[2]);
+  g->T.sig_v = A.take<float>((size_t)g->nc[0] * g->nc[1] * g->nc[2]);
   if (g->top == EMM_TOP_AIR) {
     g->T.kx = A.take<float>(g->M1);
     g->T.ky = A.take<float>(g->M2);
@@ -132,6 +134,9 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
   r.src_off = A.take<int>((size_t)nsrc * 3 + 1);
   r.src_idx = A.take<int>((size_t)nsrc * 3 * np3);
   r.src_w = A.take<float>((size_t)nsrc * 3 * np3);
+  r.cell_idx = A.take<long long>((size_t)nsrc * 3 * np3 * 4);
+  r.cell_which = A.take<int>((size_t)nsrc * 3 * np3 * 4);
+  r.cell_val = A.take<float>((size_t)nsrc * 3 * np3 * 4);
   r.chk_idx = A.take<int>(nchk);
   r.nchk = (int)nchk;
   r.C = A.take<double2>((size_t)nsrc * 6 * nchk);
@@ -143,7 +148,8 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
   r.nsteps = A.take<int>(nsrc);
   r.status = A.take<int>(nsrc);
   r.rec_idx = A.take<int>((size_t)6 * nrec * np3);
-  r.rec_val = A.take<float2>((size_t)nsrc * nf * 6 * nrec * np3);
+  r.rec_w = A.take<double>((size_t)6 * nrec * np3);
+  r.rec_out = A.take<double2>((size_t)nsrc * (nf + nf_rec) * nrec * 6);
   r.nf_rec = nf_rec;
   r.RA = A.take<double2>((size_t)nsrc * nf_rec * 6 * nrec * np3);
   r.twEf = A.take<double2>((size_t)table_steps * nf_rec);
@@ -200,9 +206,7 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   DevRun r{};
   layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), s, r);   // the full-grid mode is the larger one
   g->T = keep;
-  // emm_model_set stages the raw model in the run region: make sure it fits as well
-  const size_t stage = fixed + 2 * ((size_t)g->nc[0] * g->nc[1] * g->nc[2] * sizeof(float) + 256) + 512;
-  return std::max(A.off, stage) + 4096;
+  return std::max(A.off, fixed + 1024) + 4096;       // emm_model_set keeps a few scalars behind the per-grid region
 }
 
 extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, void *cuda_stream) {
@@ -285,31 +289,29 @@ extern "C" int emm_model_set(emm_grid *g, const float *sigma_h, const float *sig
   free_run(g);
   g->have_model = false;
   const size_t nc = (size_t)g->nc[0] * g->nc[1] * g->nc[2];
-  for (size_t t = 0; t < nc; ++t) {
-    if (!(sigma_h[t] > 0) || !std::isfinite(sigma_h[t])) return fail(EMM_EINVAL, "emm_model_set: sigma_h must be finite and > 0");
-    if (sigma_v && (!(sigma_v[t] > 0) || !std::isfinite(sigma_v[t]))) return fail(EMM_EINVAL, "emm_model_set: sigma_v must be finite and > 0");
-  }
-  try {
-    g->sig_h.assign(sigma_h, sigma_h + nc);
-    if (sigma_v) g->sig_v.assign(sigma_v, sigma_v + nc); else g->sig_v.clear();
-  } catch (const std::bad_alloc &) { return fail(EMM_ENOMEM, "emm_model_set: out of memory"); }
   g->vti = sigma_v != nullptr;
-  // stage the raw model behind the fixed region
+  // the raw model stays resident in the per-grid region (emm_run_begin reads the cells around the source nodes);
+  // validation, slab minima, effective medium and dt/eps are device passes over it: the host never walks the model
+  float *d_sh = g->T.sig_h, *d_sv = sigma_v ? g->T.sig_v : g->T.sig_h;
   Arena A;
   A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
-  float *d_sh = A.take<float>(nc);
-  float *d_sv = sigma_v ? A.take<float>(nc) : d_sh;
   double *d_min = A.take<double>(1);
-  if (A.overflow) return fail(EMM_ENOMEM, "emm_model_set: workspace too small to stage the model");
+  unsigned long long *d_scan = A.take<unsigned long long>(7);
+  if (A.overflow) return fail(EMM_ENOMEM, "emm_model_set: workspace too small");
   CU(cudaMemcpyAsync(d_sh, sigma_h, nc * sizeof(float), cudaMemcpyHostToDevice, g->stream));
   if (sigma_v) CU(cudaMemcpyAsync(d_sv, sigma_v, nc * sizeof(float), cudaMemcpyHostToDevice, g->stream));
   const unsigned long long inf_bits = 0x7ff0000000000000ULL;
+  unsigned long long scan[7] = {inf_bits, inf_bits, inf_bits, inf_bits, inf_bits, inf_bits, 0ULL};
   CU(cudaMemcpyAsync(d_min, &inf_bits, sizeof inf_bits, cudaMemcpyHostToDevice, g->stream));
-  int rc = launch_sigma_min(g, d_sh, d_sv, d_min);
+  CU(cudaMemcpyAsync(d_scan, scan, sizeof scan, cudaMemcpyHostToDevice, g->stream));
+  int rc = launch_model_scan(g, d_sh, sigma_v ? d_sv : nullptr, d_scan);
   if (rc) return rc;
+  if ((rc = launch_sigma_min(g, d_sh, d_sv, d_min))) return rc;
   double smin = 0;
   CU(cudaMemcpyAsync(&smin, d_min, sizeof smin, cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaMemcpyAsync(scan, d_scan, sizeof scan, cudaMemcpyDeviceToHost, g->stream));
   CU(cudaStreamSynchronize(g->stream));
+  if (scan[6] != 0) return fail(EMM_EINVAL, "emm_model_set: sigma_h and sigma_v must be finite and > 0 (%llu cells are not)", scan[6]);
   if (!(smin > 0) || !std::isfinite(smin)) return fail(EMM_EINVAL, "emm_model_set: non-positive effective conductivity at an updated node");
   g->smin = smin;
   const double vmax = 1.0 / std::sqrt(kMu0 * smin / (2 * g->w0));                       // v = 1/sqrt(mu eps), eps = sigma/(2 w0)
@@ -321,18 +323,9 @@ extern "C" int emm_model_set(emm_grid *g, const float *sigma_h, const float *sig
   // CPML reference speed per face = fastest padded cell inside the slab [R5]
   for (int a = 0; a < 3; ++a)
     for (int side = 0; side < 2; ++side) {
-      int lo = side == 0 ? 0 : g->N[a] - g->nb, hi = side == 0 ? g->nb - 1 : g->N[a] - 1;   // padded cell range
-      int c0 = std::min(std::max(lo - g->lo[a], 0), g->nc[a] - 1), c1 = std::min(std::max(hi - g->lo[a], 0), g->nc[a] - 1);
-      double smn = INFINITY;
-      int b0[3] = {0, 0, 0}, b1[3] = {g->nc[0] - 1, g->nc[1] - 1, g->nc[2] - 1};
-      b0[a] = c0; b1[a] = c1;
       if (a == 2 && side == 0 && g->top == EMM_TOP_AIR) { g->vref[a][side] = 0; continue; }
-      for (int k = b0[2]; k <= b1[2]; ++k) for (int j = b0[1]; j <= b1[1]; ++j) for (int i = b0[0]; i <= b1[0]; ++i) {
-        const size_t t = (size_t)i + (size_t)g->nc[0] * ((size_t)j + (size_t)g->nc[1] * (size_t)k);
-        double s = g->sig_h[t];
-        if (g->vti) s = std::min(s, (double)g->sig_v[t]);
-        smn = std::min(smn, s);
-      }
+      double smn;
+      std::memcpy(&smn, &scan[2 * a + side], sizeof smn);
       g->vref[a][side] = 1.0 / std::sqrt(kMu0 * smn / (2 * g->w0));
     }
   g->have_model = true;
@@ -342,30 +335,26 @@ extern "C" int emm_model_set(emm_grid *g, const float *sigma_h, const float *sig
 // ---------------------------------------------------------------------------------------------------
 namespace emm {
 
-// effective conductivity of E component c at node (i,j,k), same rule as the device pass ([R3])
-static double sigma_bar_host(const emm_grid *g, int c, int i, int j, int k) {
-  auto cell = [&](const std::vector<float> &s, int ii, int jj, int kk) -> double {
-    int ci = ii - g->lo[0], cj = jj - g->lo[1], ck = kk - g->lo[2];
-    if (g->top == EMM_TOP_AIR && ck < 0) return 0.0;
-    ci = std::min(std::max(ci, 0), g->nc[0] - 1);
-    cj = std::min(std::max(cj, 0), g->nc[1] - 1);
-    ck = std::min(std::max(ck, 0), g->nc[2] - 1);
-    return (double)s[(size_t)ci + (size_t)g->nc[0] * ((size_t)cj + (size_t)g->nc[1] * (size_t)ck)];
-  };
-  const std::vector<float> &sh = g->sig_h, &sv = g->vti ? g->sig_v : g->sig_h;
+// effective conductivity of E component c at node (i,j,k), same rule as the device pass ([R3]): the four raw cells
+// sharing the component's edge (index < 0: air above z = 0) and their area weights; sigma_bar = sum w s / sum w
+static void sigma_bar_cells(const emm_grid *g, int c, int i, int j, int k, long long *cell, int *which, double *w) {
   const int idx[3] = {i, j, k};
   const int a1 = (c + 1) % 3, a2 = (c + 2) % 3;        // the two transverse axes
-  double num = 0, den = 0;
+  int n = 0;
   for (int d1 = -1; d1 <= 0; ++d1)
-    for (int d2 = -1; d2 <= 0; ++d2) {
+    for (int d2 = -1; d2 <= 0; ++d2, ++n) {
       int q[3] = {idx[0], idx[1], idx[2]};
       q[a1] = std::max(idx[a1] + d1, 0);
       q[a2] = std::max(idx[a2] + d2, 0);
-      const double w = (g->xn[a1][q[a1] + 1] - g->xn[a1][q[a1]]) * (g->xn[a2][q[a2] + 1] - g->xn[a2][q[a2]]);
-      num += cell(c == 2 ? sv : sh, q[0], q[1], q[2]) * w;
-      den += w;
+      w[n] = (g->xn[a1][q[a1] + 1] - g->xn[a1][q[a1]]) * (g->xn[a2][q[a2] + 1] - g->xn[a2][q[a2]]);
+      int ci = q[0] - g->lo[0], cj = q[1] - g->lo[1], ck = q[2] - g->lo[2];
+      which[n] = (c == 2 && g->vti) ? 1 : 0;
+      if (g->top == EMM_TOP_AIR && ck < 0) { cell[n] = -1; continue; }
+      ci = std::min(std::max(ci, 0), g->nc[0] - 1);
+      cj = std::min(std::max(cj, 0), g->nc[1] - 1);
+      ck = std::min(std::max(ck, 0), g->nc[2] - 1);
+      cell[n] = (long long)ci + (long long)g->nc[0] * ((long long)cj + (long long)g->nc[1] * (long long)ck);
     }
-  return num / den;
 }
 
 static double node_width(const emm_grid *g, int a, int half, int i) {
@@ -663,8 +652,10 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     }
 
     // sources: W_c = dir_c w_x w_y w_z / V on the component's lattice, premultiplied by dt/eps ([R7])
-    std::vector<int> soff(nsrc * 3 + 1, 0), sidx;
+    std::vector<int> soff(nsrc * 3 + 1, 0), sidx, cwhich;
     std::vector<float> sw;
+    std::vector<long long> cidx;
+    std::vector<double> cwgt, sWd;
     for (int s = 0; s < nsrc; ++s) {
       const double *dir = src[s].dir, *pos = src[s].pos;
       if (src[s].type != 0 && src[s].type != 1) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: source %d has an unknown type", s); }
@@ -689,29 +680,56 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
           const int i = st[0].start + c1, j = st[1].start + c2, k = st[2].start + c3;
           const double V = node_width(g, 0, kLat[cl][0], i) * node_width(g, 1, kLat[cl][1], j) * node_width(g, 2, kLat[cl][2], k);
           const double W = dir[c] / dn * st[0].w[c1] * st[1].w[c2] * st[2].w[c3] / V;
-          const double ce = mag ? g->dt / kMu0 : g->dt * 2 * g->w0 / sigma_bar_host(g, c, i, j, k);   // dt/mu or dt/eps
+          // dt/mu, or dt/eps from the effective conductivity at the node (cells fetched from the device below)
+          long long cell[4] = {-1, -1, -1, -1};
+          int which[4] = {0, 0, 0, 0};
+          double cw[4] = {0, 0, 0, 0};
+          if (!mag) sigma_bar_cells(g, c, i, j, k, cell, which, cw);
+          for (int n4 = 0; n4 < 4; ++n4) { cidx.push_back(cell[n4]); cwhich.push_back(which[n4]); cwgt.push_back(mag ? -1.0 : cw[n4]); }
           sidx.push_back((int)(((size_t)k * g->N[1] + j) * g->P1 + i));
-          sw.push_back((float)(ce * W));
+          sWd.push_back(W);
         }
       }
       soff[s * 3 + 3] = (int)sidx.size();
     }
     for (int s = 0; s < nsrc; ++s) for (int c = 0; c < 3; ++c) if (soff[s * 3 + c + 1] < soff[s * 3 + c]) soff[s * 3 + c + 1] = soff[s * 3 + c];
     (void)np3;
+    if (!cidx.empty()) {
+      std::vector<float> cval(cidx.size());
+      if ((rc = upload(g, R->dr.cell_idx, cidx)) || (rc = upload(g, R->dr.cell_which, cwhich)) ||
+          (rc = launch_gather_cells(g, g->T.sig_h, g->vti ? g->T.sig_v : g->T.sig_h, R->dr.cell_idx, R->dr.cell_which, (int)cidx.size(), R->dr.cell_val))) {
+        free_run(g); return rc;
+      }
+      CU(cudaMemcpyAsync(cval.data(), R->dr.cell_val, cval.size() * sizeof(float), cudaMemcpyDeviceToHost, g->stream));
+      CU(cudaStreamSynchronize(g->stream));
+      for (size_t n = 0; n < sWd.size(); ++n) {
+        double ce = g->dt / kMu0;                                               // magnetic: dt/mu
+        if (cwgt[4 * n] >= 0.0) {
+          double num = 0, den = 0;
+          for (int n4 = 0; n4 < 4; ++n4) { num += (double)cval[4 * n + n4] * cwgt[4 * n + n4]; den += cwgt[4 * n + n4]; }
+          ce = g->dt * 2 * g->w0 / (num / den);                                 // electric: dt/eps
+        }
+        sw.push_back((float)(ce * sWd[n]));
+      }
+    }
     if ((rc = upload(g, const_cast<int *>(R->ds.src_mag), R->mag))) { free_run(g); return rc; }
     if ((rc = upload(g, R->dr.src_off, soff)) || (rc = upload(g, R->dr.src_idx, sidx)) || (rc = upload(g, R->dr.src_w, sw))) { free_run(g); return rc; }
 
     // receiver gather list
     std::vector<int> ridx((size_t)6 * nrec * np3);
+    std::vector<double> rwgt((size_t)6 * nrec * np3);
     R->nrec_nodes = (int)(nrec * np3);
     R->dr.nrec_nodes = R->nrec_nodes;
     for (int c = 0; c < 6; ++c) for (int q = 0; q < nrec; ++q) {
       const Stencil1 *st = &R->rst[((size_t)q * 6 + c) * 3];
       size_t n = 0;
       for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1)
+      {
+        rwgt[((size_t)c * nrec + q) * np3 + n] = st[0].w[c1] * st[1].w[c2] * st[2].w[c3];
         ridx[((size_t)c * nrec + q) * np3 + n++] = (int)(((size_t)(st[2].start + c3) * g->N[1] + st[1].start + c2) * g->P1 + st[0].start + c1);
+      }
     }
-    if ((rc = upload(g, R->dr.rec_idx, ridx))) { free_run(g); return rc; }
+    if ((rc = upload(g, R->dr.rec_idx, ridx)) || (rc = upload(g, R->dr.rec_w, rwgt))) { free_run(g); return rc; }
     CU(cudaStreamSynchronize(g->stream));
   } catch (const std::bad_alloc &) {
     free_run(g);
@@ -753,7 +771,8 @@ extern "C" int emm_run_steps(emm_grid *g, int n, int *nsteps, int *all_done) {
   return 0;
 }
 
-// compute_green_function + extract_emf (Alg. 1): Eq. 7 and receiver interpolation, fp64 on the host
+// compute_green_function + extract_emf (Alg. 1): receiver interpolation in fp64 on the device (k_rec_interp),
+// Eq. 7 in fp64 on the host
 extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
   if (!g || !g->run) return fail(EMM_EINVAL, "emm_run_end: no run in progress");
   Run *R = g->run;
@@ -761,20 +780,13 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
   if ((rc = fetch_flags(g))) return rc;
   for (int s = 0; s < R->nsrc; ++s) if (nsteps) nsteps[s] = R->nsteps[s];
   if (!out_ || R->nrec == 0) return 0;
-  const int nf = R->nf, np = R->np, nn = R->nrec_nodes;
+  const int nf = R->nf, np = R->np;
   const size_t np3 = (size_t)np * np * np;
-  // accumulators at the receiver stencil nodes: gathered from the full-grid F, or the fp64 sums of the receivers-only mode
-  std::vector<double2> val((size_t)R->nsrc * nf * 6 * nn);
-  if (R->sparse) {
-    CU(cudaMemcpyAsync(val.data(), R->dr.RA, val.size() * sizeof(double2), cudaMemcpyDeviceToHost, g->stream));
-    CU(cudaStreamSynchronize(g->stream));
-  } else {
-    if ((rc = launch_gather(g, R->ds, R->dr, nn))) return rc;
-    std::vector<float2> v32(val.size());
-    CU(cudaMemcpyAsync(v32.data(), R->dr.rec_val, v32.size() * sizeof(float2), cudaMemcpyDeviceToHost, g->stream));
-    CU(cudaStreamSynchronize(g->stream));
-    for (size_t n = 0; n < val.size(); ++n) val[n] = make_double2((double)v32[n].x, (double)v32[n].y);
-  }
+  // accumulators interpolated to the receivers on the device (from the full-grid F, or from the receivers-only sums)
+  if ((rc = launch_rec_interp(g, R->ds, R->dr, nf, R->nrec, (int)np3))) return rc;
+  std::vector<double2> val((size_t)R->nsrc * nf * R->nrec * 6);
+  CU(cudaMemcpyAsync(val.data(), R->dr.rec_out, val.size() * sizeof(double2), cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
   std::complex<double> *out = reinterpret_cast<std::complex<double> *>(out_);
   const std::complex<double> I(0, 1);
   for (int s = 0; s < R->nsrc; ++s)
@@ -783,13 +795,8 @@ extern "C" int emm_run_end(emm_grid *g, double *out_, int *nsteps) {
       const std::complex<double> sc = std::sqrt(-I * 2.0 * kPi * R->freqs[f] / (2 * g->w0));   // Eq. 7a, principal root
       for (int q = 0; q < R->nrec; ++q)
         for (int c = 0; c < 6; ++c) {
-          const Stencil1 *st = &R->rst[((size_t)q * 6 + c) * 3];
-          const double2 *v = &val[(((size_t)s * nf + f) * 6 + c) * nn + (size_t)q * np3];
-          std::complex<double> acc = 0;
-          size_t n = 0;
-          for (int c3 = 0; c3 < np; ++c3) for (int c2 = 0; c2 < np; ++c2) for (int c1 = 0; c1 < np; ++c1, ++n)
-            acc += st[0].w[c1] * st[1].w[c2] * st[2].w[c3] * std::complex<double>(v[n].x, v[n].y);
-          std::complex<double> G = acc / Jw;                                   // Eq. 7b
+          const double2 v = val[(((size_t)s * nf + f) * R->nrec + q) * 6 + c];
+          std::complex<double> G = std::complex<double>(v.x, v.y) / Jw;         // Eq. 7b
           if (!R->mag[s] && c < 3) G *= sc;                                    // electric source: G^EE = sc F_E/J'
           if (R->mag[s] && c >= 3) G /= sc;                                    // magnetic source: G^HM = F_H/(sc M')
           out[(((size_t)s * nf + f) * R->nrec + q) * 6 + c] = G;
