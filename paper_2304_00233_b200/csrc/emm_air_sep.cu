@@ -15,9 +15,9 @@
 //   cuFFT        batched 1-D transforms along y (contiguous)
 //   k_sep_filter spectral filters of Eq. 17-21 per ghost level and output component: W[o][lev][k1][n]
 //   cuFFT        batched inverse 1-D transforms along y
-//   k_sep_ydown  y-interpolate back to the N2 lattice rows, Hermitian-extend in k1 and pack the two real outputs
-//                into one complex column: ZT[k][lev*N2 + j]
-//   cuFFT        batched inverse 1-D transforms along x, input read transposed
+//   k_sep_ydown  y-interpolate back to the N2 lattice rows, Hermitian-extend in k1, pack the two real outputs into
+//                one complex value and transpose through shared memory: ZR[lev*N2 + j][k]
+//   cuFFT        batched inverse 1-D transforms along x (contiguous rows, in place)
 //   k_sep_xdown  x-interpolate back to the lattice and write the ghost rows of the two field components
 //
 // Against the plane-sized route this halves the number of length-M transforms (no x transforms of the M2 - N2
@@ -111,25 +111,47 @@ __global__ void k_sep_filter(const SepArgs A, const float *__restrict__ kx, cons
   }
 }
 
-// ZT[k][lev*N2 + j] = Za + i Zb for k = k1 and conj(Za) + i conj(Zb) for k = M1 - k1, with Za, Zb the columns of the
-// two output components interpolated back to their own y lattices.
-__global__ void k_sep_ydown(const SepArgs A, const float2 *__restrict__ W, const Tab t0, const Tab t1, float2 *__restrict__ ZT) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x, k1 = blockIdx.y, src = blockIdx.z / A.nlev, lev = blockIdx.z - src * A.nlev;
-  if (j >= A.N2) return;
+// ZR[row][k] (row = (src*nlev + lev)*N2 + j) = Za + i Zb for k = k1 and conj(Za) + i conj(Zb) for k = M1 - k1, with Za, Zb
+// the columns of the two output components interpolated back to their own y lattices.  A block works on a tile of
+// 32 lattice rows x 32 wavenumbers: the column reads run along j (one W row per warp), the row writes along k1, with
+// a shared-memory transpose in between, so that the x transform that follows reads contiguous rows.
+__global__ void __launch_bounds__(256) k_sep_ydown(const SepArgs A, const float2 *__restrict__ W, const Tab t0, const Tab t1,
+                                                   float2 *__restrict__ ZR) {
+  __shared__ float2 tp[32][33], tm[32][33];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int j0 = blockIdx.x * 32, k0 = blockIdx.y * 32, src = blockIdx.z / A.nlev, lev = blockIdx.z - src * A.nlev;
   const size_t plane = (size_t)A.K1 * A.M2;
   W += (size_t)src * 2 * A.nlev * plane;
-  const float2 *ra = W + (size_t)lev * plane + (size_t)k1 * A.M2, *rb = W + (size_t)(A.nlev + lev) * plane + (size_t)k1 * A.M2;
-  const int sa = t0.s[j], sb = t1.s[j];
-  const float4 wa = *reinterpret_cast<const float4 *>(t0.w + 4 * j), wb = *reinterpret_cast<const float4 *>(t1.w + 4 * j);
-  const float2 a0 = ra[sa], a1 = ra[sa + 1], a2 = ra[sa + 2], a3 = ra[sa + 3];
-  const float2 b0 = rb[sb], b1 = rb[sb + 1], b2 = rb[sb + 2], b3 = rb[sb + 3];
-  const float2 za = make_float2(fmaf(wa.x, a0.x, fmaf(wa.y, a1.x, fmaf(wa.z, a2.x, wa.w * a3.x))),
-                                fmaf(wa.x, a0.y, fmaf(wa.y, a1.y, fmaf(wa.z, a2.y, wa.w * a3.y))));
-  const float2 zb = make_float2(fmaf(wb.x, b0.x, fmaf(wb.y, b1.x, fmaf(wb.z, b2.x, wb.w * b3.x))),
-                                fmaf(wb.x, b0.y, fmaf(wb.y, b1.y, fmaf(wb.z, b2.y, wb.w * b3.y))));
-  const size_t nrows = (size_t)A.nsrc * A.nlev * A.N2, col = ((size_t)src * A.nlev + lev) * A.N2 + j;
-  ZT[(size_t)k1 * nrows + col] = make_float2(za.x - zb.y, za.y + zb.x);
-  if (k1 > 0 && A.M1 - k1 != k1) ZT[(size_t)(A.M1 - k1) * nrows + col] = make_float2(za.x + zb.y, zb.x - za.y);
+  const int j = j0 + tx;
+  if (j < A.N2) {
+    const int sa = t0.s[j], sb = t1.s[j];
+    const float4 wa = *reinterpret_cast<const float4 *>(t0.w + 4 * j), wb = *reinterpret_cast<const float4 *>(t1.w + 4 * j);
+#pragma unroll
+    for (int kk = ty; kk < 32; kk += 8) {
+      const int k1 = k0 + kk;
+      if (k1 >= A.K1) break;
+      const float2 *ra = W + (size_t)lev * plane + (size_t)k1 * A.M2, *rb = W + (size_t)(A.nlev + lev) * plane + (size_t)k1 * A.M2;
+      const float2 a0 = ra[sa], a1 = ra[sa + 1], a2 = ra[sa + 2], a3 = ra[sa + 3];
+      const float2 b0 = rb[sb], b1 = rb[sb + 1], b2 = rb[sb + 2], b3 = rb[sb + 3];
+      const float2 za = make_float2(fmaf(wa.x, a0.x, fmaf(wa.y, a1.x, fmaf(wa.z, a2.x, wa.w * a3.x))),
+                                    fmaf(wa.x, a0.y, fmaf(wa.y, a1.y, fmaf(wa.z, a2.y, wa.w * a3.y))));
+      const float2 zb = make_float2(fmaf(wb.x, b0.x, fmaf(wb.y, b1.x, fmaf(wb.z, b2.x, wb.w * b3.x))),
+                                    fmaf(wb.x, b0.y, fmaf(wb.y, b1.y, fmaf(wb.z, b2.y, wb.w * b3.y))));
+      tp[kk][tx] = make_float2(za.x - zb.y, za.y + zb.x);
+      tm[kk][tx] = make_float2(za.x + zb.y, zb.x - za.y);
+    }
+  }
+  __syncthreads();
+  const int k1 = k0 + tx;
+  if (k1 >= A.K1) return;
+  const bool mirror = k1 > 0 && A.M1 - k1 != k1;
+#pragma unroll
+  for (int jj = ty; jj < 32; jj += 8) {
+    if (j0 + jj >= A.N2) break;
+    float2 *row = ZR + (((size_t)src * A.nlev + lev) * A.N2 + j0 + jj) * A.M1;
+    row[k1] = tp[tx][jj];
+    if (mirror) row[A.M1 - k1] = tm[tx][jj];
+  }
 }
 
 __global__ void k_sep_xdown(const SepArgs A, const float2 *__restrict__ XR, const Tab ta, const Tab tb, float *__restrict__ fa,
@@ -153,8 +175,8 @@ size_t sep_air_scratch(const emm_grid *g, int nsrc) {
   return (size_t)nsrc * (2 * rows * g->M1 + (size_t)(2 + 2 * g->r) * K1 * g->M2);
 }
 
-// 1-D batched plans for nsrc sources: 0/1 x forward (E/H), 2/3 y forward, 4/5 y inverse, 6/7 x inverse.  The x plans
-// write (forward) or read (inverse) the transposed layout [k][row] through cuFFT's strided data layout.
+// 1-D batched plans for nsrc sources: 0/1 x forward (E/H), 2/3 y forward, 4/5 y inverse, 6/7 x inverse.  The forward x
+// plans write the transposed layout [k][row] through cuFFT's strided data layout (k_sep_yup reads it along the rows).
 int sep_air_make_plans(emm_grid *g, int nsrc) {
   if (g->sp_nsrc == nsrc) return 0;
   for (cufftHandle &h : g->sp) { if (h) cufftDestroy(h); h = 0; }
@@ -173,9 +195,9 @@ int sep_air_make_plans(emm_grid *g, int nsrc) {
     } else if (q < 6) {                // y inverse, in place on W
       batch = nsrc * 2 * nlev * K1;
       n[0] = M2; idist = odist = M2;
-    } else {                           // x inverse: ZT[k][row] -> rows [row][M1]
+    } else {                           // x inverse, in place on the rows [row][M1]
       batch = nsrc * nlev * N2;
-      n[0] = M1; istride = batch; idist = 1; odist = M1;
+      n[0] = M1; idist = odist = M1;
     }
     if (batch < 1) continue;
     if (q == 3 && nsrc == 1) batch = K1;                                  // single source, H pass: only the first plane is live
@@ -231,9 +253,9 @@ int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cu
   k_sep_filter<<<dim3((a.M2 + 127) / 128, a.K1, ns), blk, 0, st>>>(a, g->T.kx, g->T.ky, V, W);
   EMM_SEP_CHECK(g, "k_sep_filter");
   if (cufftExecC2C(g->sp[4 + is_h], W, W, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (y inverse) failed");
-  k_sep_ydown<<<dim3((a.N2 + 127) / 128, a.K1, nlev * ns), blk, 0, st>>>(a, W, fa(1, out_y[0]), fa(1, out_y[1]), XT);
+  k_sep_ydown<<<dim3((a.N2 + 31) / 32, (a.K1 + 31) / 32, nlev * ns), dim3(32, 8, 1), 0, st>>>(a, W, fa(1, out_y[0]), fa(1, out_y[1]), XR);
   EMM_SEP_CHECK(g, "k_sep_ydown");
-  if (cufftExecC2C(g->sp[6 + is_h], XT, XR, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x inverse) failed");
+  if (cufftExecC2C(g->sp[6 + is_h], XR, XR, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x inverse) failed");
   k_sep_xdown<<<dim3((a.N1 + 127) / 128, a.N2, nlev * ns), blk, 0, st>>>(a, XR, fa(0, out_x[0]), fa(0, out_x[1]), is_h ? s.H[0] : s.E[0],
                                                                           is_h ? s.H[1] : s.E[1]);
   EMM_SEP_CHECK(g, "k_sep_xdown");
