@@ -6,9 +6,10 @@ in these files comes from the CUDA path.  The oracle runs in sparse-DFT mode (ac
 receiver stencils and the check set: pointwise identical values, see test_convergence_rule).
 
     python tests/golden/make_goldens.py cfg2            # ~15 min on 8 cores
-    python tests/golden/make_goldens.py cfg3 0 100        # configs[2] with aux_dx = 100 m, to convergence: ~2 h
+    python tests/golden/make_goldens.py cfg3 0 100        # configs[2] with aux_dx = 100 m, to convergence: ~50 min
+    python tests/golden/make_goldens.py cfg4 300 100      # configs[3] with aux_dx = 100 m, 300 fixed steps: ~50 min
 
-Output: tests/golden/<name>_converged.json with the inputs' SHA-256, nsteps, delta and the complex receivers.
+Output: tests/golden/<name>_converged[_aux<dx>].json or <name>_<n>steps[_aux<dx>].json with the inputs' SHA-256, nsteps, delta and the complex receivers.
 """
 import hashlib
 import json
