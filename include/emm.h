@@ -114,6 +114,16 @@ int emm_nugrid(int n, double len, double dx, double *x_out, double *q_out);
  * point x0, by Vandermonde inversion (Eq. 9-12).  Either output may be NULL.                */
 int emm_fd_weights(int npts, const double *nodes, double x0, double *w_interp, double *w_deriv);
 
+/* Acquisition geometry of the paper's source / receiver files (L632-640: x, y, z, azimuth, dip in rad).  The paper
+ * gives the columns but no formula; reading [R13]: azimuth from +x towards +y, dip from the horizontal
+ * towards +z (z is positive downward, L646), so dir = (cos dip cos az, cos dip sin az, sin dip), a unit vector.
+ * emm_dipole_direction: the `dir` of an emm_src with that orientation.  emm_receiver_channels: what a receiver
+ * dipole with that orientation records, chan[q] = (sum_c dir_c G_E[q][c], sum_c dir_c G_H[q][c]) for n receivers;
+ * g6: complex double [n][6] as returned by emm_run for one source and frequency, chan: complex double [n][2].
+ * Host, fp64.                                                                                            */
+int emm_dipole_direction(double azimuth, double dip, double *dir /* [3] */);
+int emm_receiver_channels(const double *g6, int n, const double *azimuth /* [n] */, const double *dip /* [n] */, double *chan);
+
 /* ---- problem set-up --------------------------------------------------------------------------------- */
 
 /* Node coordinates of the model (n?1 = cells+1 values each, strictly increasing).  Builds the padded

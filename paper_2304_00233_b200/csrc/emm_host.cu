@@ -106,6 +106,34 @@ extern "C" int emm_nugrid(int n, double len, double dx, double *x_out, double *q
   return 0;
 }
 
+// acquisition geometry (L632-640), [R13]: azimuth from +x towards +y, dip from the horizontal towards +z (downward)
+extern "C" int emm_dipole_direction(double azimuth, double dip, double *dir) {
+  if (!dir || !std::isfinite(azimuth) || !std::isfinite(dip)) return fail(EMM_EINVAL, "emm_dipole_direction: bad arguments");
+  dir[0] = std::cos(dip) * std::cos(azimuth);
+  dir[1] = std::cos(dip) * std::sin(azimuth);
+  dir[2] = std::sin(dip);
+  return 0;
+}
+
+extern "C" int emm_receiver_channels(const double *g6, int n, const double *azimuth, const double *dip, double *chan) {
+  if (n < 0 || (n > 0 && (!g6 || !azimuth || !dip || !chan))) return fail(EMM_EINVAL, "emm_receiver_channels: bad arguments");
+  for (int q = 0; q < n; ++q) {
+    double d[3];
+    const int rc = emm_dipole_direction(azimuth[q], dip[q], d);
+    if (rc) return rc;
+    for (int eh = 0; eh < 2; ++eh) {
+      double re = 0, im = 0;
+      for (int c = 0; c < 3; ++c) {
+        re += d[c] * g6[((size_t)q * 6 + 3 * eh + c) * 2];
+        im += d[c] * g6[((size_t)q * 6 + 3 * eh + c) * 2 + 1];
+      }
+      chan[((size_t)q * 2 + eh) * 2] = re;
+      chan[((size_t)q * 2 + eh) * 2 + 1] = im;
+    }
+  }
+  return 0;
+}
+
 extern "C" int emm_fd_weights(int npts, const double *nodes, double x0, double *w_interp, double *w_deriv) {
   if (npts < 2 || npts > 16 || !nodes) return fail(EMM_EINVAL, "emm_fd_weights: bad arguments");
   weights(nodes, npts, x0, w_interp, w_deriv);

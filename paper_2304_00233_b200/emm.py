@@ -25,7 +25,7 @@ _GET = {"E1": 0, "E2": 1, "E3": 2, "H1": 3, "H2": 4, "H3": 5,
 _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "box_lo2", "box_lo3",
          "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2", "pitch")
 # every symbol include/emm.h declares (tests check that the library exports all of them)
-SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
+SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_dipole_direction", "emm_receiver_channels", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
            "emm_grid_fdcoef", "emm_workspace_bytes", "emm_bind_device", "emm_model_set", "emm_run", "emm_run_begin",
            "emm_run_steps", "emm_run_enqueue", "emm_run_end", "emm_get", "emm_profile", "emm_profile_read",
            "emm_launch_count", "emm_last_error")
@@ -80,6 +80,8 @@ def lib():
         L.emm_last_error.restype = C.c_char_p
         L.emm_nugrid.argtypes = [C.c_int, C.c_double, C.c_double, dp, dp]
         L.emm_fd_weights.argtypes = [C.c_int, dp, C.c_double, dp, dp]
+        L.emm_dipole_direction.argtypes = [C.c_double, C.c_double, dp]
+        L.emm_receiver_channels.argtypes = [dp, C.c_int, dp, dp, dp]
         L.emm_grid_create.argtypes = [dp, C.c_int, dp, C.c_int, dp, C.c_int, C.POINTER(GridOpts), C.POINTER(vp)]
         L.emm_grid_destroy.argtypes = [vp]
         L.emm_grid_destroy.restype = None
@@ -126,6 +128,25 @@ def emm_fd_weights(nodes, x0):
     wi, wd = np.zeros(len(nodes)), np.zeros(len(nodes))
     _chk(lib().emm_fd_weights(len(nodes), _dptr(nodes), x0, _dptr(wi), _dptr(wd)))
     return wi, wd
+
+
+def emm_dipole_direction(azimuth, dip):
+    d = np.zeros(3)
+    _chk(lib().emm_dipole_direction(float(azimuth), float(dip), _dptr(d)))
+    return d
+
+
+def emm_receiver_channels(g6, azimuth, dip):
+    """g6: complex [nrec][6] (one source, one frequency of emm_run's output) -> complex [nrec][2] (E channel, H channel)"""
+    g6 = np.ascontiguousarray(g6, dtype=np.complex128)
+    n = g6.shape[0]
+    assert g6.shape == (n, 6)
+    az = np.ascontiguousarray(np.broadcast_to(np.asarray(azimuth, dtype=np.float64), (n,)))
+    dp_ = np.ascontiguousarray(np.broadcast_to(np.asarray(dip, dtype=np.float64), (n,)))
+    out = np.zeros((n, 2), dtype=np.complex128)
+    _chk(lib().emm_receiver_channels(g6.ctypes.data_as(C.POINTER(C.c_double)), n, _dptr(az), _dptr(dp_),
+                                     out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
 
 
 nugrid, fd_weights = emm_nugrid, emm_fd_weights     # same names as the oracle binding, for shared test helpers

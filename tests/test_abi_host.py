@@ -56,6 +56,27 @@ def test_nugrid_and_weights_agree_with_oracle(emm, oracle):
         emm.emm_nugrid(10, 100.0, 20.0)
 
 
+def test_acquisition_geometry_helpers(emm):
+    """azimuth/dip columns of the paper's source/receiver files (L632-640), reading [R13]: unit vector, x at (0,0),
+    y at azimuth pi/2, z (downward) at dip pi/2; a receiver channel is the projection of the six returned components."""
+    assert np.allclose(emm.emm_dipole_direction(0.0, 0.0), [1, 0, 0], atol=1e-15)
+    assert np.allclose(emm.emm_dipole_direction(np.pi / 2, 0.0), [0, 1, 0], atol=1e-15)
+    assert np.allclose(emm.emm_dipole_direction(0.3, np.pi / 2), [0, 0, 1], atol=1e-15)
+    rng = np.random.default_rng(11)
+    az, dip = rng.uniform(-np.pi, np.pi, 9), rng.uniform(-np.pi / 2, np.pi / 2, 9)
+    d = np.array([emm.emm_dipole_direction(a, b) for a, b in zip(az, dip)])
+    assert np.allclose(np.linalg.norm(d, axis=1), 1.0, atol=1e-15)
+    assert np.allclose(np.arctan2(d[:, 1], d[:, 0]), az, atol=1e-12) and np.allclose(np.arcsin(d[:, 2]), dip, atol=1e-12)
+    g6 = rng.normal(size=(9, 6)) + 1j * rng.normal(size=(9, 6))
+    ch = emm.emm_receiver_channels(g6, az, dip)
+    assert np.allclose(ch[:, 0], np.einsum("qc,qc->q", d, g6[:, :3]), atol=1e-14)
+    assert np.allclose(ch[:, 1], np.einsum("qc,qc->q", d, g6[:, 3:]), atol=1e-14)
+    # an x-oriented receiver reads Ex and Hx
+    assert np.allclose(emm.emm_receiver_channels(g6, 0.0, 0.0), g6[:, [0, 3]], atol=1e-15)
+    with pytest.raises(emm.EmmError):
+        emm.emm_dipole_direction(float("nan"), 0.0)
+
+
 def _workloads():
     nug = None
     from oracle import emm_oracle
