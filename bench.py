@@ -67,7 +67,7 @@ def algorithmic_bytes(info, nf, nb, kernel):
            * (info["box_hi3"] - info["box_lo3"] + 1))
     zs = (2 if info["k0"] < 0 else 1) * nb
     psi = 16 * (2 * nb * N2 * N3 + 2 * nb * N1 * N3 + zs * N1 * N2)
-    return (48 if kernel == "E" else 36) * N + 48 * nf * box + psi
+    return (48 if kernel[0] == "E" else 36) * N + 48 * (0 if kernel[1:] == "0" else nf) * box + psi
 
 
 class ClockSampler:
@@ -282,6 +282,20 @@ def run_gpu(args):
     g.run_steps(1)
     for c in ("E1", "H2"):
         assert np.all(np.isfinite(g.get(c)))
+    # extra: the same K steps with one DTFT term per step in every step (dtft_pair = -1: the paper's own schedule, L454)
+    unpaired = None
+    if 0 < len(w["freqs"]) <= 5:
+        g.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=K + Wm + 4, batched=1 if nsrc > 1 else 0, dtft_pair=-1))
+        g.run_enqueue(Wm)
+        torch.cuda.synchronize()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(g.stream)
+        g.run_enqueue(K)
+        d1.record(g.stream)
+        torch.cuda.synchronize()
+        msu = d0.elapsed_time(d1)
+        unpaired = {"ms_per_step": msu / K, "value": world * nsrc * N * K / (msu * 1e-3) / 1e9,
+                    "note": "dtft_pair=-1: every update kernel adds its one term of Eq. 25 in every step; same sums, twice the accumulator traffic"}
     # extra, not the headline: the same K steps with DTFT decimation at the automatic safe stride
     decim = None
     if len(w["freqs"]) > 0:
@@ -334,18 +348,26 @@ def run_gpu(args):
             peak, peak_src = float(json.load(open(peaks_file))["hbm_gbs"]), "of measured (MEASURED_PEAKS.json hbm_gbs)"
         else:
             peak, peak_src = 6650.0, "of fallback (B200_PROFILING.md)"
-        dom = "E" if prof["E"][0] >= prof["H"][0] else "H"
-        kms = prof[dom][0] / max(prof[dom][1], 1)
+        # instances of the update kernel in this run (paired DTFT: E0/H0 = accumulator-free steps, E2/H2 = two-term steps);
+        # the dominant one = the largest duration per launch
+        avg = {k: v[0] / v[1] for k, v in prof.items() if v[1] > 0}
+        dom = max(avg, key=avg.get)
+        kms = avg[dom]
+        inst = {"E": "k_update<R,NF,E>", "H": "k_update<R,NF,H>", "E0": "k_update<R,0,E>", "H0": "k_update<R,0,H>",
+                "E2": "k_update<R,NF,E,PAIR>", "H2": "k_update<R,NF,H,PAIR>"}
         abytes = nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], dom)
         achieved = abytes / (kms * 1e-3) / 1e9
         traffic = None
         tf = os.path.join(ROOT, "profiles", "ncu_traffic.json")
         if os.path.exists(tf):
             traffic = json.load(open(tf)).get("%s:%s:rd%d:nf%d" % (w["name"], dom, w["grid"]["rd"], len(w["freqs"])))
-        roofline = {"bound": "hbm", "kernel": "k_update<%s>" % dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+        tot_update = sum(v[0] for v in prof.values())
+        roofline = {"bound": "hbm", "kernel": inst[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "algorithmic_bytes_per_launch": abytes,
-                    "kernel_ms": kms, "kernels_ms_per_step": {"E": prof["E"][0] / max(prof["E"][1], 1), "H": prof["H"][0] / max(prof["H"][1], 1)},
-                    "step_frac_in_update_kernels": (prof["E"][0] + prof["H"][0]) / (ms_prof * Kp),
+                    "kernel_ms": kms, "kernels_ms_per_launch": avg,
+                    "instances_gbs": {k: nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], k) / (avg[k] * 1e-3) / 1e9 for k in avg},
+                    "update_kernels_ms_per_step": tot_update / Kp,
+                    "step_frac_in_update_kernels": tot_update / (ms_prof * Kp),
                     "ms_per_step_serialised": ms_prof,
                     "how": "kernel_ms from a serialised pass (emm_profile); `value` is timed with the air-water boundary overlapped on a second stream"}
         cpu = None
@@ -359,7 +381,9 @@ def run_gpu(args):
                 "e2e": {"value": world * nsrc * N * K / t_e2e / 1e9, "unit": "Gcell-updates/s", "h2d_bytes_per_step": h2d / K,
                         "d2h_bytes_per_step": d2h / K, "seconds": t_e2e,
                         "what": "emm_model_set (host sigma -> device) + emm_run(fixed_steps=K) (tables up, receivers back)"},
-                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched, "dtft_decimation": decim, "receivers_only_dtft": rec_only,
+                "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched,
+                "dtft": "every term of Eq. 25, two consecutive terms per accumulator pass (emm_run_opts.dtft_pair, default)" if unpaired else "every term of Eq. 25, one per step",
+                "dtft_one_term_per_step": unpaired, "dtft_decimation": decim, "receivers_only_dtft": rec_only,
                 "multi_gpu": "replicas only: every rank runs the whole workload, no collective on the data path"}
         print(json.dumps(line))
     if world > 1:

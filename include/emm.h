@@ -79,6 +79,16 @@ typedef struct {
                       run without the 96*nf B/node term.  Same sums at those nodes, so emm_run returns the same
                       Green's functions and step counts; for runs that only want receiver data.
                       0: accumulators for every frequency on the whole DTFT box, as the paper does (L454)            */
+  int dtft_pair;   /* Paired DTFT (default, 0): every term of Eq. 25 is taken, two consecutive terms per read-modify-write
+                      of the accumulators.  An update kernel holds the field before and after its own update, i.e. the
+                      DTFT operands of two consecutive steps (L372: old H of steps it and it+1; new E of steps it-1 and
+                      it), so the steps are taken two by two: the H kernel adds both H terms in the first step, the E
+                      kernel both E terms in the second; each accumulator gets the same fused multiply-adds in the same
+                      order as with one term per step, at half the 96*nf B/node traffic.  Pairs never cross a convergence
+                      check or the end of an emm_run_steps/emm_run_enqueue batch (a left-over step takes single terms),
+                      so accumulators are complete whenever they can be read.  Applies to 1..5 frequencies with full-grid
+                      accumulators and dtft_every <= 1; otherwise ignored.  -1: one term per step in every step, as the
+                      paper's kernels do (L454, L880-884)                                                            */
 } emm_run_opts;
 
 /* integer grid facts for emm_grid_info(): */
@@ -170,7 +180,8 @@ int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_out);
 
 /* Optional timing of the two fused update kernels: emm_profile(g,1) brackets every later launch of the
  * E and H update kernel with CUDA events on the bound stream; emm_profile_read drains the stream and
- * returns the summed durations ms[2] = {E kernel, H kernel} and launch counts, then resets.           */
+ * returns the summed durations and launch counts, then resets.  ms[6], counts[6]: {E, H} one-term (or decimated)
+ * instances, {E, H} accumulator-free steps of a DTFT pair, {E, H} two-term steps of a DTFT pair.      */
 int emm_profile(emm_grid *g, int enable);
 int emm_profile_read(emm_grid *g, double *ms, int *counts);
 

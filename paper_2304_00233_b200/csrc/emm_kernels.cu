@@ -167,12 +167,33 @@ __device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0
   }
 }
 
+// Two consecutive terms of Eq. 25 in one read-modify-write of the accumulators (paired DTFT): the
+// update kernel holds the field before (uo) and after (un) its own update, i.e. the DTFT operands of two consecutive
+// steps.  F = fma(un, tb, fma(uo, ta, F)): the same two fused multiply-adds, in the same order, as two single-term passes.
+template <int NF>
+__device__ __forceinline__ void dtft4_staged2(const float4 *sm, int c, float2 *F0, size_t fstride, float4 uo, float4 un,
+                                              const float2 (&ta)[NF > 0 ? NF : 1], const float2 (&tb)[NF > 0 ? NF : 1]) {
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    float4 a0 = sm[((c * NF + f) * 2 + 0) * 128], a1 = sm[((c * NF + f) * 2 + 1) * 128];
+    a0.x = fmaf(uo.x, ta[f].x, a0.x); a0.y = fmaf(uo.x, ta[f].y, a0.y); a0.z = fmaf(uo.y, ta[f].x, a0.z); a0.w = fmaf(uo.y, ta[f].y, a0.w);
+    a1.x = fmaf(uo.z, ta[f].x, a1.x); a1.y = fmaf(uo.z, ta[f].y, a1.y); a1.z = fmaf(uo.w, ta[f].x, a1.z); a1.w = fmaf(uo.w, ta[f].y, a1.w);
+    a0.x = fmaf(un.x, tb[f].x, a0.x); a0.y = fmaf(un.x, tb[f].y, a0.y); a0.z = fmaf(un.y, tb[f].x, a0.z); a0.w = fmaf(un.y, tb[f].y, a0.w);
+    a1.x = fmaf(un.z, tb[f].x, a1.x); a1.y = fmaf(un.z, tb[f].y, a1.y); a1.z = fmaf(un.w, tb[f].x, a1.z); a1.w = fmaf(un.w, tb[f].y, a1.w);
+    float *p = reinterpret_cast<float *>(F0 + f * fstride);
+    stcs4(p, a0);
+    stcs4(p + 4, a1);
+  }
+}
+
 // Blocks per SM the register allocation is aimed at.  Measured on B200 (profiles/r1_kernel_experiments.md): with
 // many frequencies (>= 4: 48+ KB of staged accumulators per block) two fat blocks per SM win -- no register cap,
 // and the unified L1 keeps ~100 KB for the neighbour rows; with fewer frequencies three blocks win.
 template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_MINB : (NF >= 4 ? 2 : 3); }
 
-template <int R, int NF, bool IS_H>
+// PAIR: the two-term instance of the paired DTFT (NF >= 1, staged): the H kernel of step `it` takes the terms it and
+// it+1 of F_H (old and new H), the E kernel of step `it` the terms it-1 and it of F_E (old and new E) [R6].
+template <int R, int NF, bool IS_H, bool PAIR = false>
 __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0, const int sel) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
   const int src = blockIdx.z / nchunks, chunk = chunk0 + blockIdx.z - src * nchunks;   // this launch covers chunks [chunk0, chunk0 + nchunks)
@@ -186,7 +207,8 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   const int it = *s.it;
   // DTFT decimation runs two instances per pass: sel 1 = the accumulator-free one, for the steps that skip the DTFT;
   // sel 2 = the DTFT one, for the steps that contribute; the instance whose turn it is not exits here (sel 0: no split)
-  if (sel && ((sel == 2) != (it % s.dft_every == 0))) return;
+  // sel 3 = accumulator-free, unconditionally (the step of a DTFT pair in which this kernel takes no term)
+  if ((sel == 1 || sel == 2) && ((sel == 2) != (it % s.dft_every == 0))) return;
 
   const float *A1 = (IS_H ? s.E[0] : s.H[0]) + (size_t)src * g.VS;
   const float *A2 = (IS_H ? s.E[1] : s.H[1]) + (size_t)src * g.VS;
@@ -226,14 +248,18 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 
   // DTFT bookkeeping
   const int nf = s.nf;
-  const bool dft_xy = (sel != 1) && (nf > 0) && (it % s.dft_every == 0) &&        // DTFT decimation: this step contributes or not
+  const bool dft_xy = (sel != 1) && (sel != 3) && (nf > 0) && (it % s.dft_every == 0) &&        // DTFT decimation: this step contributes or not
                       (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);
   const size_t fstride = (size_t)6 * g.NZB * g.PS;      // float2 elements between frequencies
   float2 *Fsrc = s.F + (size_t)src * nf * fstride + (size_t)(IS_H ? 3 : 0) * g.NZB * g.PS;
-  const float2 *twp = (IS_H ? s.twH : s.twE) + (size_t)it * nf;
-  float2 tw[NF > 0 ? NF : 1];
+  const float2 *twp = (IS_H ? s.twH : s.twE) + (size_t)(PAIR && !IS_H ? it - 1 : it) * nf;    // PAIR: first of the two terms
+  float2 tw[NF > 0 ? NF : 1], tw2[PAIR && NF > 0 ? NF : 1];
 #pragma unroll
   for (int f = 0; f < NF; ++f) tw[f] = __ldg(twp + f);
+  if constexpr (PAIR) {
+#pragma unroll
+    for (int f = 0; f < NF; ++f) tw2[f] = __ldg(twp + nf + f);
+  }
 
   const size_t row = (size_t)j * g.P1 + i0;
   // z queues of A1, A2: planes k-R+O .. k+R-1+O
@@ -246,6 +272,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   }
 
   constexpr bool STAGED = (EMM_CPA != 0) && (NF > 0);
+  static_assert(!PAIR || STAGED, "the paired DTFT instance needs staged accumulators");
   extern __shared__ float4 smF_all[];
   float4 *smF = smF_all + (threadIdx.y * blockDim.x + threadIdx.x);
   const size_t cstride = (size_t)g.NZB * g.PS;
@@ -363,17 +390,22 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     const bool dft = dft_xy && k >= g.blo[2] && k <= g.bhi[2];
     float2 *Fk = Fsrc + (size_t)(k - g.blo[2]) * g.PS + row;
     // one component: wait for its staged accumulators, add u * twiddle, stream out, refill the slots for plane k+1
-    auto dtft_staged_component = [&](int c, float4 u) {
+    auto dtft_staged_component = [&](int c, float4 u, float4 un = zero4()) {
       cp_async_wait_2();
-      if (dft) dtft4_staged<NF>(smF, c, Fk + c * cstride, fstride, u, tw);
+      if (dft) {
+        if constexpr (PAIR) dtft4_staged2<NF>(smF, c, Fk + c * cstride, fstride, u, un, tw, tw2);
+        else dtft4_staged<NF>(smF, c, Fk + c * cstride, fstride, u, tw);
+      }
       if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2])
         stage_component<NF>(smF, c, Fk + g.PS + c * cstride, fstride);
       cp_async_commit();
     };
 
+    const float4 o1 = u1, o2 = u2, o3 = u3;      // the fields before this update (PAIR: first of the two DTFT terms)
     if (IS_H) {
       // old H sits at t = it*dt, the time level of J (Eq. 8; [R6])
-      if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
+      if constexpr (PAIR) {}
+      else if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
       else if (dft) {
         if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
         else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
@@ -383,13 +415,16 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u2 = make_float4(fmaf(-m0, c2.x, u2.x), fmaf(-m1, c2.y, u2.y), fmaf(-m2, c2.z, u2.z), fmaf(-m3, c2.w, u2.w));
       u3 = make_float4(fmaf(-m0, c3.x, u3.x), fmaf(-m1, c3.y, u3.y), fmaf(-m2, c3.z, u3.z), fmaf(-m3, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
+      // PAIR: old H is term it, new H is term it+1 (the old H of the next step)
+      if constexpr (PAIR) { dtft_staged_component(0, o1, u1); dtft_staged_component(1, o2, u2); dtft_staged_component(2, o3, u3); }
     } else {
       u1 = make_float4(fmaf(e1.x, c1.x, u1.x), fmaf(e1.y, c1.y, u1.y), fmaf(e1.z, c1.z, u1.z), fmaf(e1.w, c1.w, u1.w));
       u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
-      // new E sits at t = (it+1/2)*dt [R6]
-      if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
+      // new E sits at t = (it+1/2)*dt [R6]; PAIR: old E is term it-1, new E is term it
+      if constexpr (PAIR) { dtft_staged_component(0, o1, u1); dtft_staged_component(1, o2, u2); dtft_staged_component(2, o3, u3); }
+      else if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
       else if (dft) {
         if constexpr (NF > 0) { dtft4<NF>(Fk, fstride, u1, tw); dtft4<NF>(Fk + cstride, fstride, u2, tw); dtft4<NF>(Fk + 2 * cstride, fstride, u3, tw); }
         else { dtft4_rt(Fk, fstride, u1, twp, nf); dtft4_rt(Fk + cstride, fstride, u2, twp, nf); dtft4_rt(Fk + 2 * cstride, fstride, u3, twp, nf); }
@@ -401,13 +436,33 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 // ---- source injection (Eq. 8, [R7]): electric dipoles E_c[node] -= s(it dt) * (dt/eps W_c)[node] before the E
 // update; magnetic dipoles H_c[node] -= s((it+1/2) dt) * (dt/mu W_c)[node] after the H update and its boundary ----
 __global__ void k_inject(const DevGrid g, const DevState s, const int *__restrict__ off, const int *__restrict__ idx,
-                         const float *__restrict__ w, const int magnetic) {
+                         const float *__restrict__ w, const int magnetic, const int pairfix) {
   const int src = blockIdx.x;
   if (s.done[src] || s.src_mag[src] != magnetic) return;
-  const float st = magnetic ? s.wavh[*s.it] : s.wav[*s.it];
+  const int it = *s.it;
+  const float st = magnetic ? s.wavh[it] : s.wav[it];
+  // Paired DTFT: the two-term kernel sees the injected nodes at the wrong side of this injection for one of its
+  // terms -- electric: the E kernel of this step reads (E - st w) as the old E of term it-1; magnetic: the H kernel
+  // of this step took the new H of term it+1 before (- st w) was added.  The missing product goes into F here.
+  const float2 *twf = magnetic ? s.twH + (size_t)(it + 1) * s.nf : s.twE + (size_t)(it - 1) * s.nf;
+  const float sg = magnetic ? -1.f : 1.f;
+  const size_t fstride = (size_t)6 * g.NZB * g.PS;
   for (int c = 0; c < 3; ++c) {
     float *U = (magnetic ? s.H[c] : s.E[c]) + (size_t)src * g.VS;
-    for (int n = off[src * 3 + c] + threadIdx.x; n < off[src * 3 + c + 1]; n += blockDim.x) U[idx[n]] -= st * w[n];
+    float2 *F = s.F + (size_t)src * s.nf * fstride + (size_t)(c + (magnetic ? 3 : 0)) * g.NZB * g.PS;
+    for (int n = off[src * 3 + c] + threadIdx.x; n < off[src * 3 + c + 1]; n += blockDim.x) {
+      U[idx[n]] = fmaf(-st, w[n], U[idx[n]]);        // one rounding, with or without pairfix
+      if (pairfix) {
+        const float d = __fmul_rn(st, w[n]);
+        const int k = idx[n] / (int)g.PS, rem = idx[n] - k * (int)g.PS, j = rem / g.P1, i = rem - j * g.P1;
+        if (k >= g.blo[2] && k <= g.bhi[2] && j >= g.blo[1] && j <= g.bhi[1] && i >= g.blo[0] && i <= g.bhi[0])
+          for (int f = 0; f < s.nf; ++f) {
+            float2 &a = F[f * fstride + (size_t)(k - g.blo[2]) * g.PS + rem];
+            a.x = fmaf(sg * d, twf[f].x, a.x);
+            a.y = fmaf(sg * d, twf[f].y, a.y);
+          }
+      }
+    }
   }
 }
 
@@ -550,16 +605,30 @@ __global__ void k_rec_interp(const DevGrid g, const DevState s, const int *__res
   } while (0)
 
 // unrolled-NF instantiations stage one plane of accumulators per thread in dynamic shared memory
-template <int R, int NF, bool IS_H>
+template <int R, int NF, bool IS_H, bool PAIR = false>
 static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
   const size_t smem = EMM_CPA ? (size_t)3 * NF * 2 * 128 * sizeof(float4) : 0;
   static bool configured = false;
   if (!configured && smem > 48 * 1024) {
-    cudaFuncSetAttribute(k_update<R, NF, IS_H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_update<R, NF, IS_H, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
-  k_update<R, NF, IS_H><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel);
+  k_update<R, NF, IS_H, PAIR><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel);
 }
+
+#if EMM_CPA
+// two-term instances of the paired DTFT (1..kPairMaxNF frequencies)
+template <int R, bool IS_H>
+static void launch_update_pair(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0) {
+  switch (nf) {
+    case 1: launch_one<R, 1, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
+    case 2: launch_one<R, 2, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
+    case 3: launch_one<R, 3, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
+    case 4: launch_one<R, 4, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
+    default: launch_one<R, 5, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
+  }
+}
+#endif
 
 template <int R, bool IS_H>
 static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
@@ -576,12 +645,14 @@ static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 
 
 // part: 0 = every z chunk, 1 = only the chunks next to the air-water plane (their stencils read the ghost planes),
 // 2 = all the others.  Parts 1 and 2 can run on different streams (emm_run.cu overlaps the boundary with part 2).
-int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st) {
+// mode: 0 = one DTFT term per step (and DTFT decimation); paired DTFT: 1 = the step in which this kernel takes no
+// term (accumulator-free instance), 2 = the step in which it takes two (PAIR instance)
+int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, cudaStream_t st) {
   const DevGrid &dg = g->dg;
   const int quads = dg.P1 / 4;
   const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
   // launch one instance (nf = accumulators it is compiled for) over the chunks of `part`
-  auto launch = [&](int nf, int sel) -> int {
+  auto launch = [&](int nf, int sel, bool pair = false) -> int {
     // block: TX quads wide, 128 threads.  With accumulators: 16 or 32 quads, whichever wastes fewer lanes (long
     // contiguous accumulator rows); without: 8 quads x 16 rows, more y reuse in L1 (profiles/r1_kernel_experiments.md)
     int TX = 16;
@@ -610,7 +681,21 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream
     if (nchunks <= 0) return 0;
     dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
     if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
-    if (is_h) {
+    if (pair) {
+#if EMM_CPA
+      if (is_h) {
+        if (dg.r == 1) launch_update_pair<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+        else if (dg.r == 2) launch_update_pair<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+        else launch_update_pair<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+      } else {
+        if (dg.r == 1) launch_update_pair<1, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+        else if (dg.r == 2) launch_update_pair<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+        else launch_update_pair<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+      }
+#else
+      return fail(EMM_EINVAL, "launch_update: paired DTFT needs the staged accumulators (EMM_CPA)");
+#endif
+    } else if (is_h) {
       if (dg.r == 1) launch_update_nf<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
       else if (dg.r == 2) launch_update_nf<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
       else launch_update_nf<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
@@ -628,7 +713,11 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream
     cudaEventRecord(e0, st);
   }
   int rc;
-  if (s.nf > 0 && s.dft_every > 1) {
+  if (mode == 1) {
+    if ((rc = launch(0, 3))) return rc;
+  } else if (mode == 2) {
+    if ((rc = launch(s.nf, 0, true))) return rc;
+  } else if (s.nf > 0 && s.dft_every > 1) {
     // DTFT decimation: most steps take no accumulator at all.  Both instances are launched every step (the step index
     // lives on the device, so that a captured graph can be replayed); the one whose turn it is not exits at once.
     if ((rc = launch(0, 1)) || (rc = launch(s.nf, 2))) return rc;
@@ -639,13 +728,13 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream
     cudaEventRecord(e1, st);
     g->prof_ev.push_back(e0);
     g->prof_ev.push_back(e1);
-    g->prof_kind.push_back(is_h);
+    g->prof_kind.push_back(is_h + 2 * mode);
   }
   return 0;
 }
 
-int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic) {
-  k_inject<<<s.nsrc, 128, 0, g->stream>>>(g->dg, s, r.src_off, r.src_idx, r.src_w, magnetic);
+int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic, int pairfix) {
+  k_inject<<<s.nsrc, 128, 0, g->stream>>>(g->dg, s, r.src_off, r.src_idx, r.src_w, magnetic, pairfix);
   EMM_LAUNCH_CHECK(g, "k_inject");
   return 0;
 }

@@ -37,8 +37,11 @@ struct DevRun {
 };
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
-int launch_update(emm_grid *g, const DevState &s, int is_h, int part, cudaStream_t st);
-int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic);
+// mode: 0 = one DTFT term per step; paired DTFT: 1 = accumulator-free step of this kernel, 2 = its two-term step
+int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, cudaStream_t st);
+constexpr int kPairMaxNF = 5;       // two-term instances exist for 1..5 frequencies (the staged, unrolled ones)
+// pairfix: also add the product the two-term kernel misses at the injected nodes (see k_inject)
+int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic, int pairfix);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_rec_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);

@@ -20,6 +20,7 @@ struct Run {
   int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
   int it_min = 0, it_host = 0, table_steps = 0, dtft_every = 1;
   bool sparse = false;                   // receivers-only DTFT (emm_run_opts.sparse_dft)
+  bool pair = false;                     // paired DTFT: two consecutive terms of Eq. 25 per accumulator pass (emm_run_opts.dtft_pair)
   std::vector<double> wav, wavh;            // s(it dt), s((it+1/2) dt) rounded to fp32 (what the device injects)
   std::vector<int> mag;                     // [nsrc] 1 = magnetic dipole
   bool any_mag = false, any_el = false;
@@ -406,21 +407,30 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
   for (int q = 0; q < n; ++q) {
     if (R->it_host >= R->table_steps) return fail(EMM_EINVAL, "run: step %d beyond the twiddle table (max_steps)", R->it_host);
     cudaStream_t M = g->stream, B = g->stream_b;
-    if (R->any_el && (rc = launch_inject(g, R->ds, R->dr, 0))) return rc;     // Alg. 1 L477 (before the update: same sum)
+    // Paired DTFT: the steps of this batch are taken two by two.  In the first step of a pair the H kernel adds the terms
+    // it and it+1 of F_H (old and new H) and the E kernel none; in the second the E kernel adds the terms it-1 and it of
+    // F_E (old and new E) and the H kernel none; a left-over last step takes its single terms as usual.  A batch never
+    // crosses a convergence check (enqueue_steps), so every sum is complete where it is read.
+    int me = 0, mh = 0;
+    if (R->pair) {
+      if (q & 1) { me = 2; mh = 1; }
+      else if (q + 1 < n && R->it_host + 1 < R->table_steps) { me = 1; mh = 2; }
+    }
+    if (R->any_el && (rc = launch_inject(g, R->ds, R->dr, 0, me == 2))) return rc;     // Alg. 1 L477 (before the update: same sum)
     if (g->top != EMM_TOP_AIR) {
-      if ((rc = launch_update(g, R->ds, 0, 0, M))) return rc;                 // L476-479 + E part of L483
+      if ((rc = launch_update(g, R->ds, 0, 0, me, M))) return rc;                 // L476-479 + E part of L483
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                // check-set part of L483
       if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_update(g, R->ds, 1, 0, M))) return rc;                 // H part of L483 + L486-489
+      if ((rc = launch_update(g, R->ds, 1, 0, mh, M))) return rc;                 // H part of L483 + L486-489
     } else if (g->prof || no_overlap) {
       // one thing after the other (per-kernel timing, or EMM_NO_OVERLAP): the boundary still runs on its own stream
-      if ((rc = launch_update(g, R->ds, 0, 0, M))) return rc;
+      if ((rc = launch_update(g, R->ds, 0, 0, me, M))) return rc;
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));
       if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
       CU(cudaEventRecord(g->ev[1], B)); CU(cudaStreamWaitEvent(M, g->ev[1], 0));
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
       if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_update(g, R->ds, 1, 0, M))) return rc;
+      if ((rc = launch_update(g, R->ds, 1, 0, mh, M))) return rc;
       CU(cudaEventRecord(g->ev[2], M)); CU(cudaStreamWaitEvent(B, g->ev[2], 0));
       if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));
@@ -428,22 +438,22 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       // The boundary only feeds the z chunks next to the surface: those chunks and the FFT boundary form a short
       // chain on the helper stream while the bulk of the grid is updated on the main stream (fork/join per step).
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));      // fork (after the injection)
-      if ((rc = launch_update(g, R->ds, 0, 1, B))) return rc;                 // E, surface chunks
+      if ((rc = launch_update(g, R->ds, 0, 1, me, B))) return rc;                 // E, surface chunks
       CU(cudaEventRecord(g->ev[1], B));
       if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
-      if ((rc = launch_update(g, R->ds, 0, 2, M))) return rc;                 // E, bulk
+      if ((rc = launch_update(g, R->ds, 0, 2, me, M))) return rc;                 // E, bulk
       CU(cudaEventRecord(g->ev[2], M));
       CU(cudaStreamWaitEvent(M, g->ev[1], 0));                                // H bulk and the check set read surface-chunk E
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
       if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
       CU(cudaEventRecord(g->ev[4], M));
-      if ((rc = launch_update(g, R->ds, 1, 2, M))) return rc;                 // H, bulk
+      if ((rc = launch_update(g, R->ds, 1, 2, mh, M))) return rc;                 // H, bulk
       CU(cudaStreamWaitEvent(B, g->ev[2], 0)); CU(cudaStreamWaitEvent(B, g->ev[4], 0));
-      if ((rc = launch_update(g, R->ds, 1, 1, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
+      if ((rc = launch_update(g, R->ds, 1, 1, mh, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
       if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));      // join
     }
-    if (R->any_mag && (rc = launch_inject(g, R->ds, R->dr, 1))) return rc;    // L488, after the H update and its boundary
+    if (R->any_mag && (rc = launch_inject(g, R->ds, R->dr, 1, mh == 2))) return rc;    // L488, after the H update and its boundary
     if (R->nf > 0 && (R->it_host + 1) % R->check_every == 0 &&
         (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
     if ((rc = launch_step_end(g, R->ds))) return rc;
@@ -534,6 +544,10 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     R->check_set = o->check_set;
     R->dtft_every = o->dtft_every > 1 ? o->dtft_every : 1;
     R->sparse = o->sparse_dft != 0 && nf > 0;
+    {
+      static const bool no_pair = getenv("EMM_NO_PAIR") != nullptr;       // A/B measurements
+      R->pair = o->dtft_pair >= 0 && !no_pair && nf >= 1 && nf <= kPairMaxNF && !R->sparse && o->dtft_every >= 0 && o->dtft_every <= 1;
+    }
     if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
     R->table_steps = (R->fixed_steps ? R->fixed_steps : R->max_steps) + 1;
     double fhi = 0;
@@ -893,8 +907,7 @@ extern "C" int emm_profile(emm_grid *g, int enable) {
 extern "C" int emm_profile_read(emm_grid *g, double *ms, int *counts) {
   if (!g || !ms || !counts) return fail(EMM_EINVAL, "emm_profile_read: null argument");
   CU(cudaStreamSynchronize(g->stream));
-  ms[0] = ms[1] = 0.0;
-  counts[0] = counts[1] = 0;
+  for (int q = 0; q < 6; ++q) { ms[q] = 0.0; counts[q] = 0; }
   for (size_t q = 0; q < g->prof_kind.size(); ++q) {
     float t = 0.f;
     CU(cudaEventElapsedTime(&t, g->prof_ev[2 * q], g->prof_ev[2 * q + 1]));

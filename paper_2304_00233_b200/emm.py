@@ -58,7 +58,7 @@ class Src(C.Structure):
 class RunOpts(C.Structure):
     _fields_ = [("max_steps", C.c_int), ("fixed_steps", C.c_int), ("tol", C.c_double),
                 ("check_every", C.c_int), ("check_set", C.c_int), ("fmax", C.c_double), ("batched", C.c_int),
-                ("dtft_every", C.c_int), ("sparse_dft", C.c_int)]
+                ("dtft_every", C.c_int), ("sparse_dft", C.c_int), ("dtft_pair", C.c_int)]
 
 
 class EmmError(RuntimeError):
@@ -165,8 +165,8 @@ def _ropts(o):
     o = dict(o or {})
     r = RunOpts(int(o.pop("max_steps", 0)), int(o.pop("fixed_steps", 0)), float(o.pop("tol", 0)),
                 int(o.pop("check_every", 0)), int(o.pop("check_set", CHECK_FACES)), float(o.pop("fmax", 0)),
-                int(o.pop("batched", 0)), int(o.pop("dtft_every", 0)), int(o.pop("sparse_dft", 0)))
-    o.pop("sparse_dft", None)
+                int(o.pop("batched", 0)), int(o.pop("dtft_every", 0)), int(o.pop("sparse_dft", 0)),
+                int(o.pop("dtft_pair", 0)))
     if o:
         raise TypeError("unknown run options %s" % sorted(o))
     return r
@@ -328,10 +328,12 @@ class Grid:
         _chk(lib().emm_profile(self._h, int(enable)))
 
     def profile_read(self):
-        ms = np.zeros(2)
-        cnt = np.zeros(2, dtype=np.int32)
+        """(summed ms, launches) per update-kernel instance: E/H = one DTFT term per step (or decimated), E0/H0 = the
+        accumulator-free steps of a DTFT pair, E2/H2 = its two-term steps."""
+        ms = np.zeros(6)
+        cnt = np.zeros(6, dtype=np.int32)
         _chk(lib().emm_profile_read(self._h, _dptr(ms), cnt.ctypes.data_as(C.POINTER(C.c_int))))
-        return {"E": (float(ms[0]), int(cnt[0])), "H": (float(ms[1]), int(cnt[1]))}
+        return {k: (float(ms[q]), int(cnt[q])) for q, k in enumerate(("E", "H", "E0", "H0", "E2", "H2"))}
 
     def launch_count(self):
         return int(lib().emm_launch_count(self._h))

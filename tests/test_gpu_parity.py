@@ -40,7 +40,7 @@ def _group_errors(ga, gb, s):
     return d, n, grp
 
 
-def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, batched=0, dtft_every=0):
+def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, batched=0, dtft_every=0, dtft_pair=0):
     """Field parity at four checkpoints up to `nsteps` (200 in north_star).
 
     Tolerance: relative L2 <= 1e-5 per field wherever the field still
@@ -54,7 +54,7 @@ def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, bat
     assert abs(ga.info()["dt"] / gb.info()["dt"] - 1) < 1e-12
     for c in ("CE1", "CE2", "CE3"):
         assert _rel_l2(ga.get(c), gb.get(c)) < 1e-7, c
-    ga.run_begin(sources, w["freqs"], w["receivers"], opts)
+    ga.run_begin(sources, w["freqs"], w["receivers"], dict(opts, dtft_pair=dtft_pair))   # scheduling of the same sums: not an oracle option
     gb.run_begin(sources, w["freqs"], w["receivers"], opts)
     peak = [{"E": 0.0, "H": 0.0} for _ in sources]
     done_steps, strict_checks = 0, 0
@@ -92,14 +92,15 @@ def _field_parity(emm, oracle, w, nsteps, tol=1e-5, ftol=2e-5, sources=None, bat
     ga.close()
 
 
-@pytest.mark.parametrize("rd", [1, 2, 3])
-def test_fields_wholespace_cpml(emm, oracle, rd):
-    """configs[0] scaled: homogeneous, CPML on six faces; 70 x-nodes (2 tiles + ragged tail), 200 steps."""
+@pytest.mark.parametrize("rd,pair", [(1, 0), (2, 0), (3, 0), (2, -1)])
+def test_fields_wholespace_cpml(emm, oracle, rd, pair):
+    """configs[0] scaled: homogeneous, CPML on six faces; 70 x-nodes (2 tiles + ragged tail), 200 steps.
+    pair = 0: paired DTFT (default); -1: one term per step in every step."""
     w = W.cfg1(n=40 - 2 * rd, dx=100.0, rd=rd, nb=7)
     src = np.array(w["sources"][0][0])
     offs = np.array([300.0, 600.0, 900.0, 1200.0])        # off-axis, off-grid: all six components are non-zero
     w["receivers"] = np.stack([src[0] + 0.8 * offs, src[1] + 0.36 * offs, src[2] - 0.48 * offs], axis=1)
-    _field_parity(emm, oracle, w, 200)
+    _field_parity(emm, oracle, w, 200, dtft_pair=pair)
 
 
 @pytest.mark.parametrize("rd", [1, 2, 3])
@@ -115,14 +116,14 @@ def _small_receivers():
     return np.stack([X.ravel(), Y.ravel(), np.full(X.size, 1000.0)], axis=1)
 
 
-@pytest.mark.parametrize("rd,builder", [(2, "cfg3"), (3, "cfg4")])
-def test_fields_nonuniform_aux_plane_vti(emm, oracle, rd, builder):
+@pytest.mark.parametrize("rd,builder,pair", [(2, "cfg3", 0), (3, "cfg4", 0), (3, "cfg4", -1)])
+def test_fields_nonuniform_aux_plane_vti(emm, oracle, rd, builder, pair):
     """configs[2]/[3] scaled: non-uniform x-y-z, VTI cells from sub-sampling, auxiliary-plane air boundary."""
     kw = dict(nx=40, nz=36, rd=rd, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
     w = W.build(builder, oracle.nugrid, **kw)
     w["receivers"] = _small_receivers()
     w["sigma_v"] = (w["sigma_v"] * 0.6).astype(np.float32)                # make the anisotropy bite everywhere
-    _field_parity(emm, oracle, w, 200)
+    _field_parity(emm, oracle, w, 200, dtft_pair=pair)
 
 
 def test_fields_batched_sources(emm, oracle):
@@ -176,6 +177,52 @@ def test_receivers_only_dtft_matches_full_grid_and_oracle(emm, oracle, m):
         ga.get("F_E1")
     assert e.value.code == emm.EINVAL
     ga.run_end()
+
+
+def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle):
+    """Paired DTFT (emm_run_opts.dtft_pair, default): two consecutive terms of Eq. 25 per pass over the accumulators.
+    Same fused multiply-adds in the same order as one term per step, so fields and accumulators are bit-identical to
+    the dtft_pair = -1 run everywhere except at the injected nodes (where the missing product is added by the
+    injection kernel, rounding order differs), whatever the batch sizes (odd batches leave single steps), for an
+    electric and a magnetic dipole batched on the non-uniform grid with the air-water boundary.  Then run to
+    convergence with an odd check interval: step counts identical, receivers the same to rounding, and both match
+    the oracle."""
+    w = W.cfg3(oracle.nugrid, nx=36, nz=32, rd=2, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
+    w["receivers"] = _small_receivers()
+    srcs = [((-150.0, 30.0, 950.0), (1.0, 0.2, 0.1)), ((120.0, -60.0, 930.0), (0.1, 1.0, 0.3), "M")]
+    ga, gs = make_grid(emm, w), make_grid(emm, w)
+    ga.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=131, batched=1))
+    gs.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=131, batched=1, dtft_pair=-1))
+    total = 0
+    for n in (7, 50, 1, 33, 40):                     # 131 steps: odd and even batches, a pair split by a batch end
+        na, _ = ga.run_steps(n)
+        ns, _ = gs.run_steps(n)
+        total += n
+        assert list(na) == list(ns) == [total, total]
+        for s in range(2):
+            for c in FIELDS:
+                assert np.array_equal(ga.get(c, isrc=s), gs.get(c, isrc=s)), (total, s, c)
+            for f in (0, len(w["freqs"]) - 1):
+                for c in FIELDS:
+                    Fa, Fs = ga.get("F_" + c, isrc=s, ifreq=f), gs.get("F_" + c, isrc=s, ifreq=f)
+                    differ = Fa != Fs
+                    assert differ.sum() <= 6 ** 3, (total, s, f, c, int(differ.sum()))     # at most one source stencil
+                    assert np.abs(Fa - Fs).max() <= 1e-5 * np.abs(Fs).max(), (total, s, f, c)
+    assert np.abs(gs.get("F_E1", isrc=0, ifreq=0)).max() > 0 and np.abs(gs.get("F_H2", isrc=1, ifreq=0)).max() > 0
+    oa, _ = ga.run_end()
+    os_, _ = gs.run_end()
+    assert np.abs(oa - os_).max() <= 1e-5 * np.abs(os_).max()
+    opts = dict(tol=1e-6, check_every=75, batched=1)
+    o_p, n_p = ga.run(srcs, w["freqs"], w["receivers"], opts)
+    o_s, n_s = gs.run(srcs, w["freqs"], w["receivers"], dict(opts, dtft_pair=-1))
+    o_or, n_or = make_grid(oracle, w).run(srcs, w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
+    assert list(n_p) == list(n_s) == list(n_or) and min(n_p) > 0 and n_p[0] % 75 == 0
+    for s in range(2):
+        for sl in (slice(0, 3), slice(3, 6)):
+            ref = o_or[s][..., sl]
+            big = np.abs(ref) > 1e-3 * np.abs(ref).max()
+            assert (np.abs(o_p[s][..., sl] - ref)[big] / np.abs(ref)[big]).max() < 1e-3
+            assert (np.abs(o_p[s][..., sl] - o_s[s][..., sl])[big] / np.abs(ref)[big]).max() < 1e-5
 
 
 def test_plane_and_separable_air_routes_agree(emm, oracle, monkeypatch):
