@@ -298,6 +298,12 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       if (!IS_H) { prefetch_l2(g.ce[0] + c1); prefetch_l2(g.ce[1] + c1); prefetch_l2(g.ce[2] + c1); }
       prefetch_l2(A3 + c1);
       prefetch_l2(A1 + (size_t)(k + R + O) * g.PS + row); prefetch_l2(A2 + (size_t)(k + R + O) * g.PS + row);
+      // CPML memory variables of the next plane (slab threads only): their loads sit behind the derivative they
+      // update, so without this they are a second, DRAM-long round trip per plane
+      if (xq) { const size_t pn = ((size_t)(k + 1) * g.N2 + j) * g.XS; prefetch_l2(psx0 + pn); prefetch_l2(psx1 + pn); }
+      if (sj >= 0) { const size_t pn = ((size_t)(k + 1) * 2 * g.nb + sj) * g.P1 + i0; prefetch_l2(psy0 + pn); prefetch_l2(psy1 + pn); }
+      const int skn = slab_of(k + 1, g.N3, g.nb, g.zslab_lo);
+      if (skn >= 0) { const size_t pn = (size_t)skn * g.PS + row; prefetch_l2(psz0 + pn); prefetch_l2(psz1 + pn); }
       if (!STAGED && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) {
         const float2 *Fn = Fsrc + (size_t)(k + 1 - g.blo[2]) * g.PS + row;
         const size_t cs = (size_t)g.NZB * g.PS;
