@@ -390,6 +390,35 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
+def run_converge(args):
+    """--converge: time to converged (BASELINE.json metric, third part) of the chosen workload through Grid.run, wall
+    clock, in the four DTFT schedules; one JSON line.  Not the driver's line (that is the default run)."""
+    import torch
+    from paper_2304_00233_b200 import emm
+    emm.build()
+    w = build_workload(args, emm.emm_nugrid)
+    g = emm.Grid(w["x"], w["y"], w["z"], **w["grid"])
+    g.bind(nsrc=1, nfreq=len(w["freqs"]), max_steps=60000, nrec=len(w["receivers"]), device="cuda:0")
+    g.model_set(w["sigma_h"], w.get("sigma_v"))
+    info = g.info()
+    N = info["N1"] * info["N2"] * info["N3"]
+    base = dict(w["run"])
+    base.pop("batched", None)
+    base["max_steps"] = 60000
+    g.run(w["sources"][:1], w["freqs"], w["receivers"], dict(fixed_steps=210))     # warm-up (plans, kernels, graph capture)
+    res = {}
+    for mode, extra in (("paired", {}), ("one_term_per_step", dict(dtft_pair=-1)), ("decimated_auto", dict(dtft_every=-1)),
+                        ("receivers_only", dict(sparse_dft=1))):
+        torch.cuda.synchronize()
+        t = time.perf_counter()
+        out, ns = g.run(w["sources"][:1], w["freqs"], w["receivers"], dict(base, **extra))
+        torch.cuda.synchronize()
+        el = time.perf_counter() - t
+        res[mode] = {"seconds": el, "steps": int(ns[0]), "gcell_updates_per_s": N * int(ns[0]) / el / 1e9,
+                     "largest_receiver_amplitude": float(np.abs(out).max())}
+    print(json.dumps({"metric": "time to converged", "config": describe(w, info, 1), "schedules": res}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -402,8 +431,11 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the cell counts (debugging only)")
     ap.add_argument("--aux-dx", type=float, default=0.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--converge", action="store_true", help="time to converged in the four DTFT schedules instead of the step benchmark")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.converge:
+        run_converge(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_gpu(args)
