@@ -225,6 +225,34 @@ def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle):
             assert (np.abs(o_p[s][..., sl] - o_s[s][..., sl])[big] / np.abs(ref)[big]).max() < 1e-5
 
 
+@pytest.mark.parametrize("rd", [1, 2, 3])
+def test_paired_dtft_every_instance(emm, rd):
+    """Every two-term instance k_update<rd, nf, ., PAIR>, nf = 1..5, against the one-term schedule on a small whole-space
+    grid (CPML on six faces), 41 steps in batches of 20 + 21: fields bit-identical, accumulators bit-identical away from
+    the injected nodes and within rounding there.  nf = 6 has no two-term instance: the option is ignored."""
+    w = W.cfg1(n=26, dx=100.0, rd=rd, nb=5)
+    freqs_all = np.array([0.25, 0.5, 0.75, 1.0, 1.25, 1.5])
+    for nf in range(1, 7):
+        ga, gs = make_grid(emm, w), make_grid(emm, w)
+        ga.run_begin(w["sources"], freqs_all[:nf], w["receivers"][:2], dict(fixed_steps=41))
+        gs.run_begin(w["sources"], freqs_all[:nf], w["receivers"][:2], dict(fixed_steps=41, dtft_pair=-1))
+        for n in (20, 21):
+            ga.run_steps(n)
+            gs.run_steps(n)
+        for c in FIELDS:
+            assert np.array_equal(ga.get(c), gs.get(c)), (rd, nf, c)
+            for f in (0, nf - 1):
+                Fa, Fs = ga.get("F_" + c, ifreq=f), gs.get("F_" + c, ifreq=f)
+                assert (Fa != Fs).sum() <= (0 if nf == 6 else max(2 * rd, 4) ** 3), (rd, nf, c, f)
+                assert np.abs(Fa - Fs).max() <= 1e-5 * max(np.abs(Fs).max(), 1e-30), (rd, nf, c, f)
+        assert np.abs(gs.get("F_E1", ifreq=nf - 1)).max() > 0
+        oa, _ = ga.run_end()
+        ob, _ = gs.run_end()
+        assert np.abs(oa - ob).max() <= 1e-5 * np.abs(ob).max()
+        ga.close()
+        gs.close()
+
+
 def test_plane_and_separable_air_routes_agree(emm, oracle, monkeypatch):
     """Non-uniform x-y: the separable route (batched 1-D transforms, default) and the plane-sized 2-D route
     (EMM_AIR_PLANE=1) are the same linear map up to rounding order; both are within the field tolerance of the oracle."""
