@@ -370,6 +370,16 @@ def run_gpu(args):
                     "step_frac_in_update_kernels": tot_update / (ms_prof * Kp),
                     "ms_per_step_serialised": ms_prof,
                     "how": "kernel_ms from a serialised pass (emm_profile); `value` is timed with the air-water boundary overlapped on a second stream"}
+        # whole step against the same peak: algorithmic bytes of the update kernels of one step (paired DTFT: half of the four
+        # passes of a pair), boundary / check-set / injection bytes not counted, over the timed ms per step
+        nfq, nbq = len(w["freqs"]), w["grid"]["nb"]
+        if "E2" in avg:
+            step_bytes = nsrc * sum(algorithmic_bytes(info, nfq, nbq, k) for k in ("E0", "H0", "E2", "H2")) / 2
+        else:
+            step_bytes = nsrc * (algorithmic_bytes(info, nfq, nbq, "E") + algorithmic_bytes(info, nfq, nbq, "H"))
+        roofline["whole_step"] = {"algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / (ms / K * 1e-3) / 1e9,
+                                  "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
+                                  "note": "update-kernel bytes only, over the whole timed step (boundary, check set and injection included in the time)"}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             v, cms, cores, desc = oracle_rate(w, 20.0, 3, 1, args)
