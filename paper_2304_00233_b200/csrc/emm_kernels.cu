@@ -304,15 +304,6 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       if (sj >= 0) { const size_t pn = ((size_t)(k + 1) * 2 * g.nb + sj) * g.P1 + i0; prefetch_l2(psy0 + pn); prefetch_l2(psy1 + pn); }
       const int skn = slab_of(k + 1, g.N3, g.nb, g.zslab_lo);
       if (skn >= 0) { const size_t pn = (size_t)skn * g.PS + row; prefetch_l2(psz0 + pn); prefetch_l2(psz1 + pn); }
-#ifdef EMM_PFACC
-      if (STAGED && dft_xy && k + EMM_PFACC >= g.blo[2] && k + EMM_PFACC <= g.bhi[2] && k + EMM_PFACC < kend) {
-        const float2 *Fn = Fsrc + (size_t)(k + EMM_PFACC - g.blo[2]) * g.PS + row;
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-          for (int f = 0; f < (NF > 0 ? NF : 0); ++f) prefetch_l2(Fn + c * cstride + f * fstride);
-      }
-#endif
       if (!STAGED && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) {
         const float2 *Fn = Fsrc + (size_t)(k + 1 - g.blo[2]) * g.PS + row;
         const size_t cs = (size_t)g.NZB * g.PS;
