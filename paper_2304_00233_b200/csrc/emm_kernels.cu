@@ -108,6 +108,9 @@ __device__ __forceinline__ void dtft4_rt(float2 *F0, size_t fstride, float4 u, c
 #ifndef EMM_PF
 #define EMM_PF 1
 #endif
+#ifndef EMM_CXS
+#define EMM_CXS 1   /* accumulator-free instance: x coefficients in private shared-memory slots instead of registers */
+#endif
 #ifndef EMM_HOIST
 #define EMM_HOIST 1
 #endif
@@ -220,11 +223,25 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   const float *ty = IS_H ? g.cp[1] : g.cm[1];
   const float *tz = IS_H ? g.cp[2] : g.cm[2];
 
+  // x coefficients of the thread's 4 nodes.  The accumulator-free instance (register-capped at 3 blocks per SM) parks them
+  // in private shared-memory slots and re-reads them where the x derivatives are formed (LDS.128, no bank conflicts:
+  // slot q of thread t at [q*128 + t]); that frees 8R registers for loads in flight.
+  constexpr bool CXS = (EMM_CXS != 0) && (NF == 0);
+  constexpr int NCX = (8 * R + 3) / 4;                 // float4 slots for 4 nodes x 2R coefficients
+  extern __shared__ float4 sm_dyn[];
+  float4 *smC = sm_dyn + (threadIdx.y * blockDim.x + threadIdx.x);
   float cx[4][2 * R], cy[2 * R];
+  if constexpr (CXS) {
+    static_assert((8 * R) % 4 == 0, "4 nodes x 2R coefficients fill whole float4 slots");
+    const float4 *src4 = reinterpret_cast<const float4 *>(tx + (size_t)i0 * 2 * R);    // 4 nodes x 2R floats, 16-byte aligned
 #pragma unroll
-  for (int n = 0; n < 4; ++n)
+    for (int q = 0; q < NCX; ++q) smC[q * 128] = __ldg(src4 + q);
+  } else {
 #pragma unroll
-    for (int m = 0; m < 2 * R; ++m) cx[n][m] = __ldg(tx + (size_t)(i0 + n) * 2 * R + m);
+    for (int n = 0; n < 4; ++n)
+#pragma unroll
+      for (int m = 0; m < 2 * R; ++m) cx[n][m] = __ldg(tx + (size_t)(i0 + n) * 2 * R + m);
+  }
 #pragma unroll
   for (int m = 0; m < 2 * R; ++m) cy[m] = __ldg(ty + (size_t)j * 2 * R + m);
 
@@ -273,8 +290,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 
   constexpr bool STAGED = (EMM_CPA != 0) && (NF > 0);
   static_assert(!PAIR || STAGED, "the paired DTFT instance needs staged accumulators");
-  extern __shared__ float4 smF_all[];
-  float4 *smF = smF_all + (threadIdx.y * blockDim.x + threadIdx.x);
+  float4 *smF = smC;                                   // DTFT instances: the dynamic shared memory holds the staged accumulators
   const size_t cstride = (size_t)g.NZB * g.PS;
   // The accumulators of the three components are three commit groups, consumed in issue order and re-issued for
   // the next plane as soon as their slots are free: every copy gets almost a whole plane of lead time, and
@@ -351,6 +367,13 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     float4 D1A3, D1A2;
     {
       float w[12];
+      if constexpr (CXS) {
+#pragma unroll
+        for (int q = 0; q < NCX; ++q) {
+          const float4 v = smC[q * 128];
+          (&cx[0][0])[4 * q] = v.x; (&cx[0][0])[4 * q + 1] = v.y; (&cx[0][0])[4 * q + 2] = v.z; (&cx[0][0])[4 * q + 3] = v.w;
+        }
+      }
       window(w, has_l ? ld4(A3 + c0 - 4) : zero4(), a3c, has_r ? ld4(A3 + c0 + 4) : zero4());
       D1A3 = ddx<R, O>(w, cx);
       window(w, has_l ? ld4(A2 + c0 - 4) : zero4(), a2c, has_r ? ld4(A2 + c0 + 4) : zero4());
@@ -639,7 +662,7 @@ static void launch_update_pair(const DevGrid &dg, const DevState &s, int nf, dim
 template <int R, bool IS_H>
 static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
   switch (nf) {
-    case 0: k_update<R, 0, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0, sel); break;
+    case 0: k_update<R, 0, IS_H><<<grid, block, EMM_CXS ? (size_t)2 * R * 128 * sizeof(float4) : 0, st>>>(dg, s, kc, nchunks, chunk0, sel); break;
     case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
     case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
     case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
