@@ -65,6 +65,8 @@ struct DevState {              // per run; arrays carry a leading source dimensi
   float *psy[2][2];            // y-slab psi [nsrc][N3][2nb][P1]
   float *psz[2][2];            // z-slab psi [nsrc][2nb][N2][P1]
   float2 *F;                   // [nsrc][nf][6][NZB][N2][P1]
+  float *hist[2][3];           // grouped DTFT: [E/H][component] copies of earlier time levels [nsrc][nslots][N3][N2][P1]
+  int nslots;                  // history slots per component (group size - 2; 0: none)
   const float2 *twE, *twH;     // [max_steps][nf]
   const float *wav;            // [max_steps] s(it dt): electric sources
   const float *wavh;           // [max_steps] s((it+1/2) dt): magnetic sources

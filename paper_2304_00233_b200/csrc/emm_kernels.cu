@@ -173,12 +173,27 @@ __device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0
 // Two consecutive terms of Eq. 25 in one read-modify-write of the accumulators (paired DTFT): the
 // update kernel holds the field before (uo) and after (un) its own update, i.e. the DTFT operands of two consecutive
 // steps.  F = fma(un, tb, fma(uo, ta, F)): the same two fused multiply-adds, in the same order, as two single-term passes.
+// kNHS: history levels a grouped-DTFT pass can take besides the old and the new field of its own update (group <= kNHS + 2)
+constexpr int kNHS = 2;
+// smh: the thread's staged history quads of this component (levels 0..nh-1, oldest first), twh: their twiddles
+// [nh][nf] in global memory (uniform loads).  Order of the fused multiply-adds = order of the terms in time.
 template <int NF>
 __device__ __forceinline__ void dtft4_staged2(const float4 *sm, int c, float2 *F0, size_t fstride, float4 uo, float4 un,
-                                              const float2 (&ta)[NF > 0 ? NF : 1], const float2 (&tb)[NF > 0 ? NF : 1]) {
+                                              const float2 (&ta)[NF > 0 ? NF : 1], const float2 (&tb)[NF > 0 ? NF : 1],
+                                              const float4 *smh, const float2 *__restrict__ twh, const int nh, const int nf) {
+  float4 uh[kNHS];
+#pragma unroll
+  for (int l = 0; l < kNHS; ++l) uh[l] = l < nh ? smh[l * 128] : zero4();
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
     float4 a0 = sm[((c * NF + f) * 2 + 0) * 128], a1 = sm[((c * NF + f) * 2 + 1) * 128];
+#pragma unroll
+    for (int l = 0; l < kNHS; ++l)
+      if (l < nh) {
+        const float2 t = __ldg(twh + l * nf + f);
+        a0.x = fmaf(uh[l].x, t.x, a0.x); a0.y = fmaf(uh[l].x, t.y, a0.y); a0.z = fmaf(uh[l].y, t.x, a0.z); a0.w = fmaf(uh[l].y, t.y, a0.w);
+        a1.x = fmaf(uh[l].z, t.x, a1.x); a1.y = fmaf(uh[l].z, t.y, a1.y); a1.z = fmaf(uh[l].w, t.x, a1.z); a1.w = fmaf(uh[l].w, t.y, a1.w);
+      }
     a0.x = fmaf(uo.x, ta[f].x, a0.x); a0.y = fmaf(uo.x, ta[f].y, a0.y); a0.z = fmaf(uo.y, ta[f].x, a0.z); a0.w = fmaf(uo.y, ta[f].y, a0.w);
     a1.x = fmaf(uo.z, ta[f].x, a1.x); a1.y = fmaf(uo.z, ta[f].y, a1.y); a1.z = fmaf(uo.w, ta[f].x, a1.z); a1.w = fmaf(uo.w, ta[f].y, a1.w);
     a0.x = fmaf(un.x, tb[f].x, a0.x); a0.y = fmaf(un.x, tb[f].y, a0.y); a0.z = fmaf(un.y, tb[f].x, a0.z); a0.w = fmaf(un.y, tb[f].y, a0.w);
@@ -197,7 +212,7 @@ template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_
 // PAIR: the two-term instance of the paired DTFT (NF >= 1, staged): the H kernel of step `it` takes the terms it and
 // it+1 of F_H (old and new H), the E kernel of step `it` the terms it-1 and it of F_E (old and new E) [R6].
 template <int R, int NF, bool IS_H, bool PAIR = false>
-__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0, const int sel) {
+__global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0, const int sel, const int harg) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
   const int src = blockIdx.z / nchunks, chunk = chunk0 + blockIdx.z - src * nchunks;   // this launch covers chunks [chunk0, chunk0 + nchunks)
   if (s.done[src]) return;
@@ -295,11 +310,30 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   // The accumulators of the three components are three commit groups, consumed in issue order and re-issued for
   // the next plane as soon as their slots are free: every copy gets almost a whole plane of lead time, and
   // `cp.async.wait_group 2` before each use leaves exactly the two younger groups pending.
+  // Grouped DTFT.  harg: PAIR instance = number nh of history levels it takes besides its own old
+  // and new field (their quads are staged with the accumulators of the component, slots behind them); accumulator-free
+  // instance = history slot into which this step's field is copied for the pass that closes the group (-1: none).
+  const int nh = PAIR ? harg : 0;
+  const float *hs[3] = {nullptr, nullptr, nullptr};
+  if (PAIR || (NF == 0 && harg >= 0)) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) hs[c] = s.hist[IS_H ? 1 : 0][c] + ((size_t)src * s.nslots + (PAIR ? 0 : harg)) * g.VS;
+  }
+  constexpr int HB = 3 * (NF > 0 ? NF : 0) * 2;        // first history slot in shared memory
+  auto stage_history = [&](int c, int k) {
+    if constexpr (PAIR) {
+#pragma unroll
+      for (int l = 0; l < kNHS; ++l)
+        if (l < nh) cp_async16(smF + (HB + c * kNHS + l) * 128, hs[c] + (size_t)l * g.VS + (size_t)k * g.PS + row);
+    }
+  };
   if constexpr (STAGED) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      if (dft_xy && kbeg >= g.blo[2] && kbeg <= g.bhi[2])
+      if (dft_xy && kbeg >= g.blo[2] && kbeg <= g.bhi[2]) {
         stage_component<NF>(smF, c, Fsrc + (size_t)(kbeg - g.blo[2]) * g.PS + row + c * cstride, fstride);
+        stage_history(c, kbeg);
+      }
       cp_async_commit();
     }
   }
@@ -422,11 +456,13 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     auto dtft_staged_component = [&](int c, float4 u, float4 un = zero4()) {
       cp_async_wait_2();
       if (dft) {
-        if constexpr (PAIR) dtft4_staged2<NF>(smF, c, Fk + c * cstride, fstride, u, un, tw, tw2);
+        if constexpr (PAIR) dtft4_staged2<NF>(smF, c, Fk + c * cstride, fstride, u, un, tw, tw2, smF + (HB + c * kNHS) * 128, twp - (size_t)nh * nf, nh, nf);
         else dtft4_staged<NF>(smF, c, Fk + c * cstride, fstride, u, tw);
       }
-      if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2])
+      if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) {
         stage_component<NF>(smF, c, Fk + g.PS + c * cstride, fstride);
+        stage_history(c, k + 1);
+      }
       cp_async_commit();
     };
 
@@ -444,6 +480,9 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u2 = make_float4(fmaf(-m0, c2.x, u2.x), fmaf(-m1, c2.y, u2.y), fmaf(-m2, c2.z, u2.z), fmaf(-m3, c2.w, u2.w));
       u3 = make_float4(fmaf(-m0, c3.x, u3.x), fmaf(-m1, c3.y, u3.y), fmaf(-m2, c3.z, u3.z), fmaf(-m3, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
+      if (NF == 0 && harg >= 0) {      // H^{it} (before this update) is term `it` of the group this step belongs to
+        stcs4(const_cast<float *>(hs[0]) + c0, o1); stcs4(const_cast<float *>(hs[1]) + c0, o2); stcs4(const_cast<float *>(hs[2]) + c0, o3);
+      }
       // PAIR: old H is term it, new H is term it+1 (the old H of the next step)
       if constexpr (PAIR) { dtft_staged_component(0, o1, u1); dtft_staged_component(1, o2, u2); dtft_staged_component(2, o3, u3); }
     } else {
@@ -451,6 +490,9 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
+      if (NF == 0 && harg >= 0) {      // E^{it+1/2} (after this update, injection included) is term `it`
+        stcs4(const_cast<float *>(hs[0]) + c0, u1); stcs4(const_cast<float *>(hs[1]) + c0, u2); stcs4(const_cast<float *>(hs[2]) + c0, u3);
+      }
       // new E sits at t = (it+1/2)*dt [R6]; PAIR: old E is term it-1, new E is term it
       if constexpr (PAIR) { dtft_staged_component(0, o1, u1); dtft_staged_component(1, o2, u2); dtft_staged_component(2, o3, u3); }
       else if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }
@@ -635,40 +677,40 @@ __global__ void k_rec_interp(const DevGrid g, const DevState s, const int *__res
 
 // unrolled-NF instantiations stage one plane of accumulators per thread in dynamic shared memory
 template <int R, int NF, bool IS_H, bool PAIR = false>
-static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
-  const size_t smem = EMM_CPA ? (size_t)3 * NF * 2 * 128 * sizeof(float4) : 0;
+static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel, int harg) {
+  const size_t smem = EMM_CPA ? (size_t)(3 * NF * 2 + (PAIR ? 3 * kNHS : 0)) * 128 * sizeof(float4) : 0;
   static bool configured = false;
   if (!configured && smem > 48 * 1024) {
     cudaFuncSetAttribute(k_update<R, NF, IS_H, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
-  k_update<R, NF, IS_H, PAIR><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel);
+  k_update<R, NF, IS_H, PAIR><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel, harg);
 }
 
 #if EMM_CPA
 // two-term instances of the paired DTFT (1..kPairMaxNF frequencies)
 template <int R, bool IS_H>
-static void launch_update_pair(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0) {
+static void launch_update_pair(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int harg) {
   switch (nf) {
-    case 1: launch_one<R, 1, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
-    case 2: launch_one<R, 2, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
-    case 3: launch_one<R, 3, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
-    case 4: launch_one<R, 4, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
-    default: launch_one<R, 5, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0); break;
+    case 1: launch_one<R, 1, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0, harg); break;
+    case 2: launch_one<R, 2, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0, harg); break;
+    case 3: launch_one<R, 3, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0, harg); break;
+    case 4: launch_one<R, 4, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0, harg); break;
+    default: launch_one<R, 5, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0, harg); break;
   }
 }
 #endif
 
 template <int R, bool IS_H>
-static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel) {
+static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel, int harg) {
   switch (nf) {
-    case 0: k_update<R, 0, IS_H><<<grid, block, EMM_CXS ? (size_t)2 * R * 128 * sizeof(float4) : 0, st>>>(dg, s, kc, nchunks, chunk0, sel); break;
-    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
-    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
-    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
-    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
-    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel); break;
-    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0, sel); break;
+    case 0: k_update<R, 0, IS_H><<<grid, block, EMM_CXS ? (size_t)2 * R * 128 * sizeof(float4) : 0, st>>>(dg, s, kc, nchunks, chunk0, sel, harg); break;
+    case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
+    case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
+    case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
+    case 4: launch_one<R, 4, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
+    case 5: launch_one<R, 5, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
+    default: k_update<R, -1, IS_H><<<grid, block, 0, st>>>(dg, s, kc, nchunks, chunk0, sel, harg); break;
   }
 }
 
@@ -676,7 +718,8 @@ static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 
 // 2 = all the others.  Parts 1 and 2 can run on different streams (emm_run.cu overlaps the boundary with part 2).
 // mode: 0 = one DTFT term per step (and DTFT decimation); paired DTFT: 1 = the step in which this kernel takes no
 // term (accumulator-free instance), 2 = the step in which it takes two (PAIR instance)
-int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, cudaStream_t st) {
+// harg: mode 1 = history slot this step's field is copied into (-1: none); mode 2 = history levels the pass takes
+int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st) {
   const DevGrid &dg = g->dg;
   const int quads = dg.P1 / 4;
   const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
@@ -713,25 +756,25 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
     if (pair) {
 #if EMM_CPA
       if (is_h) {
-        if (dg.r == 1) launch_update_pair<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
-        else if (dg.r == 2) launch_update_pair<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
-        else launch_update_pair<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+        if (dg.r == 1) launch_update_pair<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
+        else if (dg.r == 2) launch_update_pair<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
+        else launch_update_pair<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
       } else {
-        if (dg.r == 1) launch_update_pair<1, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
-        else if (dg.r == 2) launch_update_pair<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
-        else launch_update_pair<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0);
+        if (dg.r == 1) launch_update_pair<1, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
+        else if (dg.r == 2) launch_update_pair<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
+        else launch_update_pair<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
       }
 #else
       return fail(EMM_EINVAL, "launch_update: paired DTFT needs the staged accumulators (EMM_CPA)");
 #endif
     } else if (is_h) {
-      if (dg.r == 1) launch_update_nf<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
-      else if (dg.r == 2) launch_update_nf<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
-      else launch_update_nf<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+      if (dg.r == 1) launch_update_nf<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
+      else if (dg.r == 2) launch_update_nf<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
+      else launch_update_nf<3, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
     } else {
-      if (dg.r == 1) launch_update_nf<1, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
-      else if (dg.r == 2) launch_update_nf<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
-      else launch_update_nf<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel);
+      if (dg.r == 1) launch_update_nf<1, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
+      else if (dg.r == 2) launch_update_nf<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
+      else launch_update_nf<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
     }
     EMM_LAUNCH_CHECK(g, is_h ? "k_update<H>" : "k_update<E>");
     return 0;

@@ -38,8 +38,10 @@ struct DevRun {
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
 // mode: 0 = one DTFT term per step; paired DTFT: 1 = accumulator-free step of this kernel, 2 = its two-term step
-int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, cudaStream_t st);
-constexpr int kPairMaxNF = 5;       // two-term instances exist for 1..5 frequencies (the staged, unrolled ones)
+// harg: mode 1 = history slot the step's field is copied into (-1 none), mode 2 = number of history levels taken
+int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st);
+constexpr int kPairMaxNF = 5;       // grouped-DTFT instances exist for 1..5 frequencies (the staged, unrolled ones)
+constexpr int kGroupMax = 4;        // largest DTFT group (terms per accumulator pass): 2 history levels + old + new
 // pairfix: also add the product the two-term kernel misses at the injected nodes (see k_inject)
 int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic, int pairfix);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);

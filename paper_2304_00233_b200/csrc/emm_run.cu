@@ -20,7 +20,7 @@ struct Run {
   int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
   int it_min = 0, it_host = 0, table_steps = 0, dtft_every = 1;
   bool sparse = false;                   // receivers-only DTFT (emm_run_opts.sparse_dft)
-  bool pair = false;                     // paired DTFT: two consecutive terms of Eq. 25 per accumulator pass (emm_run_opts.dtft_pair)
+  int group = 1;                         // grouped DTFT: terms of Eq. 25 per accumulator pass (emm_run_opts.dtft_pair); 1 = one per step
   std::vector<double> wav, wavh;            // s(it dt), s((it+1/2) dt) rounded to fp32 (what the device injects)
   std::vector<int> mag;                     // [nsrc] 1 = magnetic dipole
   bool any_mag = false, any_el = false;
@@ -110,7 +110,7 @@ static size_t chk_count(const emm_grid *g, int check_set) {
 
 // per-run region
 // nf = frequencies with full-grid accumulators, nf_rec = frequencies kept at the receiver stencils only (one of the two is 0)
-static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int table_steps, int nrec, size_t nchk, DevState &s, DevRun &r) {
+static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int table_steps, int nrec, size_t nchk, int nslots, DevState &s, DevRun &r) {
   const size_t V = vol(g), PS = (size_t)g->P1 * g->N[1];
   const int np = std::max(2 * g->r, 4);
   const size_t np3 = (size_t)np * np * np;
@@ -123,6 +123,9 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
     }
   const size_t nzb = g->bhi[2] - g->blo[2] + 1;
   s.F = A.take<float2>((size_t)nsrc * nf * 6 * nzb * PS);
+  s.nslots = nslots;
+  for (int k = 0; k < 2; ++k)
+    for (int c = 0; c < 3; ++c) s.hist[k][c] = nslots > 0 ? A.take<float>((size_t)nsrc * nslots * V) : nullptr;
   s.twE = A.take<float2>((size_t)table_steps * nf);
   s.twH = A.take<float2>((size_t)table_steps * nf);
   s.wav = A.take<float>(table_steps);
@@ -205,7 +208,8 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   const size_t fixed = A.off;
   DevState s{};
   DevRun r{};
-  layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), s, r);   // the full-grid mode is the larger one
+  layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES),
+             nfreq >= 1 && nfreq <= kPairMaxNF ? kGroupMax - 2 : 0, s, r);                           // the full-grid mode with the largest DTFT group is the larger one
   g->T = keep;
   return std::max(A.off, fixed + 1024) + 4096;       // emm_model_set keeps a few scalars behind the per-grid region
 }
@@ -404,6 +408,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
   Run *R = g->run;
   int rc;
   static const bool no_overlap = getenv("EMM_NO_OVERLAP") != nullptr;
+  int gpos = 0, gsize = 0;                   // grouped DTFT: position in / size of the current group of steps
   for (int q = 0; q < n; ++q) {
     if (R->it_host >= R->table_steps) return fail(EMM_EINVAL, "run: step %d beyond the twiddle table (max_steps)", R->it_host);
     cudaStream_t M = g->stream, B = g->stream_b;
@@ -411,26 +416,39 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
     // it and it+1 of F_H (old and new H) and the E kernel none; in the second the E kernel adds the terms it-1 and it of
     // F_E (old and new E) and the H kernel none; a left-over last step takes its single terms as usual.  A batch never
     // crosses a convergence check (enqueue_steps), so every sum is complete where it is read.
-    int me = 0, mh = 0;
-    if (R->pair) {
-      if (q & 1) { me = 2; mh = 1; }
-      else if (q + 1 < n && R->it_host + 1 < R->table_steps) { me = 1; mh = 2; }
+    int me = 0, mh = 0, he = -1, hh = -1;
+    if (R->group > 1) {
+      if (gpos >= gsize) {                   // open the next group of this batch: up to `group` steps, at least 2
+        gpos = 0;
+        gsize = std::min(std::min(R->group, n - q), R->table_steps - R->it_host);
+        if (gsize < 2) gsize = 1;
+      }
+      if (gsize >= 2) {
+        // position p of a group of m steps.  E kernel: copies its new field into history slot p (p <= m-3), nothing
+        // extra at p = m-2 (that level is the old field of the closing pass), closes the group at p = m-1 with m terms.
+        // H kernel: copies its old field into slot p (p <= m-3), closes the group at p = m-2 (old H = term m-2, new H =
+        // term m-1), nothing at p = m-1.  m = 2: the pair of two-term passes.
+        const int m = gsize, p = gpos;
+        if (p == m - 1) { me = 2; he = m - 2; } else { me = 1; he = p <= m - 3 ? p : -1; }
+        if (p == m - 2) { mh = 2; hh = m - 2; } else { mh = 1; hh = p <= m - 3 ? p : -1; }
+      }
+      ++gpos;
     }
     if (R->any_el && (rc = launch_inject(g, R->ds, R->dr, 0, me == 2))) return rc;     // Alg. 1 L477 (before the update: same sum)
     if (g->top != EMM_TOP_AIR) {
-      if ((rc = launch_update(g, R->ds, 0, 0, me, M))) return rc;                 // L476-479 + E part of L483
+      if ((rc = launch_update(g, R->ds, 0, 0, me, he, M))) return rc;                 // L476-479 + E part of L483
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                // check-set part of L483
       if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_update(g, R->ds, 1, 0, mh, M))) return rc;                 // H part of L483 + L486-489
+      if ((rc = launch_update(g, R->ds, 1, 0, mh, hh, M))) return rc;                 // H part of L483 + L486-489
     } else if (g->prof || no_overlap) {
       // one thing after the other (per-kernel timing, or EMM_NO_OVERLAP): the boundary still runs on its own stream
-      if ((rc = launch_update(g, R->ds, 0, 0, me, M))) return rc;
+      if ((rc = launch_update(g, R->ds, 0, 0, me, he, M))) return rc;
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));
       if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
       CU(cudaEventRecord(g->ev[1], B)); CU(cudaStreamWaitEvent(M, g->ev[1], 0));
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
       if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_update(g, R->ds, 1, 0, mh, M))) return rc;
+      if ((rc = launch_update(g, R->ds, 1, 0, mh, hh, M))) return rc;
       CU(cudaEventRecord(g->ev[2], M)); CU(cudaStreamWaitEvent(B, g->ev[2], 0));
       if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));
@@ -438,18 +456,18 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       // The boundary only feeds the z chunks next to the surface: those chunks and the FFT boundary form a short
       // chain on the helper stream while the bulk of the grid is updated on the main stream (fork/join per step).
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));      // fork (after the injection)
-      if ((rc = launch_update(g, R->ds, 0, 1, me, B))) return rc;                 // E, surface chunks
+      if ((rc = launch_update(g, R->ds, 0, 1, me, he, B))) return rc;                 // E, surface chunks
       CU(cudaEventRecord(g->ev[1], B));
       if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
-      if ((rc = launch_update(g, R->ds, 0, 2, me, M))) return rc;                 // E, bulk
+      if ((rc = launch_update(g, R->ds, 0, 2, me, he, M))) return rc;                 // E, bulk
       CU(cudaEventRecord(g->ev[2], M));
       CU(cudaStreamWaitEvent(M, g->ev[1], 0));                                // H bulk and the check set read surface-chunk E
       if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
       if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
       CU(cudaEventRecord(g->ev[4], M));
-      if ((rc = launch_update(g, R->ds, 1, 2, mh, M))) return rc;                 // H, bulk
+      if ((rc = launch_update(g, R->ds, 1, 2, mh, hh, M))) return rc;                 // H, bulk
       CU(cudaStreamWaitEvent(B, g->ev[2], 0)); CU(cudaStreamWaitEvent(B, g->ev[4], 0));
-      if ((rc = launch_update(g, R->ds, 1, 1, mh, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
+      if ((rc = launch_update(g, R->ds, 1, 1, mh, hh, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
       if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));      // join
     }
@@ -546,7 +564,10 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     R->sparse = o->sparse_dft != 0 && nf > 0;
     {
       static const bool no_pair = getenv("EMM_NO_PAIR") != nullptr;       // A/B measurements
-      R->pair = o->dtft_pair >= 0 && !no_pair && nf >= 1 && nf <= kPairMaxNF && !R->sparse && o->dtft_every >= 0 && o->dtft_every <= 1;
+      const bool can = o->dtft_pair >= 0 && !no_pair && nf >= 1 && nf <= kPairMaxNF && !R->sparse && o->dtft_every >= 0 && o->dtft_every <= 1;
+      static const char *env_group = getenv("EMM_DTFT_GROUP");             // A/B measurements: default group size
+      const int dflt = env_group && atoi(env_group) >= 2 ? atoi(env_group) : kGroupMax;
+      R->group = !can ? 1 : std::min(kGroupMax, o->dtft_pair >= 2 ? o->dtft_pair : dflt);
     }
     if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
     R->table_steps = (R->fixed_steps ? R->fixed_steps : R->max_steps) + 1;
@@ -604,7 +625,13 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     if (g->top == EMM_TOP_AIR && g->sep_air && (rc = sep_air_make_plans(g, nsrc))) { free_run(g); return rc; }
     Arena A;
     A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
-    layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), R->ds, R->dr);
+    layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), R->group > 2 ? R->group - 2 : 0, R->ds, R->dr);
+    if (A.overflow && R->group > 2) {        // a workspace sized by an older rule: fall back to pairs (no history copies)
+      R->group = 2;
+      A.off = g->fixed_bytes;
+      A.overflow = false;
+      layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), 0, R->ds, R->dr);
+    }
     if (g->top == EMM_TOP_AIR && g->sep_air && !A.overflow)
       for (int q = 0; q < 8; ++q)
         if (g->sp[q] && (cufftSetStream(g->sp[q], g->stream_b) != CUFFT_SUCCESS || cufftSetWorkArea(g->sp[q], R->dr.sp_ws[q]) != CUFFT_SUCCESS)) {
