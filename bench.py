@@ -57,17 +57,24 @@ def describe(w, info, nsrc):
         "l2": "working set (fields + DTFT accumulators) is >> the 126 MB L2; no flush needed"}
 
 
-def algorithmic_bytes(info, nf, nb, kernel):
+def algorithmic_bytes(info, nf, nb, kernel, m=1):
     """E kernel reads 3 H, RMWs 3 E, reads 3 dt/eps = 48 B/node; H kernel reads 3 E, RMWs 3 H
     = 36 B/node; each RMWs 3*nf complex accumulators (48*nf B) per DTFT-box node; plus 8 B per active CPML
-    memory variable (two per slab membership)."""
+    memory variable (two per slab membership).  Grouped DTFT with m terms per accumulator pass:
+    the closing pass of a group ("E2"/"H2") also reads m-2 earlier levels of its 3 components (12 B per box node each);
+    of the m-1 accumulator-free passes of a group ("E0"/"H0") m-2 write such a copy: the average is charged."""
     N1, N2, N3 = info["N1"], info["N2"], info["N3"]
     N = N1 * N2 * N3
     box = ((info["box_hi1"] - info["box_lo1"] + 1) * (info["box_hi2"] - info["box_lo2"] + 1)
            * (info["box_hi3"] - info["box_lo3"] + 1))
     zs = (2 if info["k0"] < 0 else 1) * nb
     psi = 16 * (2 * nb * N2 * N3 + 2 * nb * N1 * N3 + zs * N1 * N2)
-    return (48 if kernel[0] == "E" else 36) * N + 48 * (0 if kernel[1:] == "0" else nf) * box + psi
+    b = (48 if kernel[0] == "E" else 36) * N + 48 * (0 if kernel[1:] == "0" else nf) * box + psi
+    if kernel[1:] == "2":
+        b += 12 * max(m - 2, 0) * box
+    if kernel[1:] == "0" and m > 2:
+        b += 12 * box * (m - 2) / (m - 1)
+    return b
 
 
 class ClockSampler:
@@ -243,6 +250,7 @@ def run_gpu(args):
 
     # ---- device-resident stepping: K steps timed with CUDA events on the library's stream ----
     g.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=K + Wm + 4, batched=1 if nsrc > 1 else 0))
+    dtft_group = int(g.get("DTFT_GROUP")[0])
     g.run_enqueue(Wm)
     torch.cuda.synchronize()
     if world > 1:
@@ -351,11 +359,12 @@ def run_gpu(args):
         # instances of the update kernel in this run (paired DTFT: E0/H0 = accumulator-free steps, E2/H2 = two-term steps);
         # the dominant one = the largest duration per launch
         avg = {k: v[0] / v[1] for k, v in prof.items() if v[1] > 0}
+        mgrp = dtft_group
         dom = max(avg, key=avg.get)
         kms = avg[dom]
         inst = {"E": "k_update<R,NF,E>", "H": "k_update<R,NF,H>", "E0": "k_update<R,0,E>", "H0": "k_update<R,0,H>",
-                "E2": "k_update<R,NF,E,PAIR>", "H2": "k_update<R,NF,H,PAIR>"}
-        abytes = nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], dom)
+                "E2": "k_update<R,NF,E,PAIR> (closing pass of a DTFT group)", "H2": "k_update<R,NF,H,PAIR> (closing pass of a DTFT group)"}
+        abytes = nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], dom, mgrp)
         achieved = abytes / (kms * 1e-3) / 1e9
         traffic = None
         tf = os.path.join(ROOT, "profiles", "ncu_traffic.json")
@@ -365,7 +374,8 @@ def run_gpu(args):
         roofline = {"bound": "hbm", "kernel": inst[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "algorithmic_bytes_per_launch": abytes,
                     "kernel_ms": kms, "kernels_ms_per_launch": avg,
-                    "instances_gbs": {k: nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], k) / (avg[k] * 1e-3) / 1e9 for k in avg},
+                    "instances_gbs": {k: nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], k, mgrp) / (avg[k] * 1e-3) / 1e9 for k in avg},
+                    "dtft_group": mgrp,
                     "update_kernels_ms_per_step": tot_update / Kp,
                     "step_frac_in_update_kernels": tot_update / (ms_prof * Kp),
                     "ms_per_step_serialised": ms_prof,
@@ -373,8 +383,9 @@ def run_gpu(args):
         # whole step against the same peak: algorithmic bytes of the update kernels of one step (paired DTFT: half of the four
         # passes of a pair), boundary / check-set / injection bytes not counted, over the timed ms per step
         nfq, nbq = len(w["freqs"]), w["grid"]["nb"]
-        if "E2" in avg:
-            step_bytes = nsrc * sum(algorithmic_bytes(info, nfq, nbq, k) for k in ("E0", "H0", "E2", "H2")) / 2
+        if "E2" in avg:      # a group of m steps: m-1 accumulator-free passes and one closing pass per kernel
+            step_bytes = nsrc * sum((mgrp - 1) * algorithmic_bytes(info, nfq, nbq, k + "0", mgrp) + algorithmic_bytes(info, nfq, nbq, k + "2", mgrp)
+                                    for k in ("E", "H")) / mgrp
         else:
             step_bytes = nsrc * (algorithmic_bytes(info, nfq, nbq, "E") + algorithmic_bytes(info, nfq, nbq, "H"))
         roofline["whole_step"] = {"algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / (ms / K * 1e-3) / 1e9,
@@ -392,7 +403,7 @@ def run_gpu(args):
                         "d2h_bytes_per_step": d2h / K, "seconds": t_e2e,
                         "what": "emm_model_set (host sigma -> device) + emm_run(fixed_steps=K) (tables up, receivers back)"},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched,
-                "dtft": "every term of Eq. 25, two consecutive terms per accumulator pass (emm_run_opts.dtft_pair, default)" if unpaired else "every term of Eq. 25, one per step",
+                "dtft": ("every term of Eq. 25, %d consecutive terms per accumulator pass (emm_run_opts.dtft_pair, default)" % dtft_group) if dtft_group > 1 else "every term of Eq. 25, one per step",
                 "dtft_one_term_per_step": unpaired, "dtft_decimation": decim, "receivers_only_dtft": rec_only,
                 "multi_gpu": "replicas only: every rank runs the whole workload, no collective on the data path"}
         print(json.dumps(line))
@@ -402,7 +413,7 @@ def run_gpu(args):
 
 def run_converge(args):
     """--converge: time to converged (BASELINE.json metric, third part) of the chosen workload through Grid.run, wall
-    clock, in the four DTFT schedules; one JSON line.  Not the driver's line (that is the default run)."""
+    clock, in the five DTFT schedules; one JSON line.  Not the driver's line (that is the default run)."""
     import torch
     from paper_2304_00233_b200 import emm
     emm.build()
@@ -417,7 +428,7 @@ def run_converge(args):
     base["max_steps"] = 60000
     g.run(w["sources"][:1], w["freqs"], w["receivers"], dict(fixed_steps=210))     # warm-up (plans, kernels, graph capture)
     res = {}
-    for mode, extra in (("paired", {}), ("one_term_per_step", dict(dtft_pair=-1)), ("decimated_auto", dict(dtft_every=-1)),
+    for mode, extra in (("grouped_default", {}), ("pairs", dict(dtft_pair=2)), ("one_term_per_step", dict(dtft_pair=-1)), ("decimated_auto", dict(dtft_every=-1)),
                         ("receivers_only", dict(sparse_dft=1))):
         torch.cuda.synchronize()
         t = time.perf_counter()

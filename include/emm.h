@@ -79,16 +79,18 @@ typedef struct {
                       run without the 96*nf B/node term.  Same sums at those nodes, so emm_run returns the same
                       Green's functions and step counts; for runs that only want receiver data.
                       0: accumulators for every frequency on the whole DTFT box, as the paper does (L454)            */
-  int dtft_pair;   /* Paired DTFT (default, 0): every term of Eq. 25 is taken, two consecutive terms per read-modify-write
-                      of the accumulators.  An update kernel holds the field before and after its own update, i.e. the
-                      DTFT operands of two consecutive steps (L372: old H of steps it and it+1; new E of steps it-1 and
-                      it), so the steps are taken two by two: the H kernel adds both H terms in the first step, the E
-                      kernel both E terms in the second; each accumulator gets the same fused multiply-adds in the same
-                      order as with one term per step, at half the 96*nf B/node traffic.  Pairs never cross a convergence
-                      check or the end of an emm_run_steps/emm_run_enqueue batch (a left-over step takes single terms),
-                      so accumulators are complete whenever they can be read.  Applies to 1..5 frequencies with full-grid
-                      accumulators and dtft_every <= 1; otherwise ignored.  -1: one term per step in every step, as the
-                      paper's kernels do (L454, L880-884)                                                            */
+  int dtft_pair;   /* Grouped DTFT: every term of Eq. 25 is taken, m consecutive terms per read-modify-write of the
+                      accumulators.  An update kernel holds the field before and after its own update, i.e. the DTFT
+                      operands of two consecutive steps (L372: old H of steps it and it+1; new E of steps it-1 and it);
+                      the m-2 earlier levels of a group are copied by the accumulator-free passes of the steps before
+                      (12 B/node each) and read back by the pass that closes the group.  Each accumulator gets the same
+                      fused multiply-adds in the same order as with one term per step, at 1/m of the 96*nf B/node
+                      traffic.  Groups never cross a convergence check or the end of an emm_run_steps/emm_run_enqueue
+                      batch (shorter groups and single steps fill the rest), so accumulators are complete whenever they
+                      can be read.  Applies to 1..5 frequencies with full-grid accumulators and dtft_every <= 1; otherwise
+                      ignored.  0: default m (8 with 4-5 frequencies, 6 with 1-3); 2..8: that m (2 = pairs, no copies);
+                      -1: one term per step in every step, as the paper's kernels do (L454, L880-884).  The workspace
+                      holds (m-2)*6 field-sized arrays per source for the copies.                                    */
 } emm_run_opts;
 
 /* integer grid facts for emm_grid_info(): */
@@ -110,8 +112,9 @@ enum { EMM_GET_E1 = 0, EMM_GET_E2, EMM_GET_E3, EMM_GET_H1, EMM_GET_H2, EMM_GET_H
                                       frequency `ifreq` (Eq. 25), zero outside the DTFT box              */
        EMM_GET_CE1 = 20, EMM_GET_CE2, EMM_GET_CE3, /* float [N3][N2][N1]: dt/eps of each E component   */
        EMM_GET_JW = 30,            /* double complex [nfreq]: J'(omega') accumulated so far (Eq. 7)     */
-       EMM_GET_DELTA = 31          /* double [2]: relative change of E and H accumulators at the last
+       EMM_GET_DELTA = 31,         /* double [2]: relative change of E and H accumulators at the last
                                       convergence check                                                  */
+       EMM_GET_DTFT_GROUP = 32     /* int: terms of Eq. 25 per accumulator pass in this run (1, or the m of dtft_pair) */
 };
 
 /* ---- host-side pieces of the method (also the diagnostic surface) ------------------------------- */

@@ -174,7 +174,7 @@ __device__ __forceinline__ void dtft4_staged(const float4 *sm, int c, float2 *F0
 // update kernel holds the field before (uo) and after (un) its own update, i.e. the DTFT operands of two consecutive
 // steps.  F = fma(un, tb, fma(uo, ta, F)): the same two fused multiply-adds, in the same order, as two single-term passes.
 // kNHS: history levels a grouped-DTFT pass can take besides the old and the new field of its own update (group <= kNHS + 2)
-constexpr int kNHS = 2;
+constexpr int kNHS = kGroupMax - 2;
 // smh: the thread's staged history quads of this component (levels 0..nh-1, oldest first), twh: their twiddles
 // [nh][nf] in global memory (uniform loads).  Order of the fused multiply-adds = order of the terms in time.
 template <int NF>
@@ -314,6 +314,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   // and new field (their quads are staged with the accumulators of the component, slots behind them); accumulator-free
   // instance = history slot into which this step's field is copied for the pass that closes the group (-1: none).
   const int nh = PAIR ? harg : 0;
+  const bool hist_xy = (NF == 0) && harg >= 0 && (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);   // copies are read inside the DTFT box only
   const float *hs[3] = {nullptr, nullptr, nullptr};
   if (PAIR || (NF == 0 && harg >= 0)) {
 #pragma unroll
@@ -324,7 +325,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     if constexpr (PAIR) {
 #pragma unroll
       for (int l = 0; l < kNHS; ++l)
-        if (l < nh) cp_async16(smF + (HB + c * kNHS + l) * 128, hs[c] + (size_t)l * g.VS + (size_t)k * g.PS + row);
+        if (l < nh) cp_async16(smF + (HB + c * nh + l) * 128, hs[c] + (size_t)l * g.VS + (size_t)k * g.PS + row);
     }
   };
   if constexpr (STAGED) {
@@ -456,7 +457,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     auto dtft_staged_component = [&](int c, float4 u, float4 un = zero4()) {
       cp_async_wait_2();
       if (dft) {
-        if constexpr (PAIR) dtft4_staged2<NF>(smF, c, Fk + c * cstride, fstride, u, un, tw, tw2, smF + (HB + c * kNHS) * 128, twp - (size_t)nh * nf, nh, nf);
+        if constexpr (PAIR) dtft4_staged2<NF>(smF, c, Fk + c * cstride, fstride, u, un, tw, tw2, smF + (HB + c * nh) * 128, twp - (size_t)nh * nf, nh, nf);
         else dtft4_staged<NF>(smF, c, Fk + c * cstride, fstride, u, tw);
       }
       if (k + 1 < kend && dft_xy && k + 1 >= g.blo[2] && k + 1 <= g.bhi[2]) {
@@ -480,7 +481,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u2 = make_float4(fmaf(-m0, c2.x, u2.x), fmaf(-m1, c2.y, u2.y), fmaf(-m2, c2.z, u2.z), fmaf(-m3, c2.w, u2.w));
       u3 = make_float4(fmaf(-m0, c3.x, u3.x), fmaf(-m1, c3.y, u3.y), fmaf(-m2, c3.z, u3.z), fmaf(-m3, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
-      if (NF == 0 && harg >= 0) {      // H^{it} (before this update) is term `it` of the group this step belongs to
+      if (hist_xy && k >= g.blo[2] && k <= g.bhi[2]) {      // H^{it} (before this update) is term `it` of the group this step belongs to
         stcs4(const_cast<float *>(hs[0]) + c0, o1); stcs4(const_cast<float *>(hs[1]) + c0, o2); stcs4(const_cast<float *>(hs[2]) + c0, o3);
       }
       // PAIR: old H is term it, new H is term it+1 (the old H of the next step)
@@ -490,7 +491,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
       st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
-      if (NF == 0 && harg >= 0) {      // E^{it+1/2} (after this update, injection included) is term `it`
+      if (hist_xy && k >= g.blo[2] && k <= g.bhi[2]) {      // E^{it+1/2} (after this update, injection included) is term `it`
         stcs4(const_cast<float *>(hs[0]) + c0, u1); stcs4(const_cast<float *>(hs[1]) + c0, u2); stcs4(const_cast<float *>(hs[2]) + c0, u3);
       }
       // new E sits at t = (it+1/2)*dt [R6]; PAIR: old E is term it-1, new E is term it
@@ -678,10 +679,13 @@ __global__ void k_rec_interp(const DevGrid g, const DevState s, const int *__res
 // unrolled-NF instantiations stage one plane of accumulators per thread in dynamic shared memory
 template <int R, int NF, bool IS_H, bool PAIR = false>
 static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel, int harg) {
-  const size_t smem = EMM_CPA ? (size_t)(3 * NF * 2 + (PAIR ? 3 * kNHS : 0)) * 128 * sizeof(float4) : 0;
+  // staged accumulators + (grouped DTFT) the history quads of the levels this pass takes: sized per launch, so that a
+  // small group does not pay shared memory (= L1) for the largest one
+  const size_t smem = EMM_CPA ? (size_t)(3 * NF * 2 + (PAIR ? 3 * harg : 0)) * 128 * sizeof(float4) : 0;
+  const size_t smem_max = EMM_CPA ? (size_t)(3 * NF * 2 + (PAIR ? 3 * kNHS : 0)) * 128 * sizeof(float4) : 0;
   static bool configured = false;
-  if (!configured && smem > 48 * 1024) {
-    cudaFuncSetAttribute(k_update<R, NF, IS_H, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (!configured && smem_max > 48 * 1024) {
+    cudaFuncSetAttribute(k_update<R, NF, IS_H, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     configured = true;
   }
   k_update<R, NF, IS_H, PAIR><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel, harg);

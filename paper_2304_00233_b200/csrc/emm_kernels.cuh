@@ -41,7 +41,13 @@ struct DevRun {
 // harg: mode 1 = history slot the step's field is copied into (-1 none), mode 2 = number of history levels taken
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st);
 constexpr int kPairMaxNF = 5;       // grouped-DTFT instances exist for 1..5 frequencies (the staged, unrolled ones)
-constexpr int kGroupMax = 4;        // largest DTFT group (terms per accumulator pass): 2 history levels + old + new
+#ifndef EMM_GROUP_MAX
+#define EMM_GROUP_MAX 8
+#endif
+constexpr int kGroupMax = EMM_GROUP_MAX;   // largest DTFT group (terms per accumulator pass): history levels + old + new
+// default group: measured on B200 (profiles/r1_grouped_dtft.md) -- 8 with 4-5 frequencies (2 blocks per SM), 6 with 1-3
+// (3 blocks per SM: the staged history quads of a larger group cost the shared memory of the third block)
+inline int default_dtft_group(int nf) { return nf >= 4 ? (kGroupMax < 8 ? kGroupMax : 8) : (kGroupMax < 6 ? kGroupMax : 6); }
 // pairfix: also add the product the two-term kernel misses at the injected nodes (see k_inject)
 int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic, int pairfix);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);

@@ -209,7 +209,7 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   DevState s{};
   DevRun r{};
   layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES),
-             nfreq >= 1 && nfreq <= kPairMaxNF ? kGroupMax - 2 : 0, s, r);                           // the full-grid mode with the largest DTFT group is the larger one
+             nfreq >= 1 && nfreq <= kPairMaxNF ? kGroupMax - 2 : 0, s, r);   // history slots of the largest group a run may ask for                           // the full-grid mode with the largest DTFT group is the larger one
   g->T = keep;
   return std::max(A.off, fixed + 1024) + 4096;       // emm_model_set keeps a few scalars behind the per-grid region
 }
@@ -566,7 +566,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
       static const bool no_pair = getenv("EMM_NO_PAIR") != nullptr;       // A/B measurements
       const bool can = o->dtft_pair >= 0 && !no_pair && nf >= 1 && nf <= kPairMaxNF && !R->sparse && o->dtft_every >= 0 && o->dtft_every <= 1;
       static const char *env_group = getenv("EMM_DTFT_GROUP");             // A/B measurements: default group size
-      const int dflt = env_group && atoi(env_group) >= 2 ? atoi(env_group) : kGroupMax;
+      const int dflt = env_group && atoi(env_group) >= 2 ? atoi(env_group) : default_dtft_group(nf);
       R->group = !can ? 1 : std::min(kGroupMax, o->dtft_pair >= 2 ? o->dtft_pair : dflt);
     }
     if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
@@ -911,6 +911,10 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
     std::complex<double> *o = static_cast<std::complex<double> *>(host_out);
     const std::complex<double> I(0, 1);
     for (int f = 0; f < R->nf; ++f) o[f] = source_spectrum(g, R, isrc, f);
+    return 0;
+  }
+  if (what == EMM_GET_DTFT_GROUP) {
+    *static_cast<int *>(host_out) = R->group;
     return 0;
   }
   if (what == EMM_GET_DELTA) {

@@ -21,7 +21,7 @@ CHECK_CORNERS, CHECK_FACES, CHECK_FULL = 0, 1, 2
 EINVAL, ENOMEM, ECUDA, ENOCONV, ENAN = -1, -2, -3, -4, -5
 _GET = {"E1": 0, "E2": 1, "E3": 2, "H1": 3, "H2": 4, "H3": 5,
         "F_E1": 10, "F_E2": 11, "F_E3": 12, "F_H1": 13, "F_H2": 14, "F_H3": 15,
-        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31}
+        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31, "DTFT_GROUP": 32}
 _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "box_lo2", "box_lo3",
          "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2", "pitch")
 # every symbol include/emm.h declares (tests check that the library exports all of them)
@@ -317,6 +317,8 @@ class Grid:
             out = np.zeros(self._shape_out[1], dtype=np.complex128)
         elif what == "DELTA":
             out = np.zeros(2)
+        elif what == "DTFT_GROUP":
+            out = np.zeros(1, dtype=np.int32)
         elif what.startswith("F_"):
             out = np.zeros(self.shape, dtype=np.complex64)
         else:

@@ -179,8 +179,10 @@ def test_receivers_only_dtft_matches_full_grid_and_oracle(emm, oracle, m):
     ga.run_end()
 
 
-def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle):
-    """Paired DTFT (emm_run_opts.dtft_pair, default): two consecutive terms of Eq. 25 per pass over the accumulators.
+@pytest.mark.parametrize("group", [0, 2, 8])
+def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle, group):
+    """Grouped DTFT (emm_run_opts.dtft_pair; 0 = default group, 2 = pairs, 8 = the largest group): m consecutive terms of
+    Eq. 25 per pass over the accumulators, the earlier levels of a group copied by the passes before the closing one.
     Same fused multiply-adds in the same order as one term per step, so fields and accumulators are bit-identical to
     the dtft_pair = -1 run everywhere except at the injected nodes (where the missing product is added by the
     injection kernel, rounding order differs), whatever the batch sizes (odd batches leave single steps), for an
@@ -191,8 +193,10 @@ def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle):
     w["receivers"] = _small_receivers()
     srcs = [((-150.0, 30.0, 950.0), (1.0, 0.2, 0.1)), ((120.0, -60.0, 930.0), (0.1, 1.0, 0.3), "M")]
     ga, gs = make_grid(emm, w), make_grid(emm, w)
-    ga.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=131, batched=1))
+    ga.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=131, batched=1, dtft_pair=group))
+    assert int(ga.get("DTFT_GROUP")[0]) == (group or 6)                # three frequencies: default group 6
     gs.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=131, batched=1, dtft_pair=-1))
+    assert int(gs.get("DTFT_GROUP")[0]) == 1
     total = 0
     for n in (7, 50, 1, 33, 40):                     # 131 steps: odd and even batches, a pair split by a batch end
         na, _ = ga.run_steps(n)
@@ -213,7 +217,7 @@ def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle):
     os_, _ = gs.run_end()
     assert np.abs(oa - os_).max() <= 1e-5 * np.abs(os_).max()
     opts = dict(tol=1e-6, check_every=75, batched=1)
-    o_p, n_p = ga.run(srcs, w["freqs"], w["receivers"], opts)
+    o_p, n_p = ga.run(srcs, w["freqs"], w["receivers"], dict(opts, dtft_pair=group))
     o_s, n_s = gs.run(srcs, w["freqs"], w["receivers"], dict(opts, dtft_pair=-1))
     o_or, n_or = make_grid(oracle, w).run(srcs, w["freqs"], w["receivers"], dict(opts, sparse_dft=1))
     assert list(n_p) == list(n_s) == list(n_or) and min(n_p) > 0 and n_p[0] % 75 == 0
@@ -227,14 +231,16 @@ def test_paired_dtft_is_the_one_term_sum_bit_for_bit(emm, oracle):
 
 @pytest.mark.parametrize("rd", [1, 2, 3])
 def test_paired_dtft_every_instance(emm, rd):
-    """Every two-term instance k_update<rd, nf, ., PAIR>, nf = 1..5, against the one-term schedule on a small whole-space
-    grid (CPML on six faces), 41 steps in batches of 20 + 21: fields bit-identical, accumulators bit-identical away from
-    the injected nodes and within rounding there.  nf = 6 has no two-term instance: the option is ignored."""
+    """Every closing-pass instance k_update<rd, nf, ., PAIR>, nf = 1..5, with group sizes 6 (default), 2, 3, 5, 8, against
+    the one-term schedule on a small whole-space grid (CPML on six faces), 41 steps in batches of 20 + 21 (whole groups,
+    shorter groups and single steps): fields bit-identical, accumulators bit-identical away from the injected nodes and
+    within rounding there.  nf = 6 has no such instance: the option is ignored."""
     w = W.cfg1(n=26, dx=100.0, rd=rd, nb=5)
     freqs_all = np.array([0.25, 0.5, 0.75, 1.0, 1.25, 1.5])
     for nf in range(1, 7):
         ga, gs = make_grid(emm, w), make_grid(emm, w)
-        ga.run_begin(w["sources"], freqs_all[:nf], w["receivers"][:2], dict(fixed_steps=41))
+        ga.run_begin(w["sources"], freqs_all[:nf], w["receivers"][:2], dict(fixed_steps=41, dtft_pair=(0, 2, 3, 5, 8, 0)[nf - 1]))
+        assert int(ga.get("DTFT_GROUP")[0]) == (6, 2, 3, 5, 8, 1)[nf - 1]
         gs.run_begin(w["sources"], freqs_all[:nf], w["receivers"][:2], dict(fixed_steps=41, dtft_pair=-1))
         for n in (20, 21):
             ga.run_steps(n)
