@@ -209,8 +209,10 @@ __device__ __forceinline__ void dtft4_staged2(const float4 *sm, int c, float2 *F
 // and the unified L1 keeps ~100 KB for the neighbour rows; with fewer frequencies three blocks win.
 template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_MINB : (NF >= 4 ? 2 : 3); }
 
-// PAIR: the two-term instance of the paired DTFT (NF >= 1, staged): the H kernel of step `it` takes the terms it and
-// it+1 of F_H (old and new H), the E kernel of step `it` the terms it-1 and it of F_E (old and new E) [R6].
+// PAIR: the closing pass of a DTFT group (NF >= 1, staged).  The H kernel of step `it` holds old H
+// (term it) and new H (term it+1), the E kernel of step `it` old E (term it-1) and new E (term it) [R6]; with `harg` = nh
+// history levels (copies made by the accumulator-free passes of the nh steps before) the pass takes nh + 2 consecutive
+// terms of Eq. 25 in one read-modify-write of the accumulators, oldest first.
 template <int R, int NF, bool IS_H, bool PAIR = false>
 __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0, const int sel, const int harg) {
   constexpr int O = IS_H ? 1 : 0;            // D+ stencils start one node later than D- (Eq. 13 vs 14)
