@@ -306,12 +306,9 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   }
 
   constexpr bool STAGED = (EMM_CPA != 0) && (NF > 0);
-  static_assert(!PAIR || STAGED, "the paired DTFT instance needs staged accumulators");
+  static_assert(!PAIR || STAGED, "the closing pass of a DTFT group needs staged accumulators");
   float4 *smF = smC;                                   // DTFT instances: the dynamic shared memory holds the staged accumulators
   const size_t cstride = (size_t)g.NZB * g.PS;
-  // The accumulators of the three components are three commit groups, consumed in issue order and re-issued for
-  // the next plane as soon as their slots are free: every copy gets almost a whole plane of lead time, and
-  // `cp.async.wait_group 2` before each use leaves exactly the two younger groups pending.
   // Grouped DTFT.  harg: PAIR instance = number nh of history levels it takes besides its own old
   // and new field (their quads are staged with the accumulators of the component, slots behind them); accumulator-free
   // instance = history slot into which this step's field is copied for the pass that closes the group (-1: none).
@@ -330,6 +327,9 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
         if (l < nh) cp_async16(smF + (HB + c * nh + l) * 128, hs[c] + (size_t)l * g.VS + (size_t)k * g.PS + row);
     }
   };
+  // The accumulators of the three components are three commit groups, consumed in issue order and re-issued for
+  // the next plane as soon as their slots are free: every copy gets almost a whole plane of lead time, and
+  // `cp.async.wait_group 2` before each use leaves exactly the two younger groups pending.
   if constexpr (STAGED) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
