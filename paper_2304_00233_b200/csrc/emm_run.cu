@@ -626,11 +626,11 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     Arena A;
     A.base = static_cast<char *>(g->d_ws); A.cap = g->ws_bytes; A.dry = false; A.off = g->fixed_bytes;
     layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), R->group > 2 ? R->group - 2 : 0, R->ds, R->dr);
-    if (A.overflow && R->group > 2) {        // a workspace sized by an older rule: fall back to pairs (no history copies)
-      R->group = 2;
+    while (A.overflow && R->group > 2) {     // a workspace without room for all the history copies: the largest group that fits
+      R->group--;
       A.off = g->fixed_bytes;
       A.overflow = false;
-      layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), 0, R->ds, R->dr);
+      layout_run(g, A, nsrc, R->sparse ? 0 : nf, R->sparse ? nf : 0, R->table_steps, nrec, chk.size(), R->group - 2, R->ds, R->dr);
     }
     if (g->top == EMM_TOP_AIR && g->sep_air && !A.overflow)
       for (int q = 0; q < 8; ++q)

@@ -230,16 +230,17 @@ class Grid:
             raise EmmError(ECUDA, lib().emm_last_error().decode())
         return n
 
-    def bind(self, nsrc=1, nfreq=1, max_steps=0, nrec=64, device="cuda:0"):
+    def bind(self, nsrc=1, nfreq=1, max_steps=0, nrec=64, device="cuda:0", ws_bytes=None):
+        """ws_bytes: bind a workspace of exactly this size instead of emm_workspace_bytes() (tests of the tight-memory paths)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libemm_b200 needs a CUDA device; there is no CPU fallback")
         max_steps = max_steps or 100000
         plan = (nsrc, nfreq, max_steps, nrec)
-        if self._ws is not None and self._plan is not None and all(a <= b for a, b in zip(plan, self._plan)):
+        if ws_bytes is None and self._ws is not None and self._plan is not None and all(a <= b for a, b in zip(plan, self._plan)):
             return
         torch.cuda.set_device(device)
-        n = self.workspace_bytes(nsrc, nfreq, max_steps, nrec)
+        n = int(ws_bytes) if ws_bytes is not None else self.workspace_bytes(nsrc, nfreq, max_steps, nrec)
         self._ws = None
         self._ws = torch.empty(n, dtype=torch.uint8, device=device)
         torch.cuda.synchronize(device)

@@ -259,6 +259,36 @@ def test_paired_dtft_every_instance(emm, rd):
         gs.close()
 
 
+def test_grouped_dtft_takes_the_largest_group_the_workspace_allows(emm):
+    """A workspace short of three history slots: the run falls back from groups of 8 to groups of 5 (same sums, bit for
+    bit); without room for any copy it runs pairs; without room for the run at all it fails with EMM_ENOMEM."""
+    w = W.cfg1(n=26, dx=100.0, rd=2, nb=5)
+    freqs = np.array([0.25, 0.5, 0.75, 1.0])            # four frequencies: default group 8
+    ref = make_grid(emm, w)
+    ref.run_begin(w["sources"], freqs, w["receivers"][:2], dict(fixed_steps=40, dtft_pair=-1))
+    ref.run_steps(40)
+    Fref = ref.get("F_E1", ifreq=3)
+    info = ref.info()
+    vol = info["pitch"] * info["N2"] * info["N3"] * 4                      # bytes of one field-sized array
+    full = ref.workspace_bytes(1, len(freqs), 50, 2)
+    for short, group in ((0, 8), (3 * 6 * vol, 5), (6 * 6 * vol, 2)):
+        g = emm.Grid(w["x"], w["y"], w["z"], **w["grid"])
+        g.bind(nsrc=1, nfreq=len(freqs), max_steps=50, nrec=2, ws_bytes=full - short)
+        g.model_set(w["sigma_h"])
+        g.run_begin(w["sources"], freqs, w["receivers"][:2], dict(fixed_steps=40))
+        assert int(g.get("DTFT_GROUP")[0]) == group, (short, int(g.get("DTFT_GROUP")[0]))
+        g.run_steps(40)
+        F = g.get("F_E1", ifreq=3)
+        assert (F != Fref).sum() <= 4 ** 3 and np.abs(F - Fref).max() <= 1e-5 * np.abs(Fref).max()
+        g.close()
+    g = emm.Grid(w["x"], w["y"], w["z"], **w["grid"])
+    g.bind(nsrc=1, nfreq=len(freqs), max_steps=50, nrec=2, ws_bytes=full - 6 * 6 * vol - 30 * vol)
+    g.model_set(w["sigma_h"])
+    with pytest.raises(emm.EmmError) as e:
+        g.run_begin(w["sources"], freqs, w["receivers"][:2], dict(fixed_steps=40))
+    assert e.value.code == emm.ENOMEM
+
+
 def test_plane_and_separable_air_routes_agree(emm, oracle, monkeypatch):
     """Non-uniform x-y: the separable route (batched 1-D transforms, default) and the plane-sized 2-D route
     (EMM_AIR_PLANE=1) are the same linear map up to rounding order; both are within the field tolerance of the oracle."""
