@@ -62,7 +62,7 @@ def algorithmic_bytes(info, nf, nb, kernel, m=1):
     = 36 B/node; each RMWs 3*nf complex accumulators (48*nf B) per DTFT-box node; plus 8 B per active CPML
     memory variable (two per slab membership).  Grouped DTFT with m terms per accumulator pass:
     the closing pass of a group ("E2"/"H2") also reads m-2 earlier levels of its 3 components (12 B per box node each);
-    of the m-1 accumulator-free passes of a group ("E0"/"H0") m-2 write such a copy: the average is charged."""
+    the accumulator-free passes ("E0"/"H0") update out of place into the next buffer of the ring: no extra bytes."""
     N1, N2, N3 = info["N1"], info["N2"], info["N3"]
     N = N1 * N2 * N3
     box = ((info["box_hi1"] - info["box_lo1"] + 1) * (info["box_hi2"] - info["box_lo2"] + 1)
@@ -72,8 +72,6 @@ def algorithmic_bytes(info, nf, nb, kernel, m=1):
     b = (48 if kernel[0] == "E" else 36) * N + 48 * (0 if kernel[1:] == "0" else nf) * box + psi
     if kernel[1:] == "2":
         b += 12 * max(m - 2, 0) * box
-    if kernel[1:] == "0" and m > 2:
-        b += 12 * box * (m - 2) / (m - 1)
     return b
 
 

@@ -65,8 +65,15 @@ struct DevState {              // per run; arrays carry a leading source dimensi
   float *psy[2][2];            // y-slab psi [nsrc][N3][2nb][P1]
   float *psz[2][2];            // z-slab psi [nsrc][2nb][N2][P1]
   float2 *F;                   // [nsrc][nf][6][NZB][N2][P1]
-  float *hist[2][3];           // grouped DTFT: [E/H][component] copies of earlier time levels [nsrc][nslots][N3][N2][P1]
-  int nslots;                  // history slots per component (group size - 2; 0: none)
+  // Grouped DTFT: inside a group of m > 2 steps the fields are updated out of place through a ring
+  // of nbuf buffers per component ([nbuf][nsrc][N3][N2][P1], E[c]/H[c] of the run = buffer 0), so that earlier time levels
+  // stay readable for the pass that closes the group.  Per launch: E/H = the buffers holding the current fields, Eo/Ho =
+  // where the update kernel writes (nullptr: in place), hist = first history level of the closing pass, hstride = floats
+  // between consecutive levels.
+  float *Eo[3], *Ho[3];
+  const float *hist[2][3];
+  long long hstride;
+  int nbuf;
   const float2 *twE, *twH;     // [max_steps][nf]
   const float *wav;            // [max_steps] s(it dt): electric sources
   const float *wavh;           // [max_steps] s((it+1/2) dt): magnetic sources

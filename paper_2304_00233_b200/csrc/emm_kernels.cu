@@ -233,9 +233,14 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   const float *A1 = (IS_H ? s.E[0] : s.H[0]) + (size_t)src * g.VS;
   const float *A2 = (IS_H ? s.E[1] : s.H[1]) + (size_t)src * g.VS;
   const float *A3 = (IS_H ? s.E[2] : s.H[2]) + (size_t)src * g.VS;
-  float *U1 = (IS_H ? s.H[0] : s.E[0]) + (size_t)src * g.VS;
-  float *U2 = (IS_H ? s.H[1] : s.E[1]) + (size_t)src * g.VS;
-  float *U3 = (IS_H ? s.H[2] : s.E[2]) + (size_t)src * g.VS;
+  const float *U1 = (IS_H ? s.H[0] : s.E[0]) + (size_t)src * g.VS;
+  const float *U2 = (IS_H ? s.H[1] : s.E[1]) + (size_t)src * g.VS;
+  const float *U3 = (IS_H ? s.H[2] : s.E[2]) + (size_t)src * g.VS;
+  // where the updated field goes: in place, or (inside a DTFT group of more than two steps) the next buffer of the ring
+  float *const *Uo = IS_H ? s.Ho : s.Eo;
+  float *W1 = (Uo[0] ? Uo[0] : (IS_H ? s.H[0] : s.E[0])) + (size_t)src * g.VS;
+  float *W2 = (Uo[1] ? Uo[1] : (IS_H ? s.H[1] : s.E[1])) + (size_t)src * g.VS;
+  float *W3 = (Uo[2] ? Uo[2] : (IS_H ? s.H[2] : s.E[2])) + (size_t)src * g.VS;
   const float *tx = IS_H ? g.cp[0] : g.cm[0];
   const float *ty = IS_H ? g.cp[1] : g.cm[1];
   const float *tz = IS_H ? g.cp[2] : g.cm[2];
@@ -309,22 +314,21 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   static_assert(!PAIR || STAGED, "the closing pass of a DTFT group needs staged accumulators");
   float4 *smF = smC;                                   // DTFT instances: the dynamic shared memory holds the staged accumulators
   const size_t cstride = (size_t)g.NZB * g.PS;
-  // Grouped DTFT.  harg: PAIR instance = number nh of history levels it takes besides its own old
-  // and new field (their quads are staged with the accumulators of the component, slots behind them); accumulator-free
-  // instance = history slot into which this step's field is copied for the pass that closes the group (-1: none).
+  // Grouped DTFT.  harg (PAIR instance) = number nh of history levels it takes besides its own old
+  // and new field: whole earlier buffers of the ring, oldest first; their quads are staged with the accumulators of the
+  // component, in slots behind them.
   const int nh = PAIR ? harg : 0;
-  const bool hist_xy = (NF == 0) && harg >= 0 && (j >= g.blo[1]) && (j <= g.bhi[1]) && (i0 + 3 >= g.blo[0]) && (i0 <= g.bhi[0]);   // copies are read inside the DTFT box only
   const float *hs[3] = {nullptr, nullptr, nullptr};
-  if (PAIR || (NF == 0 && harg >= 0)) {
+  if constexpr (PAIR) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) hs[c] = s.hist[IS_H ? 1 : 0][c] + ((size_t)src * s.nslots + (PAIR ? 0 : harg)) * g.VS;
+    for (int c = 0; c < 3; ++c) hs[c] = s.hist[IS_H ? 1 : 0][c] + (size_t)src * g.VS;
   }
   constexpr int HB = 3 * (NF > 0 ? NF : 0) * 2;        // first history slot in shared memory
   auto stage_history = [&](int c, int k) {
     if constexpr (PAIR) {
 #pragma unroll
       for (int l = 0; l < kNHS; ++l)
-        if (l < nh) cp_async16(smF + (HB + c * nh + l) * 128, hs[c] + (size_t)l * g.VS + (size_t)k * g.PS + row);
+        if (l < nh) cp_async16(smF + (HB + c * nh + l) * 128, hs[c] + (size_t)l * s.hstride + (size_t)k * g.PS + row);
     }
   };
   // The accumulators of the three components are three commit groups, consumed in issue order and re-issued for
@@ -482,20 +486,14 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
       u1 = make_float4(fmaf(-m0, c1.x, u1.x), fmaf(-m1, c1.y, u1.y), fmaf(-m2, c1.z, u1.z), fmaf(-m3, c1.w, u1.w));
       u2 = make_float4(fmaf(-m0, c2.x, u2.x), fmaf(-m1, c2.y, u2.y), fmaf(-m2, c2.z, u2.z), fmaf(-m3, c2.w, u2.w));
       u3 = make_float4(fmaf(-m0, c3.x, u3.x), fmaf(-m1, c3.y, u3.y), fmaf(-m2, c3.z, u3.z), fmaf(-m3, c3.w, u3.w));
-      st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
-      if (hist_xy && k >= g.blo[2] && k <= g.bhi[2]) {      // H^{it} (before this update) is term `it` of the group this step belongs to
-        stcs4(const_cast<float *>(hs[0]) + c0, o1); stcs4(const_cast<float *>(hs[1]) + c0, o2); stcs4(const_cast<float *>(hs[2]) + c0, o3);
-      }
+      st4(W1 + c0, u1); st4(W2 + c0, u2); st4(W3 + c0, u3);
       // PAIR: old H is term it, new H is term it+1 (the old H of the next step)
       if constexpr (PAIR) { dtft_staged_component(0, o1, u1); dtft_staged_component(1, o2, u2); dtft_staged_component(2, o3, u3); }
     } else {
       u1 = make_float4(fmaf(e1.x, c1.x, u1.x), fmaf(e1.y, c1.y, u1.y), fmaf(e1.z, c1.z, u1.z), fmaf(e1.w, c1.w, u1.w));
       u2 = make_float4(fmaf(e2.x, c2.x, u2.x), fmaf(e2.y, c2.y, u2.y), fmaf(e2.z, c2.z, u2.z), fmaf(e2.w, c2.w, u2.w));
       u3 = make_float4(fmaf(e3.x, c3.x, u3.x), fmaf(e3.y, c3.y, u3.y), fmaf(e3.z, c3.z, u3.z), fmaf(e3.w, c3.w, u3.w));
-      st4(U1 + c0, u1); st4(U2 + c0, u2); st4(U3 + c0, u3);
-      if (hist_xy && k >= g.blo[2] && k <= g.bhi[2]) {      // E^{it+1/2} (after this update, injection included) is term `it`
-        stcs4(const_cast<float *>(hs[0]) + c0, u1); stcs4(const_cast<float *>(hs[1]) + c0, u2); stcs4(const_cast<float *>(hs[2]) + c0, u3);
-      }
+      st4(W1 + c0, u1); st4(W2 + c0, u2); st4(W3 + c0, u3);
       // new E sits at t = (it+1/2)*dt [R6]; PAIR: old E is term it-1, new E is term it
       if constexpr (PAIR) { dtft_staged_component(0, o1, u1); dtft_staged_component(1, o2, u2); dtft_staged_component(2, o3, u3); }
       else if constexpr (STAGED) { dtft_staged_component(0, u1); dtft_staged_component(1, u2); dtft_staged_component(2, u3); }

@@ -114,7 +114,13 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
   const size_t V = vol(g), PS = (size_t)g->P1 * g->N[1];
   const int np = std::max(2 * g->r, 4);
   const size_t np3 = (size_t)np * np * np;
-  for (int c = 0; c < 3; ++c) { s.E[c] = A.take<float>(V * nsrc); s.H[c] = A.take<float>(V * nsrc); }
+  // fields: a ring of nbuf buffers per component (nbuf = 1 unless the run groups more than two DTFT terms); buffer 0 is
+  // where the fields live outside such a group
+  const int nbuf = nslots > 0 ? nslots + 2 : 1;
+  for (int c = 0; c < 3; ++c) { s.E[c] = A.take<float>(V * nsrc * nbuf); s.H[c] = A.take<float>(V * nsrc * nbuf); }
+  for (int c = 0; c < 3; ++c) { s.Eo[c] = s.Ho[c] = nullptr; s.hist[0][c] = s.hist[1][c] = nullptr; }
+  s.nbuf = nbuf;
+  s.hstride = (long long)V * nsrc;
   for (int k = 0; k < 2; ++k)
     for (int q = 0; q < 2; ++q) {
       s.psx[k][q] = A.take<float>((size_t)nsrc * g->N[2] * g->N[1] * g->XS);
@@ -123,9 +129,7 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
     }
   const size_t nzb = g->bhi[2] - g->blo[2] + 1;
   s.F = A.take<float2>((size_t)nsrc * nf * 6 * nzb * PS);
-  s.nslots = nslots;
-  for (int k = 0; k < 2; ++k)
-    for (int c = 0; c < 3; ++c) s.hist[k][c] = nslots > 0 ? A.take<float>((size_t)nsrc * nslots * V) : nullptr;
+
   s.twE = A.take<float2>((size_t)table_steps * nf);
   s.twH = A.take<float2>((size_t)table_steps * nf);
   s.wav = A.take<float>(table_steps);
@@ -209,7 +213,7 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   DevState s{};
   DevRun r{};
   layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES),
-             nfreq >= 1 && nfreq <= kPairMaxNF ? kGroupMax - 2 : 0, s, r);   // history slots of the largest group a run may ask for                           // the full-grid mode with the largest DTFT group is the larger one
+             nfreq >= 1 && nfreq <= kPairMaxNF ? kGroupMax - 2 : 0, s, r);   // field buffers of the largest group a run may ask for                           // the full-grid mode with the largest DTFT group is the larger one
   g->T = keep;
   return std::max(A.off, fixed + 1024) + 4096;       // emm_model_set keeps a few scalars behind the per-grid region
 }
@@ -416,7 +420,9 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
     // it and it+1 of F_H (old and new H) and the E kernel none; in the second the E kernel adds the terms it-1 and it of
     // F_E (old and new E) and the H kernel none; a left-over last step takes its single terms as usual.  A batch never
     // crosses a convergence check (enqueue_steps), so every sum is complete where it is read.
-    int me = 0, mh = 0, he = -1, hh = -1;
+    int me = 0, mh = 0, he = -1, hh = -1, fix_e = 0;
+    // s1: injection + E update; s2: E boundary, check set, H update; s3: H boundary, magnetic injection, check
+    DevState s1 = R->ds, s2 = R->ds, s3 = R->ds;
     if (R->group > 1) {
       if (gpos >= gsize) {                   // open the next group of this batch: up to `group` steps, at least 2
         gpos = 0;
@@ -424,56 +430,72 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
         if (gsize < 2) gsize = 1;
       }
       if (gsize >= 2) {
-        // position p of a group of m steps.  E kernel: copies its new field into history slot p (p <= m-3), nothing
-        // extra at p = m-2 (that level is the old field of the closing pass), closes the group at p = m-1 with m terms.
-        // H kernel: copies its old field into slot p (p <= m-3), closes the group at p = m-2 (old H = term m-2, new H =
-        // term m-1), nothing at p = m-1.  m = 2: the pair of two-term passes.
+        // Position p of a group of m steps.  The E kernel closes the group at p = m-1 with m terms: its old E (term m-2),
+        // its new E (term m-1) and the m-2 levels before; the H kernel closes it at p = m-2: old H (term m-2), new H
+        // (term m-1).  m = 2: the pair of two-term passes, in place.  m > 2: step p reads buffer p of the ring and writes
+        // buffer p+1 (the last step writes buffer 0), so that E after step l (term l) stays in buffer l+1 and H before
+        // step l (term l) in buffer l until the closing pass has taken them.
         const int m = gsize, p = gpos;
-        if (p == m - 1) { me = 2; he = m - 2; } else { me = 1; he = p <= m - 3 ? p : -1; }
-        if (p == m - 2) { mh = 2; hh = m - 2; } else { mh = 1; hh = p <= m - 3 ? p : -1; }
+        if (p == m - 1) { me = 2; he = m - 2; } else me = 1;
+        if (p == m - 2) { mh = 2; hh = m - 2; } else mh = 1;
+        // the electric injection of step p lands in the buffer that holds term p-1 (closing pass: its old E): the missing
+        // product goes into the accumulators with the injection
+        fix_e = p >= 1;
+        if (m > 2) {
+          const size_t bs = (size_t)R->ds.hstride;
+          const int pn = (p + 1) % m;
+          for (int c = 0; c < 3; ++c) {
+            float *Ein = R->ds.E[c] + p * bs, *Eout = R->ds.E[c] + pn * bs, *Hin = R->ds.H[c] + p * bs, *Hout = R->ds.H[c] + pn * bs;
+            s1.E[c] = Ein; s1.Eo[c] = Eout; s1.H[c] = Hin;
+            s2.E[c] = Eout; s2.H[c] = Hin; s2.Ho[c] = Hout;
+            s3.E[c] = Eout; s3.H[c] = Hout;
+            s1.hist[0][c] = R->ds.E[c] + bs;          // E terms 0 .. m-3 sit in buffers 1 .. m-2
+            s2.hist[1][c] = R->ds.H[c];               // H terms 0 .. m-3 sit in buffers 0 .. m-3
+          }
+        }
       }
       ++gpos;
     }
-    if (R->any_el && (rc = launch_inject(g, R->ds, R->dr, 0, me == 2))) return rc;     // Alg. 1 L477 (before the update: same sum)
+    if (R->any_el && (rc = launch_inject(g, s1, R->dr, 0, fix_e))) return rc;     // Alg. 1 L477 (before the update: same sum)
     if (g->top != EMM_TOP_AIR) {
-      if ((rc = launch_update(g, R->ds, 0, 0, me, he, M))) return rc;                 // L476-479 + E part of L483
-      if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;                // check-set part of L483
-      if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_update(g, R->ds, 1, 0, mh, hh, M))) return rc;                 // H part of L483 + L486-489
+      if ((rc = launch_update(g, s1, 0, 0, me, he, M))) return rc;                 // L476-479 + E part of L483
+      if ((rc = launch_check_acc(g, s2, R->dr))) return rc;                // check-set part of L483
+      if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
+      if ((rc = launch_update(g, s2, 1, 0, mh, hh, M))) return rc;                 // H part of L483 + L486-489
     } else if (g->prof || no_overlap) {
       // one thing after the other (per-kernel timing, or EMM_NO_OVERLAP): the boundary still runs on its own stream
-      if ((rc = launch_update(g, R->ds, 0, 0, me, he, M))) return rc;
+      if ((rc = launch_update(g, s1, 0, 0, me, he, M))) return rc;
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));
-      if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
+      if ((rc = launch_air(g, s2, R->dr, 0, B))) return rc;                // L481
       CU(cudaEventRecord(g->ev[1], B)); CU(cudaStreamWaitEvent(M, g->ev[1], 0));
-      if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_update(g, R->ds, 1, 0, mh, hh, M))) return rc;
+      if ((rc = launch_check_acc(g, s2, R->dr))) return rc;
+      if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
+      if ((rc = launch_update(g, s2, 1, 0, mh, hh, M))) return rc;
       CU(cudaEventRecord(g->ev[2], M)); CU(cudaStreamWaitEvent(B, g->ev[2], 0));
-      if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
+      if ((rc = launch_air(g, s3, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));
     } else {
       // The boundary only feeds the z chunks next to the surface: those chunks and the FFT boundary form a short
       // chain on the helper stream while the bulk of the grid is updated on the main stream (fork/join per step).
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));      // fork (after the injection)
-      if ((rc = launch_update(g, R->ds, 0, 1, me, he, B))) return rc;                 // E, surface chunks
+      if ((rc = launch_update(g, s1, 0, 1, me, he, B))) return rc;                 // E, surface chunks
       CU(cudaEventRecord(g->ev[1], B));
-      if ((rc = launch_air(g, R->ds, R->dr, 0, B))) return rc;                // L481
-      if ((rc = launch_update(g, R->ds, 0, 2, me, he, M))) return rc;                 // E, bulk
+      if ((rc = launch_air(g, s2, R->dr, 0, B))) return rc;                // L481
+      if ((rc = launch_update(g, s1, 0, 2, me, he, M))) return rc;                 // E, bulk
       CU(cudaEventRecord(g->ev[2], M));
       CU(cudaStreamWaitEvent(M, g->ev[1], 0));                                // H bulk and the check set read surface-chunk E
-      if ((rc = launch_check_acc(g, R->ds, R->dr))) return rc;
-      if ((rc = launch_rec_acc(g, R->ds, R->dr))) return rc;
+      if ((rc = launch_check_acc(g, s2, R->dr))) return rc;
+      if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
       CU(cudaEventRecord(g->ev[4], M));
-      if ((rc = launch_update(g, R->ds, 1, 2, mh, hh, M))) return rc;                 // H, bulk
+      if ((rc = launch_update(g, s2, 1, 2, mh, hh, M))) return rc;                 // H, bulk
       CU(cudaStreamWaitEvent(B, g->ev[2], 0)); CU(cudaStreamWaitEvent(B, g->ev[4], 0));
-      if ((rc = launch_update(g, R->ds, 1, 1, mh, hh, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
-      if ((rc = launch_air(g, R->ds, R->dr, 1, B))) return rc;                // L491
+      if ((rc = launch_update(g, s2, 1, 1, mh, hh, B))) return rc;                 // H, surface chunks (after bulk E, check set, ghost E)
+      if ((rc = launch_air(g, s3, R->dr, 1, B))) return rc;                // L491
       CU(cudaEventRecord(g->ev[3], B)); CU(cudaStreamWaitEvent(M, g->ev[3], 0));      // join
     }
-    if (R->any_mag && (rc = launch_inject(g, R->ds, R->dr, 1, mh == 2))) return rc;    // L488, after the H update and its boundary
+    if (R->any_mag && (rc = launch_inject(g, s3, R->dr, 1, mh == 2))) return rc;    // L488, after the H update and its boundary
     if (R->nf > 0 && (R->it_host + 1) % R->check_every == 0 &&
-        (rc = launch_check(g, R->ds, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
+        (rc = launch_check(g, s3, R->dr, R->it_min, R->tol, R->fixed_steps ? 0 : 1))) return rc;   // L493-498
     if ((rc = launch_step_end(g, R->ds))) return rc;
     R->it_host++;
   }
