@@ -82,15 +82,16 @@ typedef struct {
   int dtft_pair;   /* Grouped DTFT: every term of Eq. 25 is taken, m consecutive terms per read-modify-write of the
                       accumulators.  An update kernel holds the field before and after its own update, i.e. the DTFT
                       operands of two consecutive steps (L372: old H of steps it and it+1; new E of steps it-1 and it);
-                      the m-2 earlier levels of a group are copied by the accumulator-free passes of the steps before
-                      (12 B/node each) and read back by the pass that closes the group.  Each accumulator gets the same
+                      the m-2 earlier levels of a group stay readable because inside a group the fields are updated out
+                      of place through a ring of m buffers; the pass that closes the group reads them (12 B/node each).  Each accumulator gets the same
                       fused multiply-adds in the same order as with one term per step, at 1/m of the 96*nf B/node
                       traffic.  Groups never cross a convergence check or the end of an emm_run_steps/emm_run_enqueue
                       batch (shorter groups and single steps fill the rest), so accumulators are complete whenever they
                       can be read.  Applies to 1..5 frequencies with full-grid accumulators and dtft_every <= 1; otherwise
                       ignored.  0: default m (8 with 4-5 frequencies, 6 with 1-3); 2..8: that m (2 = pairs, no copies);
                       -1: one term per step in every step, as the paper's kernels do (L454, L880-884).  The workspace
-                      holds (m-2)*6 field-sized arrays per source for the copies.                                    */
+                      holds (m-1)*6 more field-sized arrays per source for the ring; a workspace without room for them
+                      gets the largest m that fits.                                                                  */
 } emm_run_opts;
 
 /* integer grid facts for emm_grid_info(): */
