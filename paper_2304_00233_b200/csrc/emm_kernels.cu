@@ -211,7 +211,7 @@ template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_
 
 // PAIR: the closing pass of a DTFT group (NF >= 1, staged).  The H kernel of step `it` holds old H
 // (term it) and new H (term it+1), the E kernel of step `it` old E (term it-1) and new E (term it) [R6]; with `harg` = nh
-// history levels (copies made by the accumulator-free passes of the nh steps before) the pass takes nh + 2 consecutive
+// history levels (earlier buffers of the field ring the steps of the group update through) the pass takes nh + 2 consecutive
 // terms of Eq. 25 in one read-modify-write of the accumulators, oldest first.
 template <int R, int NF, bool IS_H, bool PAIR = false>
 __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const DevGrid g, const DevState s, const int kc, const int nchunks, const int chunk0, const int sel, const int harg) {
@@ -722,7 +722,7 @@ static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 
 // 2 = all the others.  Parts 1 and 2 can run on different streams (emm_run.cu overlaps the boundary with part 2).
 // mode: 0 = one DTFT term per step (and DTFT decimation); paired DTFT: 1 = the step in which this kernel takes no
 // term (accumulator-free instance), 2 = the step in which it takes two (PAIR instance)
-// harg: mode 1 = history slot this step's field is copied into (-1: none); mode 2 = history levels the pass takes
+// harg: mode 2 = history levels (earlier buffers of the ring) the closing pass takes; unused in the other modes
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st) {
   const DevGrid &dg = g->dg;
   const int quads = dg.P1 / 4;

@@ -38,7 +38,7 @@ struct DevRun {
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
 // mode: 0 = one DTFT term per step; paired DTFT: 1 = accumulator-free step of this kernel, 2 = its two-term step
-// harg: mode 1 = history slot the step's field is copied into (-1 none), mode 2 = number of history levels taken
+// harg: mode 2 = number of history levels (earlier buffers of the ring) the closing pass takes; unused otherwise
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st);
 constexpr int kPairMaxNF = 5;       // grouped-DTFT instances exist for 1..5 frequencies (the staged, unrolled ones)
 #ifndef EMM_GROUP_MAX
