@@ -92,61 +92,85 @@ static int smallest_factor(int n) {
   return n;
 }
 
-/* out[k] = sum_j in[j*stride] W^{sign*jk}, length n, W = exp(-2 pi i/n); tmp holds n values. */
-static void fft_rec(const fftplan *pl, const cplx *in, int stride, cplx *out, int n, int sign, cplx *tmp) {
-  if (n == 1) { out[0] = in[0]; return; }
+/* FB lines are transformed together: element t of line c sits at v[t*FB + c] (re) / vi[...] (im), so that every
+ * inner loop runs over the FB lines with one twiddle factor.  Per line this is the plain recursion
+ *   out[k + j m] = sum_q W_n^{q (k + j m)} sub_q[k],   sub_q = transform of in[q], in[q + p], ...   (n = p m, p prime)
+ * with the sum over q taken in order q = 0..p-1; length n, W = exp(-2 pi i/n) (sign < 0) or its conjugate.      */
+#define FB 16
+static void fft_rec(const fftplan *pl, const double *inr, const double *ini, int stride, double *outr, double *outi,
+                    int n, int sign, double *tr, double *ti) {
+  if (n == 1) {
+    for (int c = 0; c < FB; c++) { outr[c] = inr[c]; outi[c] = ini[c]; }
+    return;
+  }
   int p = smallest_factor(n), m = n / p;
-  for (int q = 0; q < p; q++) fft_rec(pl, in + (size_t)q * stride, stride * p, out + (size_t)q * m, m, sign, tmp);
+  for (int q = 0; q < p; q++)
+    fft_rec(pl, inr + (size_t)q * stride * FB, ini + (size_t)q * stride * FB, stride * p, outr + (size_t)q * m * FB,
+            outi + (size_t)q * m * FB, m, sign, tr, ti);
   int step = pl->n / n; /* W_n^a = w[a*step] */
+  const double sg = sign > 0 ? -1.0 : 1.0;       /* sign > 0: conjugate twiddles */
   for (int k = 0; k < m; k++) {
     for (int j = 0; j < p; j++) {
       int kk = k + j * m;
-      cplx acc = 0;
+      double *ar = tr + (size_t)kk * FB, *ai = ti + (size_t)kk * FB;
+      for (int c = 0; c < FB; c++) { ar[c] = 0; ai[c] = 0; }
+      int a = 0;                                 /* (q * kk) mod n, carried from q to q + 1 */
       for (int q = 0; q < p; q++) {
-        int a = (int)(((long long)q * kk) % n);
-        cplx w = pl->w[(size_t)a * step];
-        if (sign > 0) w = conj(w);
-        acc += w * out[(size_t)q * m + k];
+        const double wr = creal(pl->w[(size_t)a * step]), wi = sg * cimag(pl->w[(size_t)a * step]);
+        const double *xr = outr + ((size_t)q * m + k) * FB, *xi = outi + ((size_t)q * m + k) * FB;
+#pragma omp simd
+        for (int c = 0; c < FB; c++) {
+          ar[c] += wr * xr[c] - wi * xi[c];
+          ai[c] += wr * xi[c] + wi * xr[c];
+        }
+        a += kk; if (a >= n) a -= n;
       }
-      tmp[kk] = acc;
     }
   }
   /* second pass needed because out[q*m+k] for all q are inputs of all j */
-  for (int k = 0; k < n; k++) out[k] = tmp[k];
+  memcpy(outr, tr, sizeof(double) * (size_t)n * FB);
+  memcpy(outi, ti, sizeof(double) * (size_t)n * FB);
+}
+
+/* nl lines of length n of a[], element stride es, line stride ls, transformed in place, FB lines at a time */
+static int fft_lines(cplx *a, int n, size_t es, int nl, size_t ls, int sign, const fftplan *pl) {
+  int err = 0;
+#pragma omp parallel
+  {
+    double *buf = (double *)malloc(sizeof(double) * 6 * (size_t)n * FB);
+    if (!buf) {
+#pragma omp atomic write
+      err = 1;
+    } else {
+      double *inr = buf, *ini = buf + (size_t)n * FB, *outr = buf + 2 * (size_t)n * FB, *outi = buf + 3 * (size_t)n * FB,
+             *tr = buf + 4 * (size_t)n * FB, *ti = buf + 5 * (size_t)n * FB;
+#pragma omp for schedule(dynamic, 1)
+      for (int l0 = 0; l0 < nl; l0 += FB) {
+        const int nc = nl - l0 < FB ? nl - l0 : FB;
+        for (int t = 0; t < n; t++)
+          for (int c = 0; c < FB; c++) {
+            const cplx v = c < nc ? a[(size_t)(l0 + c) * ls + (size_t)t * es] : 0;
+            inr[(size_t)t * FB + c] = creal(v); ini[(size_t)t * FB + c] = cimag(v);
+          }
+        fft_rec(pl, inr, ini, 1, outr, outi, n, sign, tr, ti);
+        for (int t = 0; t < n; t++)
+          for (int c = 0; c < nc; c++) a[(size_t)(l0 + c) * ls + (size_t)t * es] = outr[(size_t)t * FB + c] + I * outi[(size_t)t * FB + c];
+      }
+      free(buf);
+    }
+  }
+  return err ? -1 : 0;
 }
 
 /* 2-D transform of a[n2][n1] in place.  sign=-1: F(k) = 1/(n1 n2) sum f e^{-ikx}; sign=+1:     */
 /* f = sum F e^{+ikx}  (convention of Eq. 32).                                           */
 static int fft2_inplace(cplx *a, int n1, int n2, int sign, const fftplan *p1, const fftplan *p2) {
-  int err = 0;
-#pragma omp parallel
-  {
-    int nmax = n1 > n2 ? n1 : n2;
-    cplx *buf = (cplx *)malloc(sizeof(cplx) * 3 * (size_t)nmax);
-    if (!buf) {
-#pragma omp atomic write
-      err = 1;
-    } else {
-      cplx *in = buf, *out = buf + nmax, *tmp = buf + 2 * (size_t)nmax;
-#pragma omp for
-      for (int j = 0; j < n2; j++) {
-        memcpy(in, a + (size_t)j * n1, sizeof(cplx) * (size_t)n1);
-        fft_rec(p1, in, 1, out, n1, sign, tmp);
-        memcpy(a + (size_t)j * n1, out, sizeof(cplx) * (size_t)n1);
-      }
-#pragma omp for
-      for (int i = 0; i < n1; i++) {
-        for (int j = 0; j < n2; j++) in[j] = a[(size_t)j * n1 + i];
-        fft_rec(p2, in, 1, out, n2, sign, tmp);
-        for (int j = 0; j < n2; j++) a[(size_t)j * n1 + i] = out[j];
-      }
-      free(buf);
-    }
-  }
-  if (err) return -1;
+  if (fft_lines(a, n1, 1, n2, (size_t)n1, sign, p1)) return -1;      /* rows    */
+  if (fft_lines(a, n2, (size_t)n1, n1, 1, sign, p2)) return -1;      /* columns */
   if (sign < 0) {
     double s = 1.0 / ((double)n1 * (double)n2);
-    for (size_t t = 0; t < (size_t)n1 * n2; t++) a[t] *= s;
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < n2; j++) for (int i = 0; i < n1; i++) a[(size_t)j * n1 + i] *= s;
   }
   return 0;
 }
@@ -837,6 +861,7 @@ static int airwave_bc_update_E(const emmo_grid *g, srcstate *S) {
     if (fft2_inplace(A, M1, M2, -1, &g->p1, &g->p2)) { free(A); free(B); return -1; }
     for (int m = 1; m <= r - 1; m++) {
       double h = g->xn[2][k0] - g->xn[2][k0 - m];
+#pragma omp parallel for schedule(static)
       for (int n2 = 0; n2 < M2; n2++) for (int n1 = 0; n1 < M1; n1++) {
         double kx = wavenum(n1, M1, g->dxa), ky = wavenum(n2, M2, g->dya), kh = sqrt(kx * kx + ky * ky);
         B[(size_t)n2 * M1 + n1] = A[(size_t)n2 * M1 + n1] * exp(-kh * h);
@@ -861,6 +886,7 @@ static int airwave_bc_update_H(const emmo_grid *g, srcstate *S) {
   for (int m = 1; m <= r; m++) {
     double h = g->xn[2][k0] - g->xh[2][k0 - m];
     for (int comp = 0; comp < 2; comp++) {            /* 0: Hx (uses kx), 1: Hy (uses ky) */
+#pragma omp parallel for schedule(static)
       for (int n2 = 0; n2 < M2; n2++) for (int n1 = 0; n1 < M1; n1++) {
         double kx = wavenum(n1, M1, g->dxa), ky = wavenum(n2, M2, g->dya), kh = sqrt(kx * kx + ky * ky);
         double ka = comp == 0 ? kx : ky, da = comp == 0 ? g->dxa : g->dya;

@@ -8,8 +8,14 @@ receiver stencils and the check set: pointwise identical values, see test_conver
     python tests/golden/make_goldens.py cfg2            # ~15 min on 8 cores
     python tests/golden/make_goldens.py cfg3 0 100        # configs[2] with aux_dx = 100 m, to convergence: ~50 min
     python tests/golden/make_goldens.py cfg4 300 100      # configs[3] with aux_dx = 100 m, 300 fixed steps: ~50 min
+    python tests/golden/make_goldens.py cfg4 3000 0 fields 1000,2000   # configs[3] as bench.py times it (default auxiliary
+                                                          # plane, 3125 x 3125), 3000 fixed steps, field planes: ~4.5 h on 8 cores
 
 Output: tests/golden/<name>_converged[_aux<dx>].json or <name>_<n>steps[_aux<dx>].json with the inputs' SHA-256, nsteps, delta and the complex receivers.
+With `fields` also <name>_<n>steps[_aux<dx>]_fields.npz at every listed checkpoint and at the last step: the six time-domain
+fields (float32 roundings of the oracle's fp64 values) on whole z planes -- the ghost plane above the surface that the
+air-water boundary writes, the surface plane, the plane below it, the plane nearest the seabed -- and on the x-z slice
+through the source, the L2 norm of every z plane of every field (fp64), and the partial Green's functions at the receivers.
 """
 import hashlib
 import json
@@ -38,6 +44,31 @@ def input_hash(w):
     return h.hexdigest()
 
 
+def save_fields(g, w, name, nsteps, aux_dx, t0):
+    """field planes + per-plane norms + receivers of the run in progress (oracle values only)"""
+    info = g.info()
+    out, ns = g.run_end()
+    assert int(ns[0]) == nsteps
+    k0 = info["k0"]
+    z = g.coords(2)
+    ksea = int(np.argmin(np.abs(z[:info["N3"]] - 1000.0)))
+    y = g.coords(1)
+    jsrc = int(np.argmin(np.abs(y[:info["N2"]] - w["sources"][0][0][1])))
+    planes = [k0 - 1, k0, k0 + 1, ksea]
+    res = {"planes_k": np.array(planes), "slice_j": np.array(jsrc), "nsteps": np.array(nsteps), "dt": np.array(info["dt"]),
+           "dims": np.array([info["N3"], info["N2"], info["N1"]]), "aux": np.array([info["aux_M1"], info["aux_M2"]]),
+           "receivers": out[0], "sha256": np.array(input_hash(w)), "seconds": np.array(time.time() - t0),
+           "written_by": np.array("tests/golden/make_goldens.py %s (oracle only)" % " ".join(sys.argv[1:]))}
+    for c in ("E1", "E2", "E3", "H1", "H2", "H3"):
+        f = g.get(c)
+        res["norm_" + c] = np.sqrt((f * f).sum(axis=(1, 2)))
+        res["planes_" + c] = f[planes].astype(np.float32)
+        res["slice_" + c] = f[:, jsrc, :].astype(np.float32)
+    suffix = "_%dsteps" % nsteps + ("_aux%g" % aux_dx if aux_dx else "") + "_fields.npz"
+    np.savez_compressed(os.path.join(HERE, name + suffix), **res)
+    print("wrote", name + suffix, flush=True)
+
+
 def main():
     name = sys.argv[1]
     kw = {}
@@ -53,12 +84,16 @@ def main():
     opts["sparse_dft"] = 1
     if fixed:
         opts = dict(fixed_steps=fixed, sparse_dft=1)
+    fields = len(sys.argv) > 4 and sys.argv[4] == "fields"
+    marks = sorted(int(v) for v in sys.argv[5].split(",")) if len(sys.argv) > 5 else []
     t = time.time()
     g.run_begin(w["sources"][:1], w["freqs"], w["receivers"], opts)
     done, ns = False, [0]
     while not done:
         ns, done = g.run_steps(100)
         print("steps", int(ns[0]), "delta", g.get("DELTA"), "elapsed %.0f s" % (time.time() - t), flush=True)
+        if fields and (int(ns[0]) in marks or done):
+            save_fields(g, w, name, int(ns[0]), aux_dx, t)
     out, ns = g.run_end()
     res = {"name": name, "sha256": input_hash(w), "info": g.info(), "opts": opts, "nsteps": int(ns[0]),
            "delta": [float(v) for v in g.get("DELTA")], "seconds": time.time() - t,
