@@ -48,6 +48,10 @@ typedef struct {
   double cfl;    /* dt = cfl/eta (Eq. 15-16); <=0 => 0.99                                        */
   double aux_dx; /* spacing of the auxiliary uniform plane used by the air boundary when x-y is
                     non-uniform (L288); <=0 => smallest horizontal spacing                             */
+  int air_route; /* air boundary on a non-uniform x-y grid: 0 = separable route (interpolation and transform one
+                    axis at a time, batched 1-D transforms; default), 1 = plane-sized route (interpolate to the whole
+                    auxiliary plane, 2-D transforms): the same linear map up to rounding order, about twice the
+                    work; kept as the cross-check of the separable route.  Ignored on uniform x-y.              */
 } emm_grid_opts;
 
 typedef struct {

@@ -164,6 +164,7 @@ extern "C" int emm_grid_create(const double *x, int nx1, const double *y, int ny
   g->w0 = 2 * kPi * g->f0;
   g->cfl = o->cfl > 0 ? o->cfl : 0.99;                           // L260
   g->aux_dx = o->aux_dx;
+  g->air_route = o->air_route;
   const int r = g->r, nbe = g->nb + g->ne;
   if (g->ne < r) { delete g; return fail(EMM_EINVAL, "emm_grid_create: ne must be >= rd (L686)"); }
   g->uniform_xy = uniform_axis(x, nx1) && uniform_axis(y, ny1);

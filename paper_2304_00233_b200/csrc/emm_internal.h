@@ -3,6 +3,7 @@
 // Host side keeps everything in double (grid, FD tables, CPML, wavelet, twiddles, Eq. 7); the device
 // holds fp32 fields/accumulators.  Citations are PAPER.md line numbers; [Rn] = DESIGN.md readings.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cufft.h>
 
@@ -94,13 +95,17 @@ struct DevTables {             // device pointers of the per-grid region
   void *fft_ws[3];
 };
 
+// TMA descriptors of one accumulator-free update kernel (emm_tile.cu): the three stencil fields with the halo each one
+// needs, the three updated fields, dt/eps (E kernel only).  Passed to the kernel by value (__grid_constant__).
+struct TileMaps { CUtensorMap A1, A2, A3, U1, U2, U3, C1, C2, C3; };
+
 struct Run;
 
 }  // namespace emm
 
 struct emm_grid {
   // options
-  int r = 1, nb = 0, ne = 0, top = 0;
+  int r = 1, nb = 0, ne = 0, top = 0, air_route = 0;
   double f0 = 1, w0 = 0, cfl = 0.99, aux_dx = 0;
   int nc[3] = {0, 0, 0}, N[3] = {0, 0, 0}, lo[3] = {0, 0, 0};
   std::vector<double> xn[3], xh[3];      // padded nodes [N+1], half nodes [N]
@@ -136,6 +141,11 @@ struct emm_grid {
   int sp_nsrc = 0;                       // number of sources the plans in sp[] are batched for
   double vref[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // CPML reference speed per face [R5]
   emm::Run *run = nullptr;
+  // tile pipeline of the accumulator-free update (emm_tile.cu): descriptors of the current run's field rings
+  bool tile_ok = false;
+  emm::TileMaps tile_maps[2];            // [0] E kernel, [1] H kernel
+  const float *tile_base[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // buffer 0 of the E / H rings
+  long long tile_hstride = 1;
   long long launches = 0;
   // optional per-kernel timing of the two fused update kernels (CUDA events on the bound stream)
   bool prof = false;

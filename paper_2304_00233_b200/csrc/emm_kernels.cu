@@ -16,56 +16,9 @@
 #include <algorithm>
 #include <cstdlib>
 
-#include "emm_kernels.cuh"
+#include "emm_device.cuh"
 
 namespace emm {
-
-__device__ __forceinline__ float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
-__device__ __forceinline__ void st4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
-__device__ __forceinline__ float4 ldcs4(const float *p) { return __ldcs(reinterpret_cast<const float4 *>(p)); }
-__device__ __forceinline__ void stcs4(float *p, float4 v) { __stcs(reinterpret_cast<float4 *>(p), v); }
-__device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
-__device__ __forceinline__ float4 fma4(float a, float4 b, float4 c) {
-  return make_float4(fmaf(a, b.x, c.x), fmaf(a, b.y, c.y), fmaf(a, b.z, c.z), fmaf(a, b.w, c.w));
-}
-__device__ __forceinline__ float4 sub4(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
-__device__ __forceinline__ float4 add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
-
-// slab index along an axis of length N (L317-333): low slab i < nb -> i, high slab -> nb + (N-1-i)
-__device__ __forceinline__ int slab_of(int i, int N, int nb, int has_lo) {
-  if (i < nb) return has_lo ? i : -1;
-  if (i > N - 1 - nb) return nb + (N - 1 - i);
-  return -1;
-}
-
-// x derivative of 4 nodes from a 12-wide window w[] holding nodes i0-4 .. i0+7; tap m of node n sits at
-// i0+n-R+XO+m, i.e. window slot 4+n-R+XO+m.
-template <int R, int XO>
-__device__ __forceinline__ float4 ddx(const float (&w)[12], const float (&cx)[4][2 * R]) {
-  float d[4];
-#pragma unroll
-  for (int n = 0; n < 4; ++n) {
-    float acc = 0.f;
-#pragma unroll
-    for (int m = 0; m < 2 * R; ++m) acc = fmaf(cx[n][m], w[4 + n - R + XO + m], acc);
-    d[n] = acc;
-  }
-  return make_float4(d[0], d[1], d[2], d[3]);
-}
-
-__device__ __forceinline__ void window(float (&w)[12], float4 l, float4 c, float4 r) {
-  w[0] = l.x; w[1] = l.y; w[2] = l.z; w[3] = l.w;
-  w[4] = c.x; w[5] = c.y; w[6] = c.z; w[7] = c.w;
-  w[8] = r.x; w[9] = r.y; w[10] = r.z; w[11] = r.w;
-}
-
-// CPML recursion on a quad: psi <- b psi + a D ; D <- D + psi  (Eq. 22-23 with kappa = 1, L317-333)
-__device__ __forceinline__ void cpml4(float *psi, float a, float b, float4 &D) {
-  float4 p = ld4(psi);
-  p = make_float4(fmaf(b, p.x, a * D.x), fmaf(b, p.y, a * D.y), fmaf(b, p.z, a * D.z), fmaf(b, p.w, a * D.w));
-  st4(psi, p);
-  D = add4(D, p);
-}
 
 // DTFT of 4 nodes of one component into NF accumulators (Eq. 25): F[f] += u * tw[f]
 template <int NF>
@@ -102,22 +55,6 @@ __device__ __forceinline__ void dtft4_rt(float2 *F0, size_t fstride, float4 u, c
   }
 }
 
-#ifndef EMM_MINB
-#define EMM_MINB 0   /* 0 = choose per instantiation, see update_min_blocks */
-#endif
-#ifndef EMM_PF
-#define EMM_PF 1
-#endif
-#ifndef EMM_CXS
-#define EMM_CXS 1   /* accumulator-free instance: x coefficients in private shared-memory slots instead of registers */
-#endif
-#ifndef EMM_HOIST
-#define EMM_HOIST 1
-#endif
-#ifndef EMM_CPA
-#define EMM_CPA 1
-#endif
-__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // 16-byte asynchronous global->shared copy (LDGSTS): no register is held while it is in flight.  `.ca` on purpose:
 // the two 16-byte halves of a thread's 32-byte accumulator quad are fetched by two instructions that touch the
 // same sectors; through L1 the second one hits, with `.cg` (L1 bypass) every sector is pulled from L2 twice
@@ -207,7 +144,7 @@ __device__ __forceinline__ void dtft4_staged2(const float4 *sm, int c, float2 *F
 // Blocks per SM the register allocation is aimed at.  Measured on B200 (profiles/r1_kernel_experiments.md): with
 // many frequencies (>= 4: 48+ KB of staged accumulators per block) two fat blocks per SM win -- no register cap,
 // and the unified L1 keeps ~100 KB for the neighbour rows; with fewer frequencies three blocks win.
-template <int NF> constexpr int update_min_blocks() { return EMM_MINB > 0 ? EMM_MINB : (NF >= 4 ? 2 : 3); }
+template <int NF> constexpr int update_min_blocks() { return NF >= 4 ? 2 : 3; }
 
 // PAIR: the closing pass of a DTFT group (NF >= 1, staged).  The H kernel of step `it` holds old H
 // (term it) and new H (term it+1), the E kernel of step `it` old E (term it-1) and new E (term it) [R6]; with `harg` = nh
@@ -248,7 +185,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
   // x coefficients of the thread's 4 nodes.  The accumulator-free instance (register-capped at 3 blocks per SM) parks them
   // in private shared-memory slots and re-reads them where the x derivatives are formed (LDS.128, no bank conflicts:
   // slot q of thread t at [q*128 + t]); that frees 8R registers for loads in flight.
-  constexpr bool CXS = (EMM_CXS != 0) && (NF == 0);
+  constexpr bool CXS = NF == 0;
   constexpr int NCX = (8 * R + 3) / 4;                 // float4 slots for 4 nodes x 2R coefficients
   extern __shared__ float4 sm_dyn[];
   float4 *smC = sm_dyn + (threadIdx.y * blockDim.x + threadIdx.x);
@@ -310,7 +247,7 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     q2[m] = ld4(A2 + o);
   }
 
-  constexpr bool STAGED = (EMM_CPA != 0) && (NF > 0);
+  constexpr bool STAGED = NF > 0;
   static_assert(!PAIR || STAGED, "the closing pass of a DTFT group needs staged accumulators");
   float4 *smF = smC;                                   // DTFT instances: the dynamic shared memory holds the staged accumulators
   const size_t cstride = (size_t)g.NZB * g.PS;
@@ -347,7 +284,6 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 
   for (int k = kbeg; k < kend; ++k) {
     const size_t c0 = (size_t)k * g.PS + row;
-#if EMM_PF
     // pull the next plane's streaming operands into L2 while this plane is being worked on (no registers held)
     if (k + 1 < kend) {
       const size_t c1 = c0 + g.PS;
@@ -369,7 +305,6 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
         }
       }
     }
-#endif
 #pragma unroll
     for (int m = 0; m < 2 * R - 1; ++m) { q1[m] = q1[m + 1]; q2[m] = q2[m + 1]; }
     {
@@ -380,13 +315,11 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
     float cz[2 * R];
 #pragma unroll
     for (int m = 0; m < 2 * R; ++m) cz[m] = __ldg(tz + (size_t)k * 2 * R + m);
-#if EMM_HOIST
     // issue the loads of the fields being updated (and dt/eps) together with the stencil loads: one dependent
     // memory round trip per plane instead of two
     float4 u1 = ld4(U1 + c0), u2 = ld4(U2 + c0), u3 = ld4(U3 + c0);
     float4 e1 = zero4(), e2 = zero4(), e3 = zero4();
     if (!IS_H) { e1 = ld4(g.ce[0] + c0); e2 = ld4(g.ce[1] + c0); e3 = ld4(g.ce[2] + c0); }
-#endif
     const float4 a1c = q1[R - O], a2c = q2[R - O];      // plane k of A1, A2
     const float4 a3c = ld4(A3 + c0);
 
@@ -452,11 +385,6 @@ __global__ void __launch_bounds__(128, update_min_blocks<NF>()) k_update(const D
 
     // curl (L338-346)
     const float4 c1 = sub4(D2A3, D3A2), c2 = sub4(D3A1, D1A3), c3 = sub4(D1A2, D2A1);
-#if !EMM_HOIST
-    float4 u1 = ld4(U1 + c0), u2 = ld4(U2 + c0), u3 = ld4(U3 + c0);
-    float4 e1 = zero4(), e2 = zero4(), e3 = zero4();
-    if (!IS_H) { e1 = ld4(g.ce[0] + c0); e2 = ld4(g.ce[1] + c0); e3 = ld4(g.ce[2] + c0); }   // 0 where not updated
-#endif
     const bool dft = dft_xy && k >= g.blo[2] && k <= g.bhi[2];
     float2 *Fk = Fsrc + (size_t)(k - g.blo[2]) * g.PS + row;
     // one component: wait for its staged accumulators, add u * twiddle, stream out, refill the slots for plane k+1
@@ -681,17 +609,21 @@ template <int R, int NF, bool IS_H, bool PAIR = false>
 static void launch_one(const DevGrid &dg, const DevState &s, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel, int harg) {
   // staged accumulators + (grouped DTFT) the history quads of the levels this pass takes: sized per launch, so that a
   // small group does not pay shared memory (= L1) for the largest one
-  const size_t smem = EMM_CPA ? (size_t)(3 * NF * 2 + (PAIR ? 3 * harg : 0)) * 128 * sizeof(float4) : 0;
-  const size_t smem_max = EMM_CPA ? (size_t)(3 * NF * 2 + (PAIR ? 3 * kNHS : 0)) * 128 * sizeof(float4) : 0;
-  static bool configured = false;
-  if (!configured && smem_max > 48 * 1024) {
-    cudaFuncSetAttribute(k_update<R, NF, IS_H, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-    configured = true;
+  const size_t smem = (size_t)(3 * NF * 2 + (PAIR ? 3 * harg : 0)) * 128 * sizeof(float4);
+  const size_t smem_max = (size_t)(3 * NF * 2 + (PAIR ? 3 * kNHS : 0)) * 128 * sizeof(float4);
+  if (smem_max > 48 * 1024) {
+    // the attribute belongs to the (function, device) pair: one bit per device ordinal, set on first use there
+    static unsigned long long configured = 0;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev >= 64 || !(configured >> dev & 1)) {
+      cudaFuncSetAttribute(k_update<R, NF, IS_H, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+      if (dev < 64) configured |= 1ull << dev;
+    }
   }
   k_update<R, NF, IS_H, PAIR><<<grid, block, smem, st>>>(dg, s, kc, nchunks, chunk0, sel, harg);
 }
 
-#if EMM_CPA
 // two-term instances of the paired DTFT (1..kPairMaxNF frequencies)
 template <int R, bool IS_H>
 static void launch_update_pair(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int harg) {
@@ -703,12 +635,11 @@ static void launch_update_pair(const DevGrid &dg, const DevState &s, int nf, dim
     default: launch_one<R, 5, IS_H, true>(dg, s, grid, block, st, kc, nchunks, chunk0, 0, harg); break;
   }
 }
-#endif
 
 template <int R, bool IS_H>
 static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 grid, dim3 block, cudaStream_t st, int kc, int nchunks, int chunk0, int sel, int harg) {
   switch (nf) {
-    case 0: k_update<R, 0, IS_H><<<grid, block, EMM_CXS ? (size_t)2 * R * 128 * sizeof(float4) : 0, st>>>(dg, s, kc, nchunks, chunk0, sel, harg); break;
+    case 0: k_update<R, 0, IS_H><<<grid, block, (size_t)2 * R * 128 * sizeof(float4), st>>>(dg, s, kc, nchunks, chunk0, sel, harg); break;
     case 1: launch_one<R, 1, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
     case 2: launch_one<R, 2, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
     case 3: launch_one<R, 3, IS_H>(dg, s, grid, block, st, kc, nchunks, chunk0, sel, -1); break;
@@ -729,15 +660,25 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
   const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
   // launch one instance (nf = accumulators it is compiled for) over the chunks of `part`
   auto launch = [&](int nf, int sel, bool pair = false) -> int {
+    if (nf == 0 && !pair && g->tile_ok) {
+      // accumulator-free instance: the TMA tile pipeline (emm_tile.cu), same z-chunk scheme with its own tile shape
+      int tx, ty, kc = 16;
+      tile_dims(&tx, &ty);
+      const long long xy = (long long)((dg.N1 + tx - 1) / tx) * ((dg.N2 + ty - 1) / ty) * s.nsrc;
+      while (kc > 4 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;
+      const int nall = (nk + kc - 1) / kc, nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);
+      const int chunk0 = part == 2 ? nsurf : 0, nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
+      if (nchunks <= 0) return 0;
+      const int rc = launch_tile(g, s, is_h, kc, nchunks, chunk0, sel, st);
+      if (rc) return rc;
+      EMM_LAUNCH_CHECK(g, is_h ? "k_tile<H>" : "k_tile<E>");
+      return 0;
+    }
     // block: TX quads wide, 128 threads.  With accumulators: 16 or 32 quads, whichever wastes fewer lanes (long
     // contiguous accumulator rows); without: 8 quads x 16 rows, more y reuse in L1 (profiles/r1_kernel_experiments.md)
     int TX = 16;
     if (((quads + 31) / 32) * 32 <= ((quads + 15) / 16) * 16) TX = 32;
     if (nf == 0 || quads <= 8) TX = 8;
-    {
-      static const char *env_tx = getenv("EMM_TX");        // tuning knob: quads per block row (8, 16, 32)
-      if (env_tx && atoi(env_tx) > 0) TX = atoi(env_tx);
-    }
     const int TY = 128 / TX;
     // planes per z chunk: 16 on large grids; fewer on small ones so that the grid still holds ~8 blocks per SM
     // (each block marches its planes one after the other, so a sparse grid is latency-bound)
@@ -745,10 +686,6 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
     {
       const long long xy = (long long)((quads + TX - 1) / TX) * ((dg.N2 + TY - 1) / TY) * s.nsrc;
       while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 8) kc /= 2;
-    }
-    {
-      static const char *env_kc = getenv("EMM_KC");        // tuning knob: planes per z chunk
-      if (env_kc && atoi(env_kc) > 0) kc = atoi(env_kc);
     }
     const int nall = (nk + kc - 1) / kc;
     const int nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);        // chunks whose stencils reach the ghost planes
@@ -758,7 +695,6 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
     dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
     if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
     if (pair) {
-#if EMM_CPA
       if (is_h) {
         if (dg.r == 1) launch_update_pair<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
         else if (dg.r == 2) launch_update_pair<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
@@ -768,9 +704,6 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
         else if (dg.r == 2) launch_update_pair<2, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
         else launch_update_pair<3, false>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, harg);
       }
-#else
-      return fail(EMM_EINVAL, "launch_update: paired DTFT needs the staged accumulators (EMM_CPA)");
-#endif
     } else if (is_h) {
       if (dg.r == 1) launch_update_nf<1, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);
       else if (dg.r == 2) launch_update_nf<2, true>(dg, s, nf, grid, block, st, kc, nchunks, chunk0, sel, sel == 3 ? harg : -1);

@@ -40,6 +40,10 @@ struct DevRun {
 // mode: 0 = one DTFT term per step; paired DTFT: 1 = accumulator-free step of this kernel, 2 = its two-term step
 // harg: mode 2 = number of history levels (earlier buffers of the ring) the closing pass takes; unused otherwise
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st);
+// tile pipeline of the accumulator-free update (emm_tile.cu): descriptors for a run's field rings; one launch over z chunks
+int tile_make_maps(emm_grid *g, const DevState &s);
+int launch_tile(emm_grid *g, const DevState &s, int is_h, int kc, int nchunks, int chunk0, int sel, cudaStream_t st);
+void tile_dims(int *tx, int *ty);
 constexpr int kPairMaxNF = 5;       // grouped-DTFT instances exist for 1..5 frequencies (the staged, unrolled ones)
 #ifndef EMM_GROUP_MAX
 #define EMM_GROUP_MAX 8

@@ -48,10 +48,9 @@ static size_t vol(const emm_grid *g) { return (size_t)g->P1 * g->N[1] * g->N[2];
 // cuFFT plans of the air boundary; their work areas are carved from the caller's workspace
 static int ensure_plans(emm_grid *g) {
   if (g->top != EMM_TOP_AIR || g->have_plans) return 0;
-  // non-uniform x-y: separable route with batched 1-D transforms (EMM_AIR_PLANE=1 keeps the plane-sized 2-D
-  // transforms, for A/B measurements)
-  const char *force = std::getenv("EMM_AIR_PLANE");
-  g->sep_air = !g->uniform_xy && !(force && force[0] == '1');
+  // non-uniform x-y: separable route with batched 1-D transforms (emm_air_sep.cu) unless the grid asks for the
+  // plane-sized one (emm_grid_opts.air_route)
+  g->sep_air = !g->uniform_xy && g->air_route != 1;
   if (g->sep_air) {             // its plans are batched over the sources of a run: made by emm_workspace_bytes / emm_run_begin
     g->have_plans = true;
     return 0;
@@ -411,7 +410,6 @@ static std::complex<double> source_spectrum(const emm_grid *g, const Run *R, int
 static int enqueue_steps_raw(emm_grid *g, int n) {
   Run *R = g->run;
   int rc;
-  static const bool no_overlap = getenv("EMM_NO_OVERLAP") != nullptr;
   int gpos = 0, gsize = 0;                   // grouped DTFT: position in / size of the current group of steps
   for (int q = 0; q < n; ++q) {
     if (R->it_host >= R->table_steps) return fail(EMM_EINVAL, "run: step %d beyond the twiddle table (max_steps)", R->it_host);
@@ -462,8 +460,8 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       if ((rc = launch_check_acc(g, s2, R->dr))) return rc;                // check-set part of L483
       if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
       if ((rc = launch_update(g, s2, 1, 0, mh, hh, M))) return rc;                 // H part of L483 + L486-489
-    } else if (g->prof || no_overlap) {
-      // one thing after the other (per-kernel timing, or EMM_NO_OVERLAP): the boundary still runs on its own stream
+    } else if (g->prof) {
+      // one thing after the other (per-kernel timing): the boundary still runs on its own stream
       if ((rc = launch_update(g, s1, 0, 0, me, he, M))) return rc;
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));
       if ((rc = launch_air(g, s2, R->dr, 0, B))) return rc;                // L481
@@ -508,10 +506,9 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
 static int enqueue_steps(emm_grid *g, int n) {
   Run *R = g->run;
   int rc;
-  static const bool no_graph = getenv("EMM_NO_GRAPH") != nullptr;
   while (n > 0) {
     const int ce = R->check_every;
-    const bool whole = !no_graph && !g->prof && !R->graph_failed && R->it_host >= ce && R->it_host % ce == 0 && n >= ce && R->it_host + ce <= R->table_steps;
+    const bool whole = !g->prof && !R->graph_failed && R->it_host >= ce && R->it_host % ce == 0 && n >= ce && R->it_host + ce <= R->table_steps;
     if (!whole) {
       const int m = std::min(n, ce - R->it_host % ce);
       if ((rc = enqueue_steps_raw(g, m))) return rc;
@@ -585,11 +582,8 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
     R->dtft_every = o->dtft_every > 1 ? o->dtft_every : 1;
     R->sparse = o->sparse_dft != 0 && nf > 0;
     {
-      static const bool no_pair = getenv("EMM_NO_PAIR") != nullptr;       // A/B measurements
-      const bool can = o->dtft_pair >= 0 && !no_pair && nf >= 1 && nf <= kPairMaxNF && !R->sparse && o->dtft_every >= 0 && o->dtft_every <= 1;
-      static const char *env_group = getenv("EMM_DTFT_GROUP");             // A/B measurements: default group size
-      const int dflt = env_group && atoi(env_group) >= 2 ? atoi(env_group) : default_dtft_group(nf);
-      R->group = !can ? 1 : std::min(kGroupMax, o->dtft_pair >= 2 ? o->dtft_pair : dflt);
+      const bool can = o->dtft_pair >= 0 && nf >= 1 && nf <= kPairMaxNF && !R->sparse && o->dtft_every >= 0 && o->dtft_every <= 1;
+      R->group = !can ? 1 : std::min(kGroupMax, o->dtft_pair >= 2 ? o->dtft_pair : default_dtft_group(nf));
     }
     if (R->check_set < 0 || R->check_set > 2) { free_run(g); return fail(EMM_EINVAL, "emm_run_begin: bad check_set"); }
     R->table_steps = (R->fixed_steps ? R->fixed_steps : R->max_steps) + 1;
@@ -661,6 +655,7 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
           return fail(EMM_ECUDA, "cufftSetStream/cufftSetWorkArea failed");
         }
     R->ds.dft_every = R->dtft_every;
+    if (!A.overflow && (rc = tile_make_maps(g, R->ds))) { free_run(g); return rc; }
     if (A.overflow) { size_t need = A.off; free_run(g); return fail(EMM_ENOMEM, "emm_run_begin: workspace too small (%zu bytes needed)", need); }
     // zero the whole run region (fields, psi, accumulators, flags)
     CU(cudaMemsetAsync(static_cast<char *>(g->d_ws) + g->fixed_bytes, 0, A.off - g->fixed_bytes, g->stream));

@@ -11,9 +11,9 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.environ.get("EMM_B200_LIB") or os.path.join(_HERE, "libemm_b200.so")   # override: kernel-variant experiments
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu")]
-_HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh")] + \
+_SO = os.path.join(_HERE, "libemm_b200.so")
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu")]
+_HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh", "emm_device.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
 
 TOP_CPML, TOP_AIR = 0, 1
@@ -34,8 +34,6 @@ SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_dipole_direction", "emm_receiver
 def build(force=False, verbose=False):
     """nvcc -> libemm_b200.so in-tree, sm_100a only."""
     deps = _SRC + _HDR
-    if os.environ.get("EMM_B200_LIB"):
-        return _SO                       # an explicitly chosen (experiment) library is used as it is
     if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(os.path.getmtime(p) for p in deps):
         return _SO
     cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
@@ -48,7 +46,7 @@ def build(force=False, verbose=False):
 
 class GridOpts(C.Structure):
     _fields_ = [("rd", C.c_int), ("nb", C.c_int), ("ne", C.c_int), ("top", C.c_int),
-                ("f0", C.c_double), ("cfl", C.c_double), ("aux_dx", C.c_double)]
+                ("f0", C.c_double), ("cfl", C.c_double), ("aux_dx", C.c_double), ("air_route", C.c_int)]
 
 
 class Src(C.Structure):
@@ -175,9 +173,9 @@ def _ropts(o):
 class Grid:
     """emm_grid handle + the torch workspace it is bound to."""
 
-    def __init__(self, x, y, z, rd, nb, ne=-1, top=TOP_CPML, f0=1.0, cfl=0.99, aux_dx=0.0):
+    def __init__(self, x, y, z, rd, nb, ne=-1, top=TOP_CPML, f0=1.0, cfl=0.99, aux_dx=0.0, air_route=0):
         x, y, z = (np.ascontiguousarray(v, dtype=np.float64) for v in (x, y, z))
-        o = GridOpts(rd, nb, ne, top, f0, cfl, aux_dx)
+        o = GridOpts(rd, nb, ne, top, f0, cfl, aux_dx, air_route)
         h = C.c_void_p()
         _chk(lib().emm_grid_create(_dptr(x), len(x), _dptr(y), len(y), _dptr(z), len(z), C.byref(o), C.byref(h)))
         self._h = h

@@ -289,21 +289,19 @@ def test_grouped_dtft_takes_the_largest_group_the_workspace_allows(emm):
     assert e.value.code == emm.ENOMEM
 
 
-def test_plane_and_separable_air_routes_agree(emm, oracle, monkeypatch):
+def test_plane_and_separable_air_routes_agree(emm, oracle):
     """Non-uniform x-y: the separable route (batched 1-D transforms, default) and the plane-sized 2-D route
-    (EMM_AIR_PLANE=1) are the same linear map up to rounding order; both are within the field tolerance of the oracle."""
+    (emm_grid_opts.air_route = 1) are the same linear map up to rounding order; both are within the field tolerance of the oracle."""
     w = W.cfg4(oracle.nugrid, nx=40, nz=36, rd=3, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
     w["receivers"] = _small_receivers()
     fields = {}
     for route in ("0", "1"):
-        monkeypatch.setenv("EMM_AIR_PLANE", route)
-        g = make_grid(emm, w)
+        g = make_grid(emm, w, air_route=int(route))
         g.run_begin(w["sources"], w["freqs"], w["receivers"], dict(fixed_steps=150))
         g.run_steps(150)
         fields[route] = [g.get(c) for c in ("E1", "E2", "E3", "H1", "H2", "H3")]
         g.run_end()
         g.close()
-    monkeypatch.delenv("EMM_AIR_PLANE")
     for a, b in zip(fields["0"], fields["1"]):
         assert np.abs(a).max() > 0
     ne = np.sqrt(sum(np.sum(np.asarray(a, np.float64) ** 2) for a in fields["0"][:3]))
