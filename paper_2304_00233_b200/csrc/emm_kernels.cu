@@ -665,7 +665,7 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
       int tx, ty, kc = 16;
       tile_dims(&tx, &ty);
       const long long xy = (long long)((dg.N1 + tx - 1) / tx) * ((dg.N2 + ty - 1) / ty) * s.nsrc;
-      while (kc > 4 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;
+      while (kc > 4 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;        // kc <= 32 (kMaxKC of emm_tile.cu)
       const int nall = (nk + kc - 1) / kc, nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);
       const int chunk0 = part == 2 ? nsurf : 0, nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
       if (nchunks <= 0) return 0;

@@ -29,6 +29,8 @@ constexpr int WX = TX + 8;              // row length of a tile with one halo qu
 constexpr int NCONS = 128;              // consumer threads: 16 quads x 8 rows
 constexpr int NTHREADS = NCONS + 32;    // + the producer warp
 
+constexpr int kMaxKC = 32;              // most planes a block marches over
+
 constexpr int align128(int bytes) { return (bytes + 127) / 128 * 128; }
 
 template <int R, bool IS_H, int P>
@@ -42,7 +44,8 @@ struct TileLayout {
   static constexpr int TXA = TX * HY * 4 + WX * TY * 4;     // bytes the TMA unit delivers per stage (boxes, unpadded)
   static constexpr int TXB = WX * HY * 4 + NU * U_B;
   static constexpr int BAR_OFF = DA * STA_B + DB * STB_B;
-  static constexpr int SMEM = BAR_OFF + (2 * DA + 2 * DB) * 8 + 128;    // + slack to align the base to 128 bytes
+  static constexpr int CZ_OFF = BAR_OFF + (2 * DA + 2 * DB) * 8;        // z coefficients of the chunk: kMaxKC planes x 2R
+  static constexpr int SMEM = CZ_OFF + kMaxKC * 2 * R * 4 + 128;        // + slack to align the base to 128 bytes
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -55,31 +58,18 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned long long *b, unsigned b
 __device__ __forceinline__ void mbar_arrive(unsigned long long *b) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
+// try_wait suspends the thread in hardware until the phase completes or the time hint (ns) runs out, so a waiting
+// thread -- above all the producer, which mostly waits for a slot to come free -- leaves the issue slots alone
 __device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
       "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
       "@p bra WAIT_DONE;\n"
       "bra WAIT_LOOP;\n"
       "WAIT_DONE:\n"
-      "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
-}
-// the producer's waits (a slot coming free): poll with a short sleep in between, so that the spinning thread leaves the
-// issue slots of its scheduler to the consumer warps
-__device__ __forceinline__ void mbar_wait_backoff(unsigned long long *b, unsigned parity) {
-  unsigned done = 0;
-  while (true) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n" : "=r"(done) : "r"(smem_u32(b)), "r"(parity) : "memory");
-    if (done) break;
-    __nanosleep(64);
-  }
+      "}\n" ::"r"(smem_u32(b)), "r"(parity), "r"(200000u) : "memory");
 }
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, unsigned long long *bar, int c0, int c1, int c2, int c3) {
   asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
@@ -100,13 +90,10 @@ k_tile(const __grid_constant__ TileMaps tm, const DevGrid g, const DevState s, c
   using L = TileLayout<R, IS_H, P>;
   constexpr int O = L::O, DA = L::DA, DB = L::DB;
   const int src = blockIdx.z / nchunks, chunk = chunk0 + blockIdx.z - src * nchunks;
-  // every early exit is uniform over the block and comes before the barriers exist
-  if (s.done[src]) return;
+  // the two flags that can end the block early are requested together; their latency is covered by the barrier set-up
+  const int done = s.done[src], it = *s.it;
   const int kbeg = g.klo + chunk * kc;
   const int kend = min(kbeg + kc, g.N3 - R);
-  if (kbeg >= kend) return;
-  const int it = *s.it;
-  if ((sel == 1 || sel == 2) && ((sel == 2) != (it % s.dft_every == 0))) return;     // DTFT decimation, see k_update
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
   // 128-byte aligned base, by pointer arithmetic on the shared array itself (an integer round trip would turn every
@@ -122,6 +109,9 @@ k_tile(const __grid_constant__ TileMaps tm, const DevGrid g, const DevState s, c
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  // every early exit is uniform over the block and comes before the first copy is issued
+  if (done || kbeg >= kend) return;
+  if ((sel == 1 || sel == 2) && ((sel == 2) != (it % s.dft_every == 0))) return;     // DTFT decimation, see k_update
 
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int pA0 = kbeg - R + O;                      // first plane through ring A
@@ -136,7 +126,7 @@ k_tile(const __grid_constant__ TileMaps tm, const DevGrid g, const DevState s, c
         {
           const int q = qa, fill = fa;
           if (++qa == DA) { qa = 0; ++fa; }
-          if (fill > 0) mbar_wait_backoff(emptyA + q, (fill - 1) & 1);
+          if (fill > 0) mbar_wait(emptyA + q, (fill - 1) & 1);
           unsigned char *st = ringA + q * L::STA_B;
           mbar_expect_tx(fullA + q, L::TXA);
           tma_load_4d(st, &tm.A1, fullA + q, x0, y0 - R + O, pA0 + t, wA);
@@ -146,7 +136,7 @@ k_tile(const __grid_constant__ TileMaps tm, const DevGrid g, const DevState s, c
         if (b >= 0) {
           const int q = qb, fill = fb, k = kbeg + b;
           if (++qb == DB) { qb = 0; ++fb; }
-          if (fill > 0) mbar_wait_backoff(emptyB + q, (fill - 1) & 1);
+          if (fill > 0) mbar_wait(emptyB + q, (fill - 1) & 1);
           unsigned char *st = ringB + q * L::STB_B;
           mbar_expect_tx(fullB + q, L::TXB);
           tma_load_4d(st, &tm.A3, fullB + q, x0 - 4, y0 - R + O, k, wA);
@@ -177,7 +167,13 @@ k_tile(const __grid_constant__ TileMaps tm, const DevGrid g, const DevState s, c
   float *W3 = (Uo[2] ? Uo[2] : (IS_H ? s.H[2] : s.E[2])) + node0;
   const float *txc = IS_H ? g.cp[0] : g.cm[0];
   const float *tyc = IS_H ? g.cp[1] : g.cm[1];
-  const float *tzc = (IS_H ? g.cp[2] : g.cm[2]) + (size_t)kbeg * 2 * R;
+  // z coefficients of the chunk's planes into shared memory (one uniform LDS per tap and plane instead of a global load)
+  float *czs = reinterpret_cast<float *>(sm + L::CZ_OFF);
+  {
+    const float *tzc = (IS_H ? g.cp[2] : g.cm[2]) + (size_t)kbeg * 2 * R;
+    for (int q = tid; q < (kend - kbeg) * 2 * R; q += NCONS) czs[q] = __ldg(tzc + q);
+    asm volatile("bar.sync 1, %0;" ::"n"(NCONS) : "memory");      // consumer warps only
+  }
 
   float cx[4][2 * R], cy[2 * R];
 #pragma unroll
@@ -238,8 +234,8 @@ k_tile(const __grid_constant__ TileMaps tm, const DevGrid g, const DevState s, c
     // the CPML memory variables of the slab threads (one L2 round trip, all at once)
     float cz[2 * R];
 #pragma unroll
-    for (int m = 0; m < 2 * R; ++m) cz[m] = __ldg(tzc + m);
-    tzc += 2 * R;
+    for (int m = 0; m < 2 * R; ++m) cz[m] = czs[m];
+    czs += 2 * R;
     float px0[4] = {0.f, 0.f, 0.f, 0.f}, px1[4] = {0.f, 0.f, 0.f, 0.f};
     float4 py0 = zero4(), py1 = zero4(), pz0 = zero4(), pz1 = zero4();
     const int sk = valid ? slab_of(k, g.N3, g.nb, g.zslab_lo) : -1;
