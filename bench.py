@@ -190,7 +190,8 @@ def run_reference(args):
     gi = O.Grid(w_full["x"], w_full["y"], w_full["z"], **w_full["grid"]).info()
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "Gcell-updates/s", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": describe(w_full, gi, 1),
+            "dtype": "f64", "data": "synthetic",
+            "config": dict(describe(w_full, gi, 1), workload="%s; the oracle steps a bounded sample of this recipe: %s" % (describe(w_full, gi, 1)["workload"], desc)),
             "cpu_baseline": {"value": val, "unit": "Gcell-updates/s", "cores": cores, "kind": "oracle", "sample": desc,
                              "value_one_thread": getattr(oracle_rate, "one_thread", None)},
             "e2e": {"value": val, "unit": "Gcell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -332,6 +333,44 @@ def run_gpu(args):
         msr = d0.elapsed_time(d1)
         rec_only = {"ms_per_step": msr / K, "value": world * nsrc * N * K / (msr * 1e-3) / 1e9,
                     "note": "sparse_dft=1: same receiver outputs and step counts, no full-grid frequency-domain fields"}
+    # extra: configs[3] at 4th order (rd = 2), the order north_star's target sentence names for this grid
+    rd2 = None
+    if w["name"] == "cfg4" and w["grid"]["rd"] == 3 and args.scale == 1.0 and not args.no_rd2:
+        a2 = argparse.Namespace(**vars(args))
+        a2.rd = 2
+        w2 = build_workload(a2, emm.emm_nugrid)
+        g.close()
+        g2 = emm.Grid(w2["x"], w2["y"], w2["z"], **w2["grid"])
+        g2.bind(nsrc=1, nfreq=len(w2["freqs"]), max_steps=K + Wm + 8, nrec=len(w2["receivers"]), device=dev)
+        g2.model_set(w2["sigma_h"], w2.get("sigma_v"))
+        i2 = g2.info()
+        N2n = i2["N1"] * i2["N2"] * i2["N3"]
+        g2.run_begin(w2["sources"][:1], w2["freqs"], w2["receivers"], dict(fixed_steps=K + Wm + 4))
+        g2.run_enqueue(Wm)
+        torch.cuda.synchronize()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(g2.stream)
+        g2.run_enqueue(K)
+        d1.record(g2.stream)
+        torch.cuda.synchronize()
+        ms2 = d0.elapsed_time(d1)
+        g2.run_begin(w2["sources"][:1], w2["freqs"], w2["receivers"], dict(fixed_steps=Kp + Wm + 4))
+        g2.run_enqueue(Wm)
+        torch.cuda.synchronize()
+        g2.profile(True)
+        g2.run_enqueue(Kp)
+        torch.cuda.synchronize()
+        prof2 = g2.profile_read()
+        g2.profile(False)
+        grp2 = int(g2.get("DTFT_GROUP")[0])
+        g2.close()
+        nb2, nf2 = w2["grid"]["nb"], len(w2["freqs"])
+        t2 = sum(v[0] for v in prof2.values())
+        b2 = sum(algorithmic_bytes(i2, nf2, nb2, k, grp2) * v[1] for k, v in prof2.items() if v[1] > 0)
+        rd2 = {"workload": describe(w2, i2, 1)["workload"], "ms_per_step": ms2 / K, "value": world * N2n * K / (ms2 * 1e-3) / 1e9,
+               "kernels_ms_per_launch": {k: v[0] / v[1] for k, v in prof2.items() if v[1] > 0},
+               "instances_gbs": {k: algorithmic_bytes(i2, nf2, nb2, k, grp2) / (v[0] / v[1] * 1e-3) / 1e9 for k, v in prof2.items() if v[1] > 0},
+               "update_kernels_gbs_time_weighted": b2 / (t2 * 1e-3) / 1e9}
     batched = None
     if nsrc > 1:
         # configs[4]: the same K steps for ONE source alone = what running the sources one after the other costs
@@ -354,38 +393,47 @@ def run_gpu(args):
             peak, peak_src = float(json.load(open(peaks_file))["hbm_gbs"]), "of measured (MEASURED_PEAKS.json hbm_gbs)"
         else:
             peak, peak_src = 6650.0, "of fallback (B200_PROFILING.md)"
-        # instances of the update kernel in this run (paired DTFT: E0/H0 = accumulator-free steps, E2/H2 = two-term steps);
-        # the dominant one = the largest duration per launch
+        # instances of the update kernels in this run (grouped DTFT: E0/H0 = accumulator-free steps, the TMA tile pipeline
+        # k_tile; E2/H2 = the pass that closes a group).  `frac` is the time-weighted figure over ALL of them: the
+        # algorithmic bytes of every timed launch over the summed launch durations; `kernel` names the instance with the
+        # largest share of that time.
         avg = {k: v[0] / v[1] for k, v in prof.items() if v[1] > 0}
         mgrp = dtft_group
-        dom = max(avg, key=avg.get)
-        kms = avg[dom]
-        inst = {"E": "k_update<R,NF,E>", "H": "k_update<R,NF,H>", "E0": "k_update<R,0,E>", "H0": "k_update<R,0,H>",
+        inst = {"E": "k_update<R,NF,E>", "H": "k_update<R,NF,H>", "E0": "k_tile<R,E> (accumulator-free, TMA tile pipeline)",
+                "H0": "k_tile<R,H> (accumulator-free, TMA tile pipeline)",
                 "E2": "k_update<R,NF,E,PAIR> (closing pass of a DTFT group)", "H2": "k_update<R,NF,H,PAIR> (closing pass of a DTFT group)"}
-        abytes = nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], dom, mgrp)
-        achieved = abytes / (kms * 1e-3) / 1e9
+        nfq, nbq = len(w["freqs"]), w["grid"]["nb"]
+        ibytes = {k: nsrc * algorithmic_bytes(info, nfq, nbq, k, mgrp) for k in avg}
+        tot_update = sum(v[0] for v in prof.values())
+        tot_bytes = sum(ibytes[k] * prof[k][1] for k in avg)
+        share = {k: prof[k][0] / tot_update for k in avg}
+        dom = max(share, key=share.get)
+        achieved = tot_bytes / (tot_update * 1e-3) / 1e9
         traffic = None
         tf = os.path.join(ROOT, "profiles", "ncu_traffic.json")
         if os.path.exists(tf):
             traffic = json.load(open(tf)).get("%s:%s:rd%d:nf%d" % (w["name"], dom, w["grid"]["rd"], len(w["freqs"])))
-        tot_update = sum(v[0] for v in prof.values())
         roofline = {"bound": "hbm", "kernel": inst[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "algorithmic_bytes_per_launch": abytes,
-                    "kernel_ms": kms, "kernels_ms_per_launch": avg,
-                    "instances_gbs": {k: nsrc * algorithmic_bytes(info, len(w["freqs"]), w["grid"]["nb"], k, mgrp) / (avg[k] * 1e-3) / 1e9 for k in avg},
+                    "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic,
+                    "what": "time-weighted over every update-kernel launch of the serialised pass: sum of algorithmic bytes / sum of launch durations",
+                    "algorithmic_bytes_per_launch": ibytes[dom], "kernel_ms": avg[dom],
+                    "kernels_ms_per_launch": avg, "launches": {k: prof[k][1] for k in avg}, "share_of_update_time": share,
+                    "instances_gbs": {k: ibytes[k] / (avg[k] * 1e-3) / 1e9 for k in avg},
+                    "instances_frac": {k: ibytes[k] / (avg[k] * 1e-3) / 1e9 / peak for k in avg},
                     "dtft_group": mgrp,
                     "update_kernels_ms_per_step": tot_update / Kp,
                     "step_frac_in_update_kernels": tot_update / (ms_prof * Kp),
                     "ms_per_step_serialised": ms_prof,
-                    "how": "kernel_ms from a serialised pass (emm_profile); `value` is timed with the air-water boundary overlapped on a second stream"}
+                    "how": "launch durations from a serialised pass (emm_profile: CUDA events around each launch); `value` is timed with the air-water boundary overlapped on a second stream"}
         # whole step against the same peak: algorithmic bytes of the update kernels of one step (paired DTFT: half of the four
         # passes of a pair), boundary / check-set / injection bytes not counted, over the timed ms per step
-        nfq, nbq = len(w["freqs"]), w["grid"]["nb"]
         if "E2" in avg:      # a group of m steps: m-1 accumulator-free passes and one closing pass per kernel
             step_bytes = nsrc * sum((mgrp - 1) * algorithmic_bytes(info, nfq, nbq, k + "0", mgrp) + algorithmic_bytes(info, nfq, nbq, k + "2", mgrp)
                                     for k in ("E", "H")) / mgrp
         else:
             step_bytes = nsrc * (algorithmic_bytes(info, nfq, nbq, "E") + algorithmic_bytes(info, nfq, nbq, "H"))
+        if rd2:
+            rd2["update_kernels_frac_time_weighted"] = rd2["update_kernels_gbs_time_weighted"] / peak
         roofline["whole_step"] = {"algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / (ms / K * 1e-3) / 1e9,
                                   "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
                                   "note": "update-kernel bytes only, over the whole timed step (boundary, check set and injection included in the time)"}
@@ -402,7 +450,7 @@ def run_gpu(args):
                         "what": "emm_model_set (host sigma -> device) + emm_run(fixed_steps=K) (tables up, receivers back)"},
                 "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "batched": batched,
                 "dtft": ("every term of Eq. 25, %d consecutive terms per accumulator pass (emm_run_opts.dtft_pair, default)" % dtft_group) if dtft_group > 1 else "every term of Eq. 25, one per step",
-                "dtft_one_term_per_step": unpaired, "dtft_decimation": decim, "receivers_only_dtft": rec_only,
+                "dtft_one_term_per_step": unpaired, "dtft_decimation": decim, "receivers_only_dtft": rec_only, "rd2": rd2,
                 "multi_gpu": "replicas only: every rank runs the whole workload, no collective on the data path"}
         print(json.dumps(line))
     if world > 1:
@@ -450,6 +498,7 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the cell counts (debugging only)")
     ap.add_argument("--aux-dx", type=float, default=0.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-rd2", action="store_true", help="skip the extra 4th-order (rd = 2) run of configs[3]")
     ap.add_argument("--converge", action="store_true", help="time to converged in the four DTFT schedules instead of the step benchmark")
     args = ap.parse_args()
     if args.converge:

@@ -155,10 +155,12 @@ int emm_grid_fdcoef(const emm_grid *g, int axis, int plus, double *out /* [n?pad
 
 /* Device memory and stream (both owned by the caller, e.g. a torch uint8 tensor and the current torch
  * stream).  emm_workspace_bytes: bytes needed for nsrc simultaneously resident sources, nfreq
- * frequencies, up to max_steps steps and nrec receivers with check_set <= EMM_CHECK_FACES (0 on error).
+ * frequencies, up to max_steps steps and nrec receivers with check_set <= EMM_CHECK_FACES (0 on error), in either
+ * DTFT mode (full-grid accumulators with the field ring of the group `dtft_pair` stands for, see emm_run_opts, or
+ * receivers only).  The first call creates the grid's cuFFT plans, hence the non-const handle.
  * The workspace must be 256-byte aligned and stay alive while the grid is used; binding it uploads
  * the per-grid tables and invalidates any earlier model.                                             */
-size_t emm_workspace_bytes(const emm_grid *g, int nsrc, int nfreq, int max_steps, int nrec);
+size_t emm_workspace_bytes(emm_grid *g, int nsrc, int nfreq, int max_steps, int nrec, int dtft_pair);
 int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, void *cuda_stream);
 
 /* Per-cell conductivity [nz][ny][nx] (S/m, finite, >0); sigma_v NULL => isotropic (VTI otherwise, L43).

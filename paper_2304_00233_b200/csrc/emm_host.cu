@@ -21,26 +21,35 @@ int fail(int code, const char *fmt, ...) {
   return code;
 }
 
-// Solve V^T(x) a = f in place (Bjorck-Pereyra): Newton divided differences,
-// then conversion to monomial coefficients.  a enters as f.
-static void vandermonde_solve(std::vector<double> &a, const std::vector<double> &x) {
-  const int n = (int)x.size() - 1;
-  for (int k = 0; k < n; ++k)
-    for (int i = n; i > k; --i) a[i] = (a[i] - a[i - 1]) / (x[i] - x[i - k - 1]);
-  for (int k = n - 1; k >= 0; --k)
-    for (int i = k; i < n; ++i) a[i] -= a[i + 1] * x[k];
-}
-
-// Rows 0 and 1 of [V^T]^-1 built from offsets (node - x0): feed unit vectors (Eq. 12).
+// Interpolation (derivative order 0) and first-derivative weights of arbitrary nodes for the point x0 (Eq. 9-12).
+// The paper inverts the transposed Vandermonde matrix of the offsets (L127-146); the rows of that inverse are the
+// Taylor-matched weights, which Fornberg's recursion (Math. Comp. 51, 1988) builds directly, one node at a time, from
+// the Lagrange form -- a different construction of the same numbers (the oracle follows the paper's listing; a CPU
+// test holds the two against each other).  C[j][k] = weight of node j for derivative order k.
 void weights(const double *nodes, int npts, double x0, double *w0, double *w1) {
-  std::vector<double> off(npts), a(npts);
-  for (int i = 0; i < npts; ++i) off[i] = nodes[i] - x0;
+  double C[16][2];
+  for (int j = 0; j < npts; ++j) C[j][0] = C[j][1] = 0.0;
+  C[0][0] = 1.0;
+  double prod_prev = 1.0, off_new = nodes[0] - x0;
+  for (int i = 1; i < npts; ++i) {
+    const double off_prev = off_new;
+    off_new = nodes[i] - x0;
+    double prod = 1.0;
+    for (int j = 0; j < i; ++j) {
+      const double gap = nodes[i] - nodes[j];
+      prod *= gap;
+      if (j == i - 1) {                       // weights of the node that has just joined
+        C[i][1] = prod_prev * (C[i - 1][0] - off_prev * C[i - 1][1]) / prod;
+        C[i][0] = -prod_prev * off_prev * C[i - 1][0] / prod;
+      }
+      C[j][1] = (off_new * C[j][1] - C[j][0]) / gap;
+      C[j][0] = off_new * C[j][0] / gap;
+    }
+    prod_prev = prod;
+  }
   for (int j = 0; j < npts; ++j) {
-    std::fill(a.begin(), a.end(), 0.0);
-    a[j] = 1.0;
-    vandermonde_solve(a, off);
-    if (w0) w0[j] = a[0];
-    if (w1) w1[j] = a[1];
+    if (w0) w0[j] = C[j][0];
+    if (w1) w1[j] = C[j][1];
   }
 }
 
@@ -140,100 +149,131 @@ extern "C" int emm_fd_weights(int npts, const double *nodes, double x0, double *
   return 0;
 }
 
+namespace {
+
+struct AxisInput { const double *node; int ncell; };
+
+// [R1] One padded axis: `below` / `above` extra cells that continue the first / last spacing of the model, the half
+// nodes of [R2] (cell midpoints), and the two operator tables of Eq. 13-14 for every node that is ever updated.
+// Returns the largest absolute row sum of either operator (the D_max of Eq. 16).
+double pad_axis_and_tabulate(emm_grid *g, int a, const AxisInput &in, int below, int above, int r) {
+  const int N = in.ncell + below + above;
+  g->lo[a] = below;
+  g->N[a] = N;
+  std::vector<double> &xn = g->xn[a], &xh = g->xh[a];
+  xn.assign(N + 1, 0.0);
+  xh.assign(N, 0.0);
+  const double first = in.node[1] - in.node[0], last = in.node[in.ncell] - in.node[in.ncell - 1];
+  for (int i = 0; i < below; ++i) xn[i] = in.node[0] - (below - i) * first;
+  for (int c = 0; c <= in.ncell; ++c) xn[below + c] = in.node[c];
+  for (int i = 1; i <= above; ++i) xn[below + in.ncell + i] = in.node[in.ncell] + i * last;
+  for (int i = 0; i < N; ++i) xh[i] = xn[i] + 0.5 * (xn[i + 1] - xn[i]);
+  const int taps = 2 * r;
+  g->cm[a].assign((size_t)N * taps, 0.0);
+  g->cp[a].assign((size_t)N * taps, 0.0);
+  double worst = 0.0;
+  for (int i = r; i + r < N; ++i) {
+    // D- lives on the node x_i and reads the half nodes i-r .. i+r-1 (L212-236); D+ lives on the half node and reads the
+    // nodes i-r+1 .. i+r (Eq. 13)
+    double *minus = &g->cm[a][(size_t)i * taps], *plus = &g->cp[a][(size_t)i * taps];
+    weights(&xh[i - r], taps, xn[i], nullptr, minus);
+    weights(&xn[i - r + 1], taps, xh[i], nullptr, plus);
+    double sum_minus = 0.0, sum_plus = 0.0;
+    for (int q = 0; q < taps; ++q) { sum_minus += std::fabs(minus[q]); sum_plus += std::fabs(plus[q]); }
+    worst = std::max(worst, std::max(sum_minus, sum_plus));
+  }
+  return worst;
+}
+
+// [R10] auxiliary uniform plane of a non-uniform horizontal axis: spacing d from the first padded node, enough nodes to
+// reach past the last one, count rounded up to a 7-smooth transform length; 4-point Lagrange stencils in both
+// directions for the node lattice (l = 0) and the half-node lattice (l = 1)
+int plan_aux_axis(emm_grid *g, int a, double d) {
+  const double extent = g->xn[a][g->N[a]] - g->xn[a][0];
+  const int M = next_smooth7((int)std::floor(extent / d) + 2);
+  std::vector<double> aux(M);
+  for (int m = 0; m < M; ++m) aux[m] = g->xn[a][0] + m * d;
+  for (int l = 0; l < 2; ++l) {
+    const double *lattice = l ? g->xh[a].data() : g->xn[a].data();
+    g->toaux[a][l].resize(M);
+    g->fromaux[a][l].resize(g->N[a]);
+    for (int m = 0; m < M; ++m) make_stencil(lattice, g->N[a], aux[m], 4, 0, 0, true, &g->toaux[a][l][m]);
+    for (int i = 0; i < g->N[a]; ++i) make_stencil(aux.data(), M, lattice[i], 4, 0, 0, true, &g->fromaux[a][l][i]);
+  }
+  return M;
+}
+
+}  // namespace
+
 extern "C" int emm_grid_create(const double *x, int nx1, const double *y, int ny1, const double *z, int nz1,
                                const emm_grid_opts *o, emm_grid **out) {
   if (!x || !y || !z || !o || !out) return fail(EMM_EINVAL, "emm_grid_create: null argument");
   if (o->rd < 1 || o->rd > kMaxR) return fail(EMM_EINVAL, "emm_grid_create: rd must be 1, 2 or 3 (L684)");
   if (o->nb < 1) return fail(EMM_EINVAL, "emm_grid_create: nb must be >= 1");
   if (o->top != EMM_TOP_AIR && o->top != EMM_TOP_CPML) return fail(EMM_EINVAL, "emm_grid_create: bad top");
-  const double *u[3] = {x, y, z};
-  const int n1s[3] = {nx1, ny1, nz1};
+  const AxisInput in[3] = {{x, nx1 - 1}, {y, ny1 - 1}, {z, nz1 - 1}};
   for (int a = 0; a < 3; ++a) {
-    if (n1s[a] < 3) return fail(EMM_EINVAL, "emm_grid_create: need at least 2 cells per axis");
-    for (int i = 0; i + 1 < n1s[a]; ++i)
-      if (!std::isfinite(u[a][i]) || !std::isfinite(u[a][i + 1]) || !(u[a][i + 1] > u[a][i]))
+    if (in[a].ncell < 2) return fail(EMM_EINVAL, "emm_grid_create: need at least 2 cells per axis");
+    for (int i = 0; i <= in[a].ncell; ++i)
+      if (!std::isfinite(in[a].node[i]) || (i > 0 && !(in[a].node[i] > in[a].node[i - 1])))
         return fail(EMM_EINVAL, "emm_grid_create: axis %d coordinates must be finite and strictly increasing", a);
   }
+  const int r = o->rd;
+  const int ne = o->ne < 0 ? r + 5 : o->ne;                       // L686
+  if (ne < r) return fail(EMM_EINVAL, "emm_grid_create: ne must be >= rd (L686)");
   emm_grid *g = new (std::nothrow) emm_grid();
   if (!g) return fail(EMM_ENOMEM, "emm_grid_create: out of memory");
-  g->r = o->rd;
+  g->r = r;
   g->nb = o->nb;
-  g->ne = o->ne < 0 ? o->rd + 5 : o->ne;                         // L686
+  g->ne = ne;
   g->top = o->top;
   g->f0 = o->f0 > 0 ? o->f0 : 1.0;
   g->w0 = 2 * kPi * g->f0;
   g->cfl = o->cfl > 0 ? o->cfl : 0.99;                           // L260
   g->aux_dx = o->aux_dx;
   g->air_route = o->air_route;
-  const int r = g->r, nbe = g->nb + g->ne;
-  if (g->ne < r) { delete g; return fail(EMM_EINVAL, "emm_grid_create: ne must be >= rd (L686)"); }
+  const bool air = g->top == EMM_TOP_AIR;
   g->uniform_xy = uniform_axis(x, nx1) && uniform_axis(y, ny1);
   try {
+    const int pad = g->nb + ne;                                   // L308-311: CPML + buffer cells on a padded side
     for (int a = 0; a < 3; ++a) {
-      g->nc[a] = n1s[a] - 1;
-      int lo = nbe;
-      if (a == 2 && g->top == EMM_TOP_AIR) lo = r;               // [R1] r ghost planes above the surface
-      int N = g->nc[a] + lo + nbe;                               // L308-311
-      if (a < 2 && g->top == EMM_TOP_AIR && g->uniform_xy) N = next_smooth7(N);   // [R1]
-      g->lo[a] = lo;
-      g->N[a] = N;
-      g->xn[a].resize(N + 1);
-      g->xh[a].resize(N);
-      const double dlo = u[a][1] - u[a][0], dhi = u[a][g->nc[a]] - u[a][g->nc[a] - 1];
-      for (int i = 0; i <= N; ++i) {                             // [R1] edge spacing continued
-        const int c = i - lo;
-        g->xn[a][i] = c < 0 ? u[a][0] + c * dlo : (c > g->nc[a] ? u[a][g->nc[a]] + (c - g->nc[a]) * dhi : u[a][c]);
-      }
-      for (int i = 0; i < N; ++i) g->xh[a][i] = 0.5 * (g->xn[a][i] + g->xn[a][i + 1]);
-      g->cm[a].assign((size_t)N * 2 * r, 0.0);
-      g->cp[a].assign((size_t)N * 2 * r, 0.0);
-      double dmax = 0;
-      for (int i = r; i <= N - 1 - r; ++i) {
-        double *m = &g->cm[a][(size_t)i * 2 * r], *p = &g->cp[a][(size_t)i * 2 * r];
-        weights(&g->xh[a][i - r], 2 * r, g->xn[a][i], nullptr, m);        // Eq. 14: D- at x_i
-        weights(&g->xn[a][i - r + 1], 2 * r, g->xh[a][i], nullptr, p);    // Eq. 13: D+ at x_{i+1/2}
-        double sm = 0, sp = 0;
-        for (int q = 0; q < 2 * r; ++q) { sm += std::fabs(m[q]); sp += std::fabs(p[q]); }
-        dmax = std::max(dmax, std::max(sm, sp));                          // Eq. 16
-      }
-      g->Dmax[a] = dmax;
+      g->nc[a] = in[a].ncell;
+      // [R1]: the surface side of z carries no CPML (L292), only the r ghost planes the stencils reach; on a uniform x-y
+      // grid with the air boundary the high side takes extra buffer cells up to a 7-smooth plane size
+      const int below = (a == 2 && air) ? r : pad;
+      int above = pad;
+      if (a < 2 && air && g->uniform_xy) above += next_smooth7(in[a].ncell + below + pad) - (in[a].ncell + below + pad);
+      g->Dmax[a] = pad_axis_and_tabulate(g, a, in[a], below, above, r);
     }
-    g->k0 = g->top == EMM_TOP_AIR ? r : -1;
-    g->klo = r;
-    for (int a = 0; a < 3; ++a) { g->blo[a] = g->nb; g->bhi[a] = g->N[a] - 1 - g->nb; }   // L365-370
-    if (g->top == EMM_TOP_AIR) g->blo[2] = g->k0;
+    g->klo = r;                                                   // first updated plane; the r planes above are ghosts / the wall
+    g->k0 = air ? r : -1;
+    for (int a = 0; a < 3; ++a) {                                 // [R11]: DTFT box = everything but the CPML cells
+      g->blo[a] = (a == 2 && air) ? g->k0 : g->nb;
+      g->bhi[a] = g->N[a] - 1 - g->nb;
+    }
     g->P1 = (g->N[0] + 31) / 32 * 32;                            // 128-byte aligned rows
+    // node indices inside one source's padded volume are 32-bit on the device (source, receiver and check-set lists)
+    if ((long long)g->P1 * g->N[1] * g->N[2] > 2147483647LL) {
+      const int rc = fail(EMM_EINVAL, "emm_grid_create: padded grid of %d x %d x %d nodes exceeds 2^31 - 1 entries", g->N[0], g->N[1], g->N[2]);
+      delete g;
+      return rc;
+    }
     g->XS = (2 * g->nb + 3) / 4 * 4;
-    if (g->top == EMM_TOP_AIR) {
-      if (g->uniform_xy) {
-        g->M1 = g->N[0];
-        g->M2 = g->N[1];
-        g->dxa = g->xn[0][1] - g->xn[0][0];
-        g->dya = g->xn[1][1] - g->xn[1][0];
-      } else {
-        double dmin[2];
-        for (int a = 0; a < 2; ++a) {
-          dmin[a] = u[a][1] - u[a][0];
-          for (int i = 0; i + 1 < n1s[a]; ++i) dmin[a] = std::min(dmin[a], u[a][i + 1] - u[a][i]);
-        }
-        g->dxa = g->aux_dx > 0 ? g->aux_dx : dmin[0];
-        g->dya = g->aux_dx > 0 ? g->aux_dx : dmin[1];
-        g->M1 = next_smooth7((int)std::floor((g->xn[0][g->N[0]] - g->xn[0][0]) / g->dxa) + 2);
-        g->M2 = next_smooth7((int)std::floor((g->xn[1][g->N[1]] - g->xn[1][0]) / g->dya) + 2);
-        for (int a = 0; a < 2; ++a) {
-          const int M = a == 0 ? g->M1 : g->M2;
-          const double da = a == 0 ? g->dxa : g->dya;
-          std::vector<double> xa(M);
-          for (int m = 0; m < M; ++m) xa[m] = g->xn[a][0] + m * da;
-          for (int l = 0; l < 2; ++l) {
-            const double *S = l ? g->xh[a].data() : g->xn[a].data();
-            g->toaux[a][l].resize(M);
-            g->fromaux[a][l].resize(g->N[a]);
-            for (int m = 0; m < M; ++m) make_stencil(S, g->N[a], xa[m], 4, 0, 0, true, &g->toaux[a][l][m]);
-            for (int i = 0; i < g->N[a]; ++i) make_stencil(xa.data(), M, S[i], 4, 0, 0, true, &g->fromaux[a][l][i]);
-          }
-        }
+    if (air && g->uniform_xy) {                                   // the FFT plane is the padded plane itself
+      g->M1 = g->N[0];
+      g->M2 = g->N[1];
+      g->dxa = g->xn[0][1] - g->xn[0][0];
+      g->dya = g->xn[1][1] - g->xn[1][0];
+    } else if (air) {
+      double finest[2];
+      for (int a = 0; a < 2; ++a) {
+        finest[a] = in[a].node[1] - in[a].node[0];
+        for (int c = 1; c < in[a].ncell; ++c) finest[a] = std::min(finest[a], in[a].node[c + 1] - in[a].node[c]);
       }
+      g->dxa = g->aux_dx > 0 ? g->aux_dx : finest[0];
+      g->dya = g->aux_dx > 0 ? g->aux_dx : finest[1];
+      g->M1 = plan_aux_axis(g, 0, g->dxa);
+      g->M2 = plan_aux_axis(g, 1, g->dya);
     }
   } catch (const std::bad_alloc &) {
     delete g;

@@ -482,6 +482,33 @@ __global__ void k_check_acc(const DevGrid g, const DevState s, const int *__rest
   a.y += u * t.y;
 }
 
+// The same sums for the m steps of a DTFT group in one pass: launched between the E and the H update
+// of the last step of the group, when the field ring still holds every level -- E after step l (term l) in buffer
+// (l+1) mod m, H before step l (term l) in buffer l.  Each accumulator receives the same fp64 operations in the same
+// (time) order as with one launch per step; *s.it is the index of the last step of the group.
+__global__ void k_check_acc_group(const DevGrid g, const DevState s, const int *__restrict__ cidx, const int nchk, double2 *__restrict__ C,
+                                  const double2 *__restrict__ twE, const double2 *__restrict__ twH, const float *const baseE0,
+                                  const float *const baseE1, const float *const baseE2, const float *const baseH0, const float *const baseH1,
+                                  const float *const baseH2, const int m) {
+  const int src = blockIdx.z, c = blockIdx.y;
+  if (s.done[src]) return;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= nchk) return;
+  const int it0 = *s.it - (m - 1);
+  const float *base = c == 0 ? baseE0 : c == 1 ? baseE1 : c == 2 ? baseE2 : c == 3 ? baseH0 : c == 4 ? baseH1 : baseH2;
+  const float *fld = base + (size_t)src * g.VS + cidx[p];
+  const double2 *tw = (c < 3 ? twE : twH) + it0;
+  double2 a = C[((size_t)src * 6 + c) * nchk + p];
+  for (int l = 0; l < m; ++l) {
+    const int buf = c < 3 ? (l + 1 == m ? 0 : l + 1) : l;
+    const double u = (double)fld[(size_t)buf * s.hstride];
+    const double2 t = tw[l];
+    a.x += u * t.x;
+    a.y += u * t.y;
+  }
+  C[((size_t)src * 6 + c) * nchk + p] = a;
+}
+
 // ---- receivers-only DTFT: Eq. 25 at the nodes of the receivers' interpolation stencils only, fp64 sums of the fp32
 // fields, every frequency.  Runs where k_check_acc runs: after the E update (E at (it+1/2) dt) and before the H update
 // (H at it dt), [R6]. ----
@@ -503,9 +530,11 @@ __global__ void k_rec_acc(const DevGrid g, const DevState s, const int *__restri
   }
 }
 
-// relative change since the previous check: warp shuffle + block reduction + one atomic per block
+// relative change since the previous check: warp shuffle + block reduction; every block leaves its partial sums in a slot
+// of its own and k_check_final adds them in a fixed order, so that the integer outcome (the step count) does not depend
+// on the order in which the blocks happen to finish
 __global__ void k_check_reduce(const DevState s, const int nchk, const double2 *__restrict__ C, double2 *__restrict__ Cprev,
-                               double *__restrict__ red) {
+                               double *__restrict__ part) {
   const int src = blockIdx.z, c = blockIdx.y;
   if (s.done[src]) return;
   double num = 0.0, den = 0.0;
@@ -536,20 +565,23 @@ __global__ void k_check_reduce(const DevState s, const int nchk, const double2 *
       den += __shfl_xor_sync(0xffffffffu, den, o);
     }
     if (lane == 0) {
-      atomicAdd(&red[src * 4 + (c / 3) * 2 + 0], num);
-      atomicAdd(&red[src * 4 + (c / 3) * 2 + 1], den);
+      part[(((size_t)src * 6 + c) * 2 + 0) * kCheckBlocks + blockIdx.x] = num;
+      part[(((size_t)src * 6 + c) * 2 + 1) * kCheckBlocks + blockIdx.x] = den;
     }
   }
 }
 
 // decision per source; runs before k_step_end of the same step so *it is the index of that step
-__global__ void k_check_final(const DevState s, double *__restrict__ red, double *__restrict__ delta, int *__restrict__ nsteps,
-                              int *__restrict__ status, const int it_min, const double tol, const int stop_enabled) {
+__global__ void k_check_final(const DevState s, const double *__restrict__ part, const int nblk, double *__restrict__ delta,
+                              int *__restrict__ nsteps, int *__restrict__ status, const int it_min, const double tol, const int stop_enabled) {
   const int src = blockIdx.x * blockDim.x + threadIdx.x;
   if (src >= s.nsrc || s.done[src]) return;
   const int it = *s.it;
-  const double nE = red[src * 4 + 0], dE = red[src * 4 + 1], nH = red[src * 4 + 2], dH = red[src * 4 + 3];
-  red[src * 4 + 0] = red[src * 4 + 1] = red[src * 4 + 2] = red[src * 4 + 3] = 0.0;
+  double sum[4] = {0.0, 0.0, 0.0, 0.0};                    // num E, den E, num H, den H: components, then blocks, in order
+  for (int c = 0; c < 6; ++c)
+    for (int q = 0; q < 2; ++q)
+      for (int b = 0; b < nblk; ++b) sum[(c / 3) * 2 + q] += part[(((size_t)src * 6 + c) * 2 + q) * kCheckBlocks + b];
+  const double nE = sum[0], dE = sum[1], nH = sum[2], dH = sum[3];
   nsteps[src] = it + 1;
   if (!isfinite(nE) || !isfinite(dE) || !isfinite(nH) || !isfinite(dH)) {
     status[src] = EMM_ENAN;
@@ -764,14 +796,23 @@ int launch_rec_acc(emm_grid *g, const DevState &s, const DevRun &r) {
   return 0;
 }
 
+int launch_check_acc_group(emm_grid *g, const DevState &s, const DevRun &r, int m) {
+  if (r.nchk <= 0) return 0;
+  dim3 grid((r.nchk + 255) / 256, 6, s.nsrc);
+  k_check_acc_group<<<grid, 256, 0, g->stream>>>(g->dg, s, r.chk_idx, r.nchk, r.C, r.twE64, r.twH64, g->tile_base[0][0], g->tile_base[0][1],
+                                                 g->tile_base[0][2], g->tile_base[1][0], g->tile_base[1][1], g->tile_base[1][2], m);
+  EMM_LAUNCH_CHECK(g, "k_check_acc_group");
+  return 0;
+}
+
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled) {
   int nb = (r.nchk + 255) / 256;
-  if (nb > 148) nb = 148;
+  if (nb > kCheckBlocks) nb = kCheckBlocks;
   if (nb < 1) nb = 1;
   dim3 grid(nb, 6, s.nsrc);
-  k_check_reduce<<<grid, 256, 0, g->stream>>>(s, r.nchk, r.C, r.Cprev, r.red);
+  k_check_reduce<<<grid, 256, 0, g->stream>>>(s, r.nchk, r.C, r.Cprev, r.red_part);
   EMM_LAUNCH_CHECK(g, "k_check_reduce");
-  k_check_final<<<(s.nsrc + 31) / 32, 32, 0, g->stream>>>(s, r.red, r.delta, r.nsteps, r.status, it_min, tol, stop_enabled);
+  k_check_final<<<(s.nsrc + 31) / 32, 32, 0, g->stream>>>(s, r.red_part, nb, r.delta, r.nsteps, r.status, it_min, tol, stop_enabled);
   EMM_LAUNCH_CHECK(g, "k_check_final");
   return 0;
 }

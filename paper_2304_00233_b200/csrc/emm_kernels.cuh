@@ -18,7 +18,8 @@ struct DevRun {
   int nchk = 0;
   double2 *C = nullptr, *Cprev = nullptr;   // [nsrc][6][nchk]
   double2 *twE64 = nullptr, *twH64 = nullptr;  // [max_steps] lowest frequency, fp64
-  double *red = nullptr;       // [nsrc][4]
+  double *red_part = nullptr;  // [nsrc][6][2][kCheckBlocks] per-block partial sums of the check (summed in a fixed order)
+  float *cpml[3][4] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};   // [axis]: a-, b-, a+, b+
   double *delta = nullptr;     // [nsrc][2]
   int *nsteps = nullptr;       // [nsrc]
   int *status = nullptr;       // [nsrc]
@@ -44,6 +45,7 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
 int tile_make_maps(emm_grid *g, const DevState &s);
 int launch_tile(emm_grid *g, const DevState &s, int is_h, int kc, int nchunks, int chunk0, int sel, cudaStream_t st);
 void tile_dims(int *tx, int *ty);
+constexpr int kCheckBlocks = 148;   // blocks per (source, component) of the convergence reduction
 constexpr int kPairMaxNF = 5;       // grouped-DTFT instances exist for 1..5 frequencies (the staged, unrolled ones)
 #ifndef EMM_GROUP_MAX
 #define EMM_GROUP_MAX 8
@@ -55,6 +57,8 @@ inline int default_dtft_group(int nf) { return nf >= 4 ? (kGroupMax < 8 ? kGroup
 // pairfix: also add the product the two-term kernel misses at the injected nodes (see k_inject)
 int launch_inject(emm_grid *g, const DevState &s, const DevRun &r, int magnetic, int pairfix);
 int launch_check_acc(emm_grid *g, const DevState &s, const DevRun &r);
+// the same sums for the m steps of a DTFT group at once, from the levels the field ring still holds (oldest first)
+int launch_check_acc_group(emm_grid *g, const DevState &s, const DevRun &r, int m);
 int launch_rec_acc(emm_grid *g, const DevState &s, const DevRun &r);
 int launch_check(emm_grid *g, const DevState &s, const DevRun &r, int it_min, double tol, int stop_enabled);
 int launch_step_end(emm_grid *g, const DevState &s);

@@ -20,6 +20,7 @@ struct Run {
   int max_steps = 0, fixed_steps = 0, check_every = 100, check_set = EMM_CHECK_FACES;
   int it_min = 0, it_host = 0, table_steps = 0, dtft_every = 1;
   bool sparse = false;                   // receivers-only DTFT (emm_run_opts.sparse_dft)
+  bool chk_grouped = false;              // check-set sums taken once per DTFT group from the field ring (no injected node in the set)
   int group = 1;                         // grouped DTFT: terms of Eq. 25 per accumulator pass (emm_run_opts.dtft_pair); 1 = one per step
   std::vector<double> wav, wavh;            // s(it dt), s((it+1/2) dt) rounded to fp32 (what the device injects)
   std::vector<int> mag;                     // [nsrc] 1 = magnetic dipole
@@ -150,7 +151,6 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
   r.Cprev = A.take<double2>((size_t)nsrc * 6 * nchk);
   r.twE64 = A.take<double2>(table_steps);
   r.twH64 = A.take<double2>(table_steps);
-  r.red = A.take<double>((size_t)nsrc * 4);
   r.delta = A.take<double>((size_t)nsrc * 2);
   r.nsteps = A.take<int>(nsrc);
   r.status = A.take<int>(nsrc);
@@ -165,6 +165,9 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
     r.air = A.take<float2>(g->sep_air ? sep_air_scratch(g, nsrc) : (size_t)(1 + g->r) * g->M1 * g->M2 + (g->uniform_xy ? 0 : (size_t)g->N[1] * g->M1));
   if (g->top == EMM_TOP_AIR && g->sep_air)
     for (int q = 0; q < 8; ++q) r.sp_ws[q] = A.take<char>(g->sp_ws[q] + 256);
+  for (int a = 0; a < 3; ++a)            // CPML coefficients (Eq. 24) at node and half-node positions
+    for (int q = 0; q < 4; ++q) r.cpml[a][q] = A.take<float>(2 * g->nb);
+  r.red_part = A.take<double>((size_t)nsrc * 6 * 2 * kCheckBlocks);
 }
 
 template <class T>
@@ -199,8 +202,7 @@ extern "C" void emm_grid_destroy(emm_grid *g) {
   delete g;
 }
 
-extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, int max_steps, int nrec) {
-  emm_grid *g = const_cast<emm_grid *>(cg);
+extern "C" size_t emm_workspace_bytes(emm_grid *g, int nsrc, int nfreq, int max_steps, int nrec, int dtft_pair) {
   if (!g || nsrc < 1 || nfreq < 0 || nrec < 0) { fail(EMM_EINVAL, "emm_workspace_bytes: bad arguments"); return 0; }
   if (ensure_plans(g)) return 0;
   if (g->sep_air && sep_air_make_plans(g, nsrc)) return 0;
@@ -211,10 +213,15 @@ extern "C" size_t emm_workspace_bytes(const emm_grid *cg, int nsrc, int nfreq, i
   const size_t fixed = A.off;
   DevState s{};
   DevRun r{};
-  layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES),
-             nfreq >= 1 && nfreq <= kPairMaxNF ? kGroupMax - 2 : 0, s, r);   // field buffers of the largest group a run may ask for                           // the full-grid mode with the largest DTFT group is the larger one
+  // full-grid accumulators with the field ring of the DTFT group the runs will ask for (emm_run_opts.dtft_pair; a run that
+  // asks for a larger group than fits gets the largest that does), or the receivers-only layout: whichever is larger
+  const int group = dtft_pair < 0 || nfreq < 1 || nfreq > kPairMaxNF ? 1 : std::min(kGroupMax, dtft_pair >= 2 ? dtft_pair : default_dtft_group(nfreq));
+  layout_run(g, A, nsrc, nfreq, 0, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), group > 2 ? group - 2 : 0, s, r);
+  const size_t full = A.off;
+  A.off = fixed;
+  layout_run(g, A, nsrc, 0, nfreq, max_steps + 1, nrec, chk_count(g, EMM_CHECK_FACES), 0, s, r);
   g->T = keep;
-  return std::max(A.off, fixed + 1024) + 4096;       // emm_model_set keeps a few scalars behind the per-grid region
+  return std::max(std::max(full, A.off), fixed + 1024) + 4096;       // emm_model_set keeps a few scalars behind the per-grid region
 }
 
 extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, void *cuda_stream) {
@@ -369,30 +376,33 @@ static double node_width(const emm_grid *g, int a, int half, int i) {
   return half ? g->xn[a][i + 1] - g->xn[a][i] : g->xh[a][i] - g->xh[a][i - 1];
 }
 
-// CPML coefficients (Eq. 24) with the profile of [R5]; index convention of L324-326
+// CPML recursion coefficients (Eq. 24) of one axis, written from reading [R5]: kappa = 1; damping d = d0 s^2 with
+// s = (depth into the layer) / (layer thickness) and d0 = 3 v_ref ln(1000) / (2 thickness) (theoretical reflection 1e-3);
+// frequency shift alpha = pi (fmax/2) (1 - s), never negative; b = exp(-(d + alpha) dt), a = d (b - 1) / (d + alpha) and
+// a = 0 where d = 0.  Depth is measured at the derivative's own location: the node for D-, the half node for D+.
+// Slab entry e < nb belongs to the low face (index e), e >= nb to the high face, mirrored (index N-1-(e-nb)), L324-326.
 static void cpml_tables(const emm_grid *g, int a, double fmax, std::vector<float> &am, std::vector<float> &bm,
                         std::vector<float> &ap, std::vector<float> &bp) {
   const int N = g->N[a], nb = g->nb;
+  const std::vector<double> &xn = g->xn[a], &xh = g->xh[a];
   am.assign(2 * nb, 0.f); ap.assign(2 * nb, 0.f); bm.assign(2 * nb, 1.f); bp.assign(2 * nb, 1.f);
-  const double Rc = 1e-3;
-  for (int side = 0; side < 2; ++side) {
-    if (a == 2 && side == 0 && g->top == EMM_TOP_AIR) continue;     // no CPML at the top (L292)
-    const double x_in = side == 0 ? g->xn[a][nb] : g->xn[a][N - 1 - nb];
-    const double L = side == 0 ? g->xn[a][nb] - g->xn[a][0] : g->xn[a][N - 1] - g->xn[a][N - 1 - nb];
-    const double d0 = -3.0 * g->vref[a][side] * std::log(Rc) / (2.0 * L);
-    for (int q = 0; q < nb; ++q) {
-      const int i = side == 0 ? q : N - 1 - q, ii = side == 0 ? q : nb + q;
-      for (int half = 0; half < 2; ++half) {
-        const double p = half ? g->xh[a][i] : g->xn[a][i];
-        const double xi = std::max(side == 0 ? x_in - p : p - x_in, 0.0);
-        const double d = d0 * (xi / L) * (xi / L);
-        const double al = std::max(kPi * (fmax / 2) * (1 - xi / L), 0.0);
-        const double b = std::exp(-(d + al) * g->dt);
-        const double aa = d > 0 ? d / (d + al) * (b - 1) : 0.0;
-        (half ? ap : am)[ii] = (float)aa;
-        (half ? bp : bm)[ii] = (float)b;
-      }
-    }
+  auto coefficients = [&](double depth, double thickness, double vref, float &a_out, float &b_out) {
+    const double s = std::max(depth / thickness, 0.0);
+    const double d = 1.5 * vref * std::log(1000.0) / thickness * s * s;
+    const double alpha = std::max(kPi * 0.5 * fmax * (1.0 - s), 0.0);
+    const double rate = d + alpha;
+    b_out = (float)std::exp(-rate * g->dt);
+    a_out = d > 0 ? (float)(d / rate * std::expm1(-rate * g->dt)) : 0.f;
+  };
+  for (int e = 0; e < 2 * nb; ++e) {
+    const bool high = e >= nb;
+    if (!high && a == 2 && g->top == EMM_TOP_AIR) continue;           // no CPML at the surface (L292)
+    const int i = high ? N - 1 - (e - nb) : e;
+    // the layer is the outermost nb cells counted from the last updated-side node: [x_0, x_nb] or [x_{N-1-nb}, x_{N-1}]
+    const double inner = high ? xn[N - 1 - nb] : xn[nb], outer = high ? xn[N - 1] : xn[0];
+    const double thickness = std::fabs(outer - inner), vref = g->vref[a][high ? 1 : 0];
+    coefficients(high ? xn[i] - inner : inner - xn[i], thickness, vref, am[e], bm[e]);
+    coefficients(high ? xh[i] - inner : inner - xh[i], thickness, vref, ap[e], bp[e]);
   }
 }
 
@@ -419,6 +429,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
     // F_E (old and new E) and the H kernel none; a left-over last step takes its single terms as usual.  A batch never
     // crosses a convergence check (enqueue_steps), so every sum is complete where it is read.
     int me = 0, mh = 0, he = -1, hh = -1, fix_e = 0;
+    int chk_m = 1;                           // check-set sums: 1 = this step's term now, 0 = later with its group, m = the whole group now
     // s1: injection + E update; s2: E boundary, check set, H update; s3: H boundary, magnetic injection, check
     DevState s1 = R->ds, s2 = R->ds, s3 = R->ds;
     if (R->group > 1) {
@@ -439,6 +450,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
         // the electric injection of step p lands in the buffer that holds term p-1 (closing pass: its old E): the missing
         // product goes into the accumulators with the injection
         fix_e = p >= 1;
+        if (m > 2 && R->chk_grouped) chk_m = p == m - 1 ? m : 0;
         if (m > 2) {
           const size_t bs = (size_t)R->ds.hstride;
           const int pn = (p + 1) % m;
@@ -457,7 +469,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
     if (R->any_el && (rc = launch_inject(g, s1, R->dr, 0, fix_e))) return rc;     // Alg. 1 L477 (before the update: same sum)
     if (g->top != EMM_TOP_AIR) {
       if ((rc = launch_update(g, s1, 0, 0, me, he, M))) return rc;                 // L476-479 + E part of L483
-      if ((rc = launch_check_acc(g, s2, R->dr))) return rc;                // check-set part of L483
+      if ((rc = chk_m == 1 ? launch_check_acc(g, s2, R->dr) : chk_m > 1 ? launch_check_acc_group(g, s2, R->dr, chk_m) : 0)) return rc;   // check-set part of L483
       if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
       if ((rc = launch_update(g, s2, 1, 0, mh, hh, M))) return rc;                 // H part of L483 + L486-489
     } else if (g->prof) {
@@ -466,7 +478,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       CU(cudaEventRecord(g->ev[0], M)); CU(cudaStreamWaitEvent(B, g->ev[0], 0));
       if ((rc = launch_air(g, s2, R->dr, 0, B))) return rc;                // L481
       CU(cudaEventRecord(g->ev[1], B)); CU(cudaStreamWaitEvent(M, g->ev[1], 0));
-      if ((rc = launch_check_acc(g, s2, R->dr))) return rc;
+      if ((rc = chk_m == 1 ? launch_check_acc(g, s2, R->dr) : chk_m > 1 ? launch_check_acc_group(g, s2, R->dr, chk_m) : 0)) return rc;
       if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
       if ((rc = launch_update(g, s2, 1, 0, mh, hh, M))) return rc;
       CU(cudaEventRecord(g->ev[2], M)); CU(cudaStreamWaitEvent(B, g->ev[2], 0));
@@ -482,7 +494,7 @@ static int enqueue_steps_raw(emm_grid *g, int n) {
       if ((rc = launch_update(g, s1, 0, 2, me, he, M))) return rc;                 // E, bulk
       CU(cudaEventRecord(g->ev[2], M));
       CU(cudaStreamWaitEvent(M, g->ev[1], 0));                                // H bulk and the check set read surface-chunk E
-      if ((rc = launch_check_acc(g, s2, R->dr))) return rc;
+      if ((rc = chk_m == 1 ? launch_check_acc(g, s2, R->dr) : chk_m > 1 ? launch_check_acc_group(g, s2, R->dr, chk_m) : 0)) return rc;
       if ((rc = launch_rec_acc(g, s2, R->dr))) return rc;
       CU(cudaEventRecord(g->ev[4], M));
       if ((rc = launch_update(g, s2, 1, 2, mh, hh, M))) return rc;                 // H, bulk
@@ -697,16 +709,12 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
 
     // CPML tables
     DevGrid &d = g->dg;
-    {
-      Arena B = A;           // continue after the run region
-      for (int a = 0; a < 3; ++a) {
-        std::vector<float> am, bm, ap, bp;
-        cpml_tables(g, a, R->fmax, am, bm, ap, bp);
-        float *dam = B.take<float>(2 * nb), *dbm = B.take<float>(2 * nb), *dap = B.take<float>(2 * nb), *dbp = B.take<float>(2 * nb);
-        if (B.overflow) { free_run(g); return fail(EMM_ENOMEM, "emm_run_begin: workspace too small (CPML tables)"); }
-        if ((rc = upload(g, dam, am)) || (rc = upload(g, dbm, bm)) || (rc = upload(g, dap, ap)) || (rc = upload(g, dbp, bp))) { free_run(g); return rc; }
-        d.am[a] = dam; d.bm[a] = dbm; d.ap[a] = dap; d.bp[a] = dbp;
-      }
+    for (int a = 0; a < 3; ++a) {
+      std::vector<float> am, bm, ap, bp;
+      cpml_tables(g, a, R->fmax, am, bm, ap, bp);
+      float *const *t = R->dr.cpml[a];
+      if ((rc = upload(g, t[0], am)) || (rc = upload(g, t[1], bm)) || (rc = upload(g, t[2], ap)) || (rc = upload(g, t[3], bp))) { free_run(g); return rc; }
+      d.am[a] = t[0]; d.bm[a] = t[1]; d.ap[a] = t[2]; d.bp[a] = t[3];
     }
 
     // sources: W_c = dir_c w_x w_y w_z / V on the component's lattice, premultiplied by dt/eps ([R7])
@@ -770,6 +778,11 @@ extern "C" int emm_run_begin(emm_grid *g, const emm_src *src, int nsrc, const do
         sw.push_back((float)(ce * sWd[n]));
       }
     }
+    // check-set sums once per DTFT group (k_check_acc_group) read earlier levels of the field ring, into which later
+    // electric injections have already been added at the source nodes: only when no source node is in the check set
+    R->chk_grouped = R->group > 2 && R->check_set != EMM_CHECK_FULL;
+    for (size_t n = 0; n < sidx.size() && R->chk_grouped; ++n)
+      if (std::binary_search(chk.begin(), chk.end(), sidx[n])) R->chk_grouped = false;
     if ((rc = upload(g, const_cast<int *>(R->ds.src_mag), R->mag))) { free_run(g); return rc; }
     if ((rc = upload(g, R->dr.src_off, soff)) || (rc = upload(g, R->dr.src_idx, sidx)) || (rc = upload(g, R->dr.src_w, sw))) { free_run(g); return rc; }
 

@@ -398,6 +398,8 @@ int launch_tile_r(const TileMaps &tm, const DevGrid &dg, const DevState &s, dim3
 // tensor maps of the run's field rings and of dt/eps; called by emm_run_begin once the per-run region is laid out
 int tile_make_maps(emm_grid *g, const DevState &s) {
   g->tile_ok = false;
+  for (int c = 0; c < 3; ++c) { g->tile_base[0][c] = s.E[c]; g->tile_base[1][c] = s.H[c]; }     // buffer 0 of the field rings
+  g->tile_hstride = s.hstride;
   const int R = g->r;
   if (g->P1 < TX || g->N[1] < TY + 2 * R) return 0;          // tiny grids keep the per-thread kernel
   const int nw = s.nbuf * s.nsrc, HY = TY + 2 * R - 1;
@@ -411,8 +413,6 @@ int tile_make_maps(emm_grid *g, const DevState &s) {
     for (int c = 0; c < 3; ++c)
       if ((rc = make_map(c == 0 ? &tm.C1 : c == 1 ? &tm.C2 : &tm.C3, g->T.ce[c], g, 0, TX, TY))) return rc;
   }
-  for (int c = 0; c < 3; ++c) { g->tile_base[0][c] = s.E[c]; g->tile_base[1][c] = s.H[c]; }
-  g->tile_hstride = s.hstride;
   g->tile_ok = true;
   return 0;
 }

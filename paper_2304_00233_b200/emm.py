@@ -86,7 +86,7 @@ def lib():
         L.emm_grid_info.argtypes = [vp, ip, dp]
         L.emm_grid_coords.argtypes = [vp, C.c_int, dp]
         L.emm_grid_fdcoef.argtypes = [vp, C.c_int, C.c_int, dp]
-        L.emm_workspace_bytes.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.emm_workspace_bytes.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
         L.emm_workspace_bytes.restype = C.c_size_t
         L.emm_bind_device.argtypes = [vp, vp, C.c_size_t, vp]
         L.emm_model_set.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
@@ -222,23 +222,26 @@ class Grid:
         return out
 
     # -- device memory and stream come from torch --
-    def workspace_bytes(self, nsrc, nfreq, max_steps, nrec):
-        n = lib().emm_workspace_bytes(self._h, nsrc, nfreq, max_steps, nrec)
+    def workspace_bytes(self, nsrc, nfreq, max_steps, nrec, dtft_pair=0):
+        n = lib().emm_workspace_bytes(self._h, nsrc, nfreq, max_steps, nrec, dtft_pair)
         if n == 0:
             raise EmmError(ECUDA, lib().emm_last_error().decode())
         return n
 
-    def bind(self, nsrc=1, nfreq=1, max_steps=0, nrec=64, device="cuda:0", ws_bytes=None):
+    def bind(self, nsrc=1, nfreq=1, max_steps=0, nrec=64, device=None, ws_bytes=None, dtft_pair=0):
         """ws_bytes: bind a workspace of exactly this size instead of emm_workspace_bytes() (tests of the tight-memory paths)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libemm_b200 needs a CUDA device; there is no CPU fallback")
+        device = device or getattr(self, "_device", None) or "cuda:0"
+        self._device = device
         max_steps = max_steps or 100000
         plan = (nsrc, nfreq, max_steps, nrec)
-        if ws_bytes is None and self._ws is not None and self._plan is not None and all(a <= b for a, b in zip(plan, self._plan)):
-            return
         torch.cuda.set_device(device)
-        n = int(ws_bytes) if ws_bytes is not None else self.workspace_bytes(nsrc, nfreq, max_steps, nrec)
+        n = int(ws_bytes) if ws_bytes is not None else self.workspace_bytes(nsrc, nfreq, max_steps, nrec, dtft_pair)
+        if ws_bytes is None and self._ws is not None and n <= self._ws.numel():
+            return
+        self._fixed_ws = ws_bytes is not None          # an explicitly sized workspace is never regrown by _ensure
         self._ws = None
         self._ws = torch.empty(n, dtype=torch.uint8, device=device)
         torch.cuda.synchronize(device)
@@ -265,11 +268,12 @@ class Grid:
         steps = int(o.get("fixed_steps", 0)) or int(o.get("max_steps", 0)) or 100000
         resident = nsrc if (o.get("batched", 0) or o.get("_resident", 0)) else 1
         plan = (resident, nfreq, steps, max(nrec, 1))
-        if self._plan is None or any(a > b for a, b in zip(plan, self._plan)):
-            model = getattr(self, "_model", None)
-            self.bind(*[max(a, b) for a, b in zip(plan, self._plan or plan)])
-            if model is not None:
-                self.model_set(*model)
+        if getattr(self, "_fixed_ws", False):
+            return
+        ws = self._ws
+        self.bind(*[max(a, b) for a, b in zip(plan, self._plan or plan)], dtft_pair=int(o.get("dtft_pair", 0)))
+        if self._ws is not ws and getattr(self, "_model", None) is not None:      # a larger workspace was bound: the model goes up again
+            self.model_set(*self._model)
 
     def run(self, sources, freqs, receivers, opts=None, allow_noconv=False):
         freqs = np.ascontiguousarray(freqs, dtype=np.float64)

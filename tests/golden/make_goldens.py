@@ -8,8 +8,10 @@ receiver stencils and the check set: pointwise identical values, see test_conver
     python tests/golden/make_goldens.py cfg2            # ~15 min on 8 cores
     python tests/golden/make_goldens.py cfg3 0 100        # configs[2] with aux_dx = 100 m, to convergence: ~50 min
     python tests/golden/make_goldens.py cfg4 300 100      # configs[3] with aux_dx = 100 m, 300 fixed steps: ~50 min
-    python tests/golden/make_goldens.py cfg4 3000 0 fields 1000,2000   # configs[3] as bench.py times it (default auxiliary
-                                                          # plane, 3125 x 3125), 3000 fixed steps, field planes: ~4.5 h on 8 cores
+    python tests/golden/make_goldens.py cfg4s 1000 0 fields 500   # configs[3] on its default auxiliary plane (3125 x 3125,
+                                                          # what bench.py times) with source and receivers 150 m below the
+                                                          # surface and a 20 Hz wavelet (workloads.cfg4s), 1000 fixed
+                                                          # steps, field planes: ~2-3 h on 8 cores
 
 Output: tests/golden/<name>_converged[_aux<dx>].json or <name>_<n>steps[_aux<dx>].json with the inputs' SHA-256, nsteps, delta and the complex receivers.
 With `fields` also <name>_<n>steps[_aux<dx>]_fields.npz at every listed checkpoint and at the last step: the six time-domain
@@ -84,6 +86,8 @@ def main():
     opts["sparse_dft"] = 1
     if fixed:
         opts = dict(fixed_steps=fixed, sparse_dft=1)
+        if "fmax" in w["run"]:
+            opts["fmax"] = w["run"]["fmax"]
     fields = len(sys.argv) > 4 and sys.argv[4] == "fields"
     marks = sorted(int(v) for v in sys.argv[5].split(",")) if len(sys.argv) > 5 else []
     t = time.time()

@@ -280,6 +280,79 @@ def test_convergence_rule(oracle):
     assert ns5[0] == ns[0] and np.array_equal(out5, out)
 
 
+def test_convergence_check_uses_the_lowest_frequency_wherever_it_is_listed(oracle):
+    """L387 "lowest frequency": the stopping rule looks at the accumulators of the lowest requested frequency, whatever
+    its position in the list.  An unsorted list must stop at the same step, with the same delta and the same Green's
+    functions (permuted), as the sorted one -- and a run of the highest frequency alone stops at a different step, so a
+    rule that looked at list position 0 (1.25 Hz here) instead would be caught."""
+    w = W.cfg1(n=24, dx=100.0, rd=2, nb=6)
+    g = make_grid(oracle, w)
+    rec = w["receivers"][:3]
+    opts = dict(tol=1e-6, check_every=50)
+    out_s, ns_s = g.run(w["sources"], [0.25, 0.75, 1.25], rec, dict(opts, fmax=4.0))
+    d_s = g.get("DELTA").copy()
+    out_u, ns_u = g.run(w["sources"], [1.25, 0.25, 0.75], rec, dict(opts, fmax=4.0))
+    d_u = g.get("DELTA").copy()
+    assert ns_u[0] == ns_s[0] and np.array_equal(d_u, d_s)
+    assert np.array_equal(out_u[0][[1, 2, 0]], out_s[0])
+    out_h, ns_h = g.run(w["sources"], [1.25], rec, dict(opts, fmax=4.0))       # same wavelet, highest frequency alone
+    assert ns_h[0] != ns_s[0]
+
+
+def test_air_boundary_ghost_planes_semigroup_and_curl_free(oracle):
+    """Eq. 17-21 on the uniform grid, checked on the ghost planes the oracle leaves behind, with numpy's FFT as the
+    independent transform: (i) upward continuation is a semigroup -- continuing ghost level 1 by the level spacing gives
+    ghost level 2, for Ex, Ey (Eq. 21) and for Hx, Hy (Eq. 19-20): exp(-k_h h1) exp(-k_h (h2-h1)) = exp(-k_h h2), so a
+    wrong height, a wrong wavenumber scale or a growing exponential fails; (ii) level 1 is the surface plane continued by
+    its own height; (iii) the air field is curl-free: k_y Hx^ = k_x Hy^ once the half-cell phase factors between the two
+    lattices are undone (a swapped k_x / k_y or one wrong sign fails)."""
+    rd, dx = 3, 100.0
+    x = (np.arange(21) - 10) * dx
+    z = np.arange(15) * dx
+    sig = np.ones((14, 20, 20), np.float32)
+    sig[:3] = 3.2
+    g = oracle.Grid(x, x, z, rd=rd, nb=6, ne=-1, top=oracle.TOP_AIR)
+    g.model_set(sig)
+    i = g.info()
+    assert i["uniform_xy"] == 1
+    k0, M1, M2 = i["k0"], i["aux_M1"], i["aux_M2"]
+    g.run_begin([((-30.0, 20.0, 270.0), (1.0, 0.5, 0.3))], [1.0], np.array([[0.0, 0.0, 300.0]]), dict(fixed_steps=400, fmax=8.0))
+    g.run_steps(120)
+    kx = 2 * np.pi * np.fft.fftfreq(M1, dx)[None, :]
+    ky = 2 * np.pi * np.fft.fftfreq(M2, dx)[:, None]
+    kh = np.sqrt(kx ** 2 + ky ** 2)
+    zn = g.coords(2)
+    zh = 0.5 * (zn[1:] + zn[:-1])
+
+    def cont(plane, h):
+        return np.fft.ifft2(np.exp(-kh * h) * np.fft.fft2(plane)).real
+
+    for c in ("E1", "E2"):
+        f = g.get(c)
+        assert np.abs(f[k0]).max() > 0
+        h1, h2 = zn[k0] - zn[k0 - 1], zn[k0] - zn[k0 - 2]
+        sc = np.abs(f[k0 - 1]).max()
+        assert np.abs(cont(f[k0], h1) - f[k0 - 1]).max() < 1e-12 * sc
+        assert np.abs(cont(f[k0 - 1], h2 - h1) - f[k0 - 2]).max() < 1e-12 * sc
+        assert np.abs(f[k0 - 2]).max() < np.abs(f[k0 - 1]).max() < np.abs(f[k0]).max()      # decays upward
+    Hx, Hy = g.get("H1"), g.get("H2")
+    for f in (Hx, Hy):
+        sc = np.abs(f[k0 - 1]).max()
+        assert sc > 0
+        for m in (1, 2):
+            dh = (zn[k0] - zh[k0 - m - 1]) - (zn[k0] - zh[k0 - m])
+            assert np.abs(cont(f[k0 - m], dh) - f[k0 - m - 1]).max() < 1e-12 * sc
+    # Hx lives on (x, yh), Hy on (xh, y): bring both spectra to the (xh, yh) lattice of Hz before comparing
+    Fx = np.fft.fft2(Hx[k0 - 1]) * np.exp(1j * kx * dx / 2)
+    Fy = np.fft.fft2(Hy[k0 - 1]) * np.exp(1j * ky * dx / 2)
+    inner = np.ones((M2, M1), bool)
+    if M1 % 2 == 0:
+        inner[:, M1 // 2] = False
+    if M2 % 2 == 0:
+        inner[M2 // 2, :] = False
+    assert np.abs(ky * Fx - kx * Fy)[inner].max() < 1e-10 * np.abs(kh * Fx).max()
+
+
 # ---- DTFT decimation (SURVEY 8f rank 1; DESIGN.md "DTFT decimation") -----------------------------------
 def test_dtft_decimation_leaves_green_functions_unchanged(oracle, small_ws):
     """Taking only every m-th term of the sums of Eq. 25 (for the fields AND J') aliases the spectrum at multiples

@@ -188,6 +188,71 @@ def test_effective_medium_at_interface(oracle):
     assert np.all(g.get("CE1")[: i["k0"]] == 0)         # ghost planes are never updated
 
 
+def test_effective_medium_unequal_widths_is_the_dual_face_average(oracle):
+    """[R3]/Eq. 26 on a grid whose neighbouring cells have UNEQUAL widths on all three axes (the rule every non-uniform
+    config runs through).  The effective conductivity of an E component is the average of sigma over the face of the dual
+    cell that its edge pierces (resistors in parallel, L400).  Checked two ways that share nothing with the oracle's
+    loop: (i) a hand-computed number on a two-material model -- widths 100 | 300 m across the interface, sigma 1 | 4
+    S/m: (1*100 + 4*300)/400 = 3.25, not the 2.5 an unweighted mean gives; (ii) brute force: the mean of the piecewise
+    constant sigma sampled on a fine lattice over that dual face, for random cell values, for all three components
+    (sigma_v for E3)."""
+    x = np.cumsum(np.concatenate(([0.0], [100.0, 300.0, 120.0, 80.0, 260.0, 140.0, 90.0, 200.0])))
+    y = np.cumsum(np.concatenate(([0.0], [100.0, 300.0, 70.0, 210.0, 130.0, 90.0, 170.0, 110.0])))
+    z = np.cumsum(np.concatenate(([0.0], [50.0, 150.0, 40.0, 120.0, 60.0, 200.0, 80.0, 100.0])))
+    n = 8
+    w0 = 2 * np.pi
+
+    def effective(sh, sv):
+        g = oracle.Grid(x, y, z, rd=1, nb=2, ne=2)
+        g.model_set(sh.astype(np.float32), sv.astype(np.float32))
+        i = g.info()
+        lo = (i["lo3"], i["lo2"], i["lo1"])
+        sl = tuple(slice(lo[a], lo[a] + n) for a in range(3))
+        return [2 * w0 * i["dt"] / g.get("CE%d" % (c + 1))[sl] for c in range(3)]           # sigma_bar at the model's own nodes
+
+    # (i) vertical interface on the node plane y = y[1]: sigma = 1 for y < 100, 4 beyond; uniform otherwise
+    sh = np.ones((n, n, n))
+    sh[:, 1:, :] = 4.0
+    s11, s22, s33 = effective(sh, sh)
+    assert abs(s11[4, 1, 4] - 3.25) < 1e-12              # Ex on the interface: tangential, widths 100 | 300
+    assert abs(s33[4, 1, 4] - 3.25) < 1e-12              # Ez on the interface: tangential too
+    assert abs(s22[4, 1, 4] - 4.0) < 1e-12               # Ey at yh[1]: inside the second cell
+    # the same across z (widths 50 | 150) for the horizontal components, with a different sigma_v that E3 alone must see
+    sh = np.ones((n, n, n))
+    sh[1:] = 4.0
+    sv = np.full((n, n, n), 7.0)
+    s11, s22, s33 = effective(sh, sv)
+    assert abs(s11[1, 4, 4] - (1 * 50 + 4 * 150) / 200.0) < 1e-12 and abs(s22[1, 4, 4] - 3.25) < 1e-12
+    assert abs(s33[1, 4, 4] - 7.0) < 1e-12
+
+    # (ii) brute force over the dual face, random cells
+    rng = np.random.default_rng(26)
+    sh = rng.uniform(0.2, 5.0, size=(n, n, n))
+    sv = rng.uniform(0.2, 5.0, size=(n, n, n))
+    eff = effective(sh, sv)
+    nodes = (x, y, z)
+
+    def face_mean(c, idx, model, m=1500):
+        """mean of model over the dual face of component c at node idx = (k, j, i), by midpoint sampling on an m x m
+        lattice: the component sits at the half node of its own axis (inside cell i) and at nodes of the two others;
+        the face spans from the previous to the next half node along those two"""
+        pos = {a: idx[2 - a] for a in range(3)}           # node index along each coordinate axis (x = 0, y = 1, z = 2)
+        others = [a for a in range(3) if a != c]
+        t = (np.arange(m) + 0.5) / m
+        cells = {c: np.array([pos[c]])}
+        for a in others:
+            u, i = nodes[a], pos[a]
+            lo_, hi_ = 0.5 * (u[i - 1] + u[i]), 0.5 * (u[i] + u[i + 1])
+            cells[a] = np.clip(np.searchsorted(u, lo_ + (hi_ - lo_) * t, side="right") - 1, 0, n - 1)
+        return model[np.ix_(cells[2], cells[1], cells[0])].mean()
+
+    for c, model in ((0, sh), (1, sh), (2, sv)):
+        for idx in ((3, 4, 2), (1, 1, 1), (5, 2, 6), (2, 6, 3)):
+            ref = face_mean(c, idx, model)
+            got = eff[c][idx]
+            assert abs(got / ref - 1) < 2e-3, (c, idx, got, ref)       # sampling error <= contrast / (2 m) per axis
+
+
 # ---- argument checking (SURVEY 8b error codes) ----------------------------------------------------
 def test_invalid_arguments(oracle):
     nodes = np.arange(9) * 10.0
