@@ -103,6 +103,16 @@ def test_fields_wholespace_cpml(emm, oracle, rd, pair):
     _field_parity(emm, oracle, w, 200, dtft_pair=pair)
 
 
+def test_wide_cpml_layer_in_an_exactly_sized_workspace(emm, oracle):
+    """nb = 34: the twelve CPML coefficient tables are longer than one 256-byte allocation unit each; the workspace is the
+    one emm_workspace_bytes asks for (the binding allocates exactly that), so the tables must be part of its count."""
+    w = W.cfg1(n=14, dx=100.0, rd=2, nb=34)
+    src = np.array(w["sources"][0][0])
+    offs = np.array([150.0, 300.0, 420.0])                 # off-axis, off-grid: all six components are non-zero
+    w["receivers"] = np.stack([src[0] + 0.8 * offs, src[1] + 0.36 * offs, src[2] - 0.48 * offs], axis=1)
+    _field_parity(emm, oracle, w, 120)
+
+
 @pytest.mark.parametrize("rd", [1, 2, 3])
 def test_fields_layered_air_uniform(emm, oracle, rd):
     """configs[1] scaled: layered marine model, FFT air-water boundary on the padded plane itself."""
