@@ -9,7 +9,7 @@ The oracle cannot step a 43 M-node grid for thousands of steps inside a test, so
     (oracle only): step count exact, receivers within 1e-3;
   * configs[3] (cfg4, the bench workload) is checked through properties that hold at any size, on sampled
     nodes chosen on tile / chunk / quad boundaries of the launch configuration: one time step reproduces the
-    definition of the update (Eq. 8, 13, 14 with the library's own tables, fp64) and the fused DTFT equals the
+    definition of the update (Eq. 8, 13, 14 with the ORACLE's tables and dt/eps, fp64) and the fused DTFT equals the
     sum of Eq. 25 over the steps taken;
   * configs[4] (cfg5): the batched launch is bit-identical to running the sources one after the other.
 """
@@ -107,17 +107,24 @@ def cfg4_run(emm):
     return w, g, info
 
 
-def test_cfg4_full_size_one_step_equals_definition(emm, cfg4_run):
+def test_cfg4_full_size_one_step_equals_definition(emm, oracle, cfg4_run):
+    """One step of the CUDA path at full size against the definition of the update (Eq. 8, 13, 14) evaluated in fp64 with the
+    ORACLE's operator tables, dt/eps and time step for this grid and model (its emmo_grid_create / emmo_model_set), applied to the
+    fields the GPU held before the step."""
     w, g, info = cfg4_run
     r = w["grid"]["rd"]
     names = ("E1", "E2", "E3", "H1", "H2", "H3")
     old = {c: g.get(c) for c in names}
     g.run_steps(1)
     new = {c: g.get(c) for c in names}
-    ce = [g.get("CE%d" % (c + 1)) for c in range(3)]
-    tm = [g.fdcoef(a, 0) for a in range(3)]
-    tp = [g.fdcoef(a, 1) for a in range(3)]
-    dtmu = info["dt"] / MU0
+    go = make_grid(oracle, w)
+    io = go.info()
+    assert (io["N1"], io["N2"], io["N3"]) == (info["N1"], info["N2"], info["N3"]) and abs(io["dt"] / info["dt"] - 1) < 1e-12
+    ce = [go.get("CE%d" % (c + 1)) for c in range(3)]
+    tm = [go.fdcoef(a, 0) for a in range(3)]
+    tp = [go.fdcoef(a, 1) for a in range(3)]
+    go.close()
+    dtmu = io["dt"] / MU0
     rng = np.random.default_rng(11)
     src = _source_node(g)
     pts = _sample_nodes(info, r, rng, src)
@@ -350,3 +357,56 @@ def test_cfg5_full_size_200_steps_batched_fields_match_live_oracle(emm, oracle):
         assert big.sum() >= 3 and (np.abs(A - B)[big] / np.abs(B)[big]).max() < 1e-3
     ga.close()
     gb.close()
+
+
+def test_cfg4_default_aux_plane_1000_steps_fields_match_oracle_golden(emm):
+    """configs[3]'s grid, model and DEFAULT auxiliary plane (3125 x 3125: the air-water boundary exactly as bench.py times
+    it) with the shallow source of workloads.cfg4s, 1000 steps: by then the wave has been through the boundary for several
+    hundred steps.  Oracle values stored by `tests/golden/make_goldens.py cfg4s 1000 0 fields 500` (oracle only, ~3 h):
+    the six fields on four whole z planes (the ghost plane the boundary writes, the surface plane, the one below, the seabed
+    plane) and on the x-z slice through the source, the L2 norm of every z plane, the partial Green's functions at 441
+    receivers.  Field tolerance: north_star's 1e-5 relative L2 is stated for 200 steps; fp32 rounding accumulates like the
+    square root of the step count, so 1000 steps are given 1e-5 * sqrt(5) = 2.24e-5, per plane and per field, against
+    that field's own norm on the plane (planes on which the field is identically zero in the oracle must be zero)."""
+    path = os.path.join(HERE, "golden", "cfg4s_1000steps_fields.npz")
+    gold = np.load(path)
+    w = W.cfg4s(emm.emm_nugrid)
+    g = make_grid(emm, w)
+    info = g.info()
+    assert [info["N3"], info["N2"], info["N1"]] == list(gold["dims"]) and [info["aux_M1"], info["aux_M2"]] == list(gold["aux"]) == [3125, 3125]
+    assert abs(info["dt"] / float(gold["dt"]) - 1) < 1e-12
+    nsteps = int(gold["nsteps"])
+    g.run_begin(w["sources"][:1], w["freqs"], w["receivers"], dict(fixed_steps=nsteps, fmax=w["run"]["fmax"]))
+    ns, done = g.run_steps(nsteps)
+    assert int(ns[0]) == nsteps and done
+    tol = 1e-5 * np.sqrt(nsteps / 200.0)
+    planes, jsl = [int(k) for k in gold["planes_k"]], int(gold["slice_j"])
+    checked = 0
+    for c in ("E1", "E2", "E3", "H1", "H2", "H3"):
+        f = g.get(c).astype(np.float64)
+        assert np.all(np.isfinite(f))
+        ref_norms = gold["norm_" + c]
+        got_norms = np.sqrt((f * f).sum(axis=(1, 2)))
+        assert np.abs(got_norms - ref_norms).max() <= tol * ref_norms.max(), c
+        for q, k in enumerate(planes):
+            ref = gold["planes_" + c][q].astype(np.float64)
+            nr = np.linalg.norm(ref)
+            if nr == 0.0:
+                assert np.all(f[k] == 0.0), (c, k)
+                continue
+            assert nr > 1e-6 * ref_norms.max(), (c, k)               # the plane carries signal: the wave has reached it
+            e = np.linalg.norm(f[k] - ref) / nr
+            checked += 1
+            assert e < tol, (c, "plane", k, e)
+        ref = gold["slice_" + c].astype(np.float64)
+        e = np.linalg.norm(f[:, jsl, :] - ref) / np.linalg.norm(ref)
+        assert e < tol, (c, "slice", e)
+    assert checked >= 20                                             # 6 fields x 4 planes, minus the components the ghost plane does not hold
+    out, _ = g.run_end()
+    ref = gold["receivers"]
+    for sl in (slice(0, 3), slice(3, 6)):
+        A, B = out[0][..., sl], ref[..., sl]
+        big = np.abs(B) > 1e-3 * np.abs(B).max()
+        assert big.sum() >= 50, big.sum()
+        assert (np.abs(A - B)[big] / np.abs(B)[big]).max() < 1e-3
+    g.close()
