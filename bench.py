@@ -268,7 +268,11 @@ def run_gpu(args):
     # per-kernel durations of the two update kernels: a second pass over the same state with CUDA events around
     # every launch (emm_profile); in that pass the steps run one kernel after the other (no stream overlap, no
     # CUDA graph) so that each duration is the kernel's own
-    Kp = min(K, 50)
+    # whole DTFT groups only, so that every closing pass of the profile carries the full number of history levels (the
+    # algorithmic bytes of the instance table assume the full group)
+    Kp = min(K, 48)
+    if dtft_group > 1:
+        Kp = max(dtft_group, Kp // dtft_group * dtft_group)
     g.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=Kp + Wm + 4, batched=1 if nsrc > 1 else 0))
     g.run_enqueue(Wm)
     torch.cuda.synchronize()

@@ -1069,6 +1069,14 @@ int emmo_get(emmo_grid *g, int isrc, int what, int ifreq, void *host_out) {
     for (size_t p = 0; p < R->ndft; p++) o[R->dft_idx[p]] = S->F[((size_t)c * R->nf + ifreq) * R->ndft + p];
     return 0;
   }
+  if (what == EMMO_GET_CPML) {       /* read-out of the tables of cpml_tables(); ifreq carries the axis */
+    if (ifreq < 0 || ifreq > 2) return fail(EMMO_EINVAL, "get: bad axis");
+    double *o = (double *)host_out;
+    const int n = 2 * g->nb;
+    memcpy(o, R->am[ifreq], sizeof(double) * n); memcpy(o + n, R->bm[ifreq], sizeof(double) * n);
+    memcpy(o + 2 * n, R->ap[ifreq], sizeof(double) * n); memcpy(o + 3 * n, R->bp[ifreq], sizeof(double) * n);
+    return 0;
+  }
   if (what == EMMO_GET_JW) { memcpy(host_out, S->Jw, sizeof(cplx) * R->nf); return 0; }
   if (what == EMMO_GET_DELTA) { memcpy(host_out, S->delta, sizeof(double) * 2); return 0; }
   return fail(EMMO_EINVAL, "get: unknown item %d", what);

@@ -80,7 +80,10 @@ enum { EMMO_GET_E1 = 0, EMMO_GET_E2, EMMO_GET_E3, EMMO_GET_H1, EMMO_GET_H2, EMMO
        EMMO_GET_F_E1 = 10, EMMO_GET_F_E2, EMMO_GET_F_E3, EMMO_GET_F_H1, EMMO_GET_F_H2, EMMO_GET_F_H3, /* complex double [N3][N2][N1], zero outside the DFT set; needs ifreq */
        EMMO_GET_CE1 = 20, EMMO_GET_CE2, EMMO_GET_CE3,      /* dt/eps per component, double[N3][N2][N1] */
        EMMO_GET_JW = 30,                                   /* complex double [nfreq]: J'(omega') so far */
-       EMMO_GET_DELTA = 31                                 /* double[2]: delta_E, delta_H of the last check */
+       EMMO_GET_DELTA = 31,                                /* double[2]: delta_E, delta_H of the last check */
+       EMMO_GET_CPML = 40                                  /* double [4][2*nb] of axis `ifreq` (0,1,2): a and b of Eq. 24 at the node
+                                                              positions (D-), then a and b at the half-node positions (D+); slab
+                                                              index as L324-326 (low face 0..nb-1, high face mirrored nb..2nb-1)     */
 };
 
 /* Eq.27-29 / listing L421-443: geometric grid, n intervals, total length len, first interval dx. */

@@ -18,7 +18,7 @@ EINVAL, ENOMEM, ENOCONV, ENAN = -1, -2, -4, -5
 COMPONENTS = ("E1", "E2", "E3", "H1", "H2", "H3")
 _GET = {"E1": 0, "E2": 1, "E3": 2, "H1": 3, "H2": 4, "H3": 5,
         "F_E1": 10, "F_E2": 11, "F_E3": 12, "F_H1": 13, "F_H2": 14, "F_H3": 15,
-        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31}
+        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31, "CPML": 40}
 _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "box_lo2", "box_lo3",
          "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2")
 
@@ -144,6 +144,7 @@ class Grid:
         self._h = h
         self.ncell = (len(x) - 1, len(y) - 1, len(z) - 1)
         self.rd = rd
+        self.nb = nb
 
     def close(self):
         if getattr(self, "_h", None):
@@ -226,6 +227,8 @@ class Grid:
             out = np.zeros(self._shape_out[1], dtype=np.complex128)
         elif what == "DELTA":
             out = np.zeros(2)
+        elif what == "CPML":                 # ifreq = axis; rows: a(node), b(node), a(half node), b(half node)
+            out = np.zeros((4, 2 * self.nb))
         elif what.startswith("F_"):
             out = np.zeros(self.shape, dtype=np.complex128)
         else:

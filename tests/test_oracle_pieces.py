@@ -253,6 +253,60 @@ def test_effective_medium_unequal_widths_is_the_dual_face_average(oracle):
             assert abs(got / ref - 1) < 2e-3, (c, idx, got, ref)       # sampling error <= contrast / (2 m) per axis
 
 
+# ---- CPML coefficients (Eq. 22-24; profile of DESIGN.md [R5]) ------------------------------
+def test_cpml_coefficients_obey_eq24_and_the_profile_reflects_1e_minus_3(oracle):
+    """The oracle's a, b tables read back and taken apart with Eq. 24 itself (kappa = 1): b = exp(-(d + alpha) dt) and
+    a = d (b - 1) / (d + alpha) give rate = -ln b / dt, d = a rate / (b - 1), alpha = rate - d.  What must then hold:
+    (i) 0 < b <= 1 and -1 < a <= 0 everywhere (a stable, decaying recursion); (ii) the limits of Eq. 24: where the
+    frequency shift vanishes (depth = layer thickness and beyond) a = b - 1 exactly, and towards the inner edge a -> 0
+    like depth^2 while b -> exp(-alpha dt) (no damping, d -> 0); (iii) the damping profile is the quadratic one, the same
+    curve at node (D-) and half-node (D+) positions, and its theoretical normal-incidence reflection coefficient
+    exp(-(2/v) integral_0^L d) is the 1e-3 that [R5] states; (iv) alpha falls linearly from pi fmax / 2 at the inner edge to 0
+    at the outer one; (v) with top = AIR the surface side of z has no layer (a = 0, b = 1, L292).  A dropped factor, a
+    sign, node and half-node tables swapped, the mirrored index of L324-326 reversed or a wrong reference speed fail one
+    of these."""
+    d_ax = (100.0, 80.0, 50.0)
+    n, nb, fmax, sigma = 14, 6, 5.0, 0.8
+    nodes = [np.arange(n + 1) * d for d in d_ax]
+    for top in (oracle.TOP_CPML, oracle.TOP_AIR):
+        g = oracle.Grid(nodes[0], nodes[1], nodes[2], rd=2, nb=nb, ne=-1, top=top)
+        g.model_set(np.full((n, n, n), sigma, np.float32))
+        dt = g.info()["dt"]
+        g.run_begin([((650.0, 560.0, 350.0), (1, 0, 0))], [1.0], [[700.0, 560.0, 350.0]], dict(fixed_steps=2, fmax=fmax))
+        v = np.sqrt(2 * 2 * np.pi * 1.0 / (4e-7 * np.pi * float(np.float32(sigma))))       # 1/sqrt(mu eps), eps = sigma / (2 omega0) (L47)
+        for axis in range(3):
+            am, bm, ap, bp = g.get("CPML", ifreq=axis)
+            delta, L = d_ax[axis], nb * d_ax[axis]
+            for side in (0, 1):
+                sl = slice(0, nb) if side == 0 else slice(nb, 2 * nb)
+                if axis == 2 and side == 0 and top == oracle.TOP_AIR:
+                    assert np.all(am[sl] == 0) and np.all(ap[sl] == 0) and np.all(bm[sl] == 1) and np.all(bp[sl] == 1)      # (v)
+                    continue
+                q = np.arange(nb)
+                # depth of slab entry q into the layer: low face entry q is index q, high face entry q is index N-1-q
+                depth_node = (nb - q) * delta
+                depth_half = (nb - q) * delta + (-0.5 if side == 0 else 0.5) * delta
+                depth = np.concatenate([depth_node, depth_half])
+                a, b = np.concatenate([am[sl], ap[sl]]), np.concatenate([bm[sl], bp[sl]])
+                assert np.all((b > 0) & (b <= 1)) and np.all((a > -1) & (a <= 0))                                           # (i)
+                rate = -np.log(b) / dt
+                d = a * rate / np.expm1(-rate * dt)
+                alpha = rate - d
+                outer = depth >= L * (1 - 1e-12)
+                assert outer.sum() >= 1 and np.allclose(a[outer], b[outer] - 1, rtol=1e-13, atol=0)                           # (ii) alpha = 0
+                c = d / depth ** 2
+                assert np.allclose(c, c[0], rtol=1e-9)                                                                      # (iii) quadratic, one curve
+                refl = np.exp(-(2.0 / v) * c[0] * L ** 3 / 3.0)                                                             # integral of c xi^2 over [0, L]
+                assert abs(refl / 1e-3 - 1) < 1e-9, (axis, side, refl)
+                order = np.argsort(depth)
+                assert np.all(np.diff(np.abs(a[order])) > 0)                                                                # (ii) |a| grows with depth ...
+                inner = order[0]
+                assert abs(a[inner] / (d[inner] * dt) + 1) < rate[inner] * dt                                               # ... a -> -d dt -> 0 as d -> 0
+                assert abs(b[inner] - np.exp(-alpha[inner] * dt)) <= d[inner] * dt                                          # ... and b -> exp(-alpha dt)
+                assert np.allclose(alpha, np.maximum(np.pi * fmax / 2 * (1 - depth / L), 0), rtol=1e-9, atol=1e-9)          # (iv)
+        g.close()
+
+
 # ---- argument checking (SURVEY 8b error codes) ----------------------------------------------------
 def test_invalid_arguments(oracle):
     nodes = np.arange(9) * 10.0
