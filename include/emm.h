@@ -119,7 +119,10 @@ enum { EMM_GET_E1 = 0, EMM_GET_E2, EMM_GET_E3, EMM_GET_H1, EMM_GET_H2, EMM_GET_H
        EMM_GET_JW = 30,            /* double complex [nfreq]: J'(omega') accumulated so far (Eq. 7)     */
        EMM_GET_DELTA = 31,         /* double [2]: relative change of E and H accumulators at the last
                                       convergence check                                                  */
-       EMM_GET_DTFT_GROUP = 32     /* int: terms of Eq. 25 per accumulator pass in this run (1, or the m of dtft_pair) */
+       EMM_GET_DTFT_GROUP = 32,    /* int: terms of Eq. 25 per accumulator pass in this run (1, or the m of dtft_pair) */
+       EMM_GET_CHECK_N = 33,       /* int: number of points of the check set of this run [R9]                  */
+       EMM_GET_CHECK_ACC = 34      /* double complex [6][EMM_GET_CHECK_N]: the fp64 check-set accumulators of the lowest
+                                      frequency (Ex,Ey,Ez,Hx,Hy,Hz), complete up to the last step taken          */
 };
 
 /* ---- host-side pieces of the method (also the diagnostic surface) ------------------------------- */
@@ -194,6 +197,25 @@ int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_out);
  * instances, {E, H} accumulator-free steps of a DTFT pair, {E, H} two-term steps of a DTFT pair.      */
 int emm_profile(emm_grid *g, int enable);
 int emm_profile_read(emm_grid *g, double *ms, int *counts);
+
+/* ---- an entry point that allocates nothing -------------------------------------------------------------------------
+ * The convergence measure of the run (L385-387, DESIGN.md [R9]) as a stand-alone call for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid allocation):
+ *   delta[s][0] = || now - prev ||_2 / || now ||_2 over the three E components of source s, delta[s][1] the same over H,
+ *   NaN where the denominator is 0.
+ * It is a variant of the run driver's reduction kernels (warp shuffle + block reduction, per-block partial sums in scratch
+ * memory, added in a fixed order); its scratch is a file-scope device array inside the library, 222 KB, held by every GPU
+ * that loads the library until the process exits.  No cudaMalloc, cudaFree or allocating library routine is called.
+ *   d_acc_now, d_acc_prev  DEVICE pointers, double complex [nsrc][6][nchk] as (re,im) pairs: the check-set accumulators now
+ *                          and at the previous check (not modified)
+ *   d_delta                DEVICE pointer, double [nsrc][2], written by kernels enqueued on cuda_stream (no host sync)
+ * Limits: nsrc <= EMM_CHECK_STATIC_MAX_NSRC, nchk <= EMM_CHECK_STATIC_MAX_NCHK; larger sizes are rejected with EMM_EINVAL.
+ * All calls share the one scratch array, which keeps the last call's contents; every slot a call reads it has written
+ * itself, so nothing is cleared.  Calls that overlap on the GPU (two streams, two host threads) race on it: keep them on
+ * one stream.  The device current at the call is the one used.                                                        */
+#define EMM_CHECK_STATIC_MAX_NSRC 16
+#define EMM_CHECK_STATIC_MAX_NCHK (1 << 27)
+int emm_check_delta_static(const double *d_acc_now, const double *d_acc_prev, int nchk, int nsrc, double *d_delta, void *cuda_stream);
 
 /* number of kernel launches issued by this library since the grid was created (bench evidence) */
 long long emm_launch_count(const emm_grid *g);

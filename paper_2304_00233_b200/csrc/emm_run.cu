@@ -947,6 +947,16 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
     *static_cast<int *>(host_out) = R->group;
     return 0;
   }
+  if (what == EMM_GET_CHECK_N) {
+    *static_cast<int *>(host_out) = R->dr.nchk;
+    return 0;
+  }
+  if (what == EMM_GET_CHECK_ACC) {
+    if (R->dr.nchk <= 0) return fail(EMM_EINVAL, "emm_get: this run has no check set");
+    CU(cudaMemcpyAsync(host_out, R->dr.C + (size_t)isrc * 6 * R->dr.nchk, sizeof(double2) * 6 * R->dr.nchk, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    return 0;
+  }
   if (what == EMM_GET_DELTA) {
     CU(cudaMemcpyAsync(host_out, R->dr.delta + 2 * isrc, 2 * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
     CU(cudaStreamSynchronize(g->stream));

@@ -12,7 +12,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libemm_b200.so")
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu")]
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu", "emm_noalloc.cu")]
 _HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh", "emm_device.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
 
@@ -21,14 +21,14 @@ CHECK_CORNERS, CHECK_FACES, CHECK_FULL = 0, 1, 2
 EINVAL, ENOMEM, ECUDA, ENOCONV, ENAN = -1, -2, -3, -4, -5
 _GET = {"E1": 0, "E2": 1, "E3": 2, "H1": 3, "H2": 4, "H3": 5,
         "F_E1": 10, "F_E2": 11, "F_E3": 12, "F_H1": 13, "F_H2": 14, "F_H3": 15,
-        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31, "DTFT_GROUP": 32}
+        "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31, "DTFT_GROUP": 32, "CHECK_N": 33, "CHECK_ACC": 34}
 _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "box_lo2", "box_lo3",
          "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2", "pitch")
 # every symbol include/emm.h declares (tests check that the library exports all of them)
 SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_dipole_direction", "emm_receiver_channels", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
            "emm_grid_fdcoef", "emm_workspace_bytes", "emm_bind_device", "emm_model_set", "emm_run", "emm_run_begin",
            "emm_run_steps", "emm_run_enqueue", "emm_run_end", "emm_get", "emm_profile", "emm_profile_read",
-           "emm_launch_count", "emm_last_error")
+           "emm_launch_count", "emm_last_error", "emm_check_delta_static")
 
 
 def build(force=False, verbose=False):
@@ -98,6 +98,7 @@ def lib():
         L.emm_get.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
         L.emm_profile.argtypes = [vp, C.c_int]
         L.emm_profile_read.argtypes = [vp, dp, ip]
+        L.emm_check_delta_static.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
         L.emm_launch_count.argtypes = [vp]
         L.emm_launch_count.restype = C.c_longlong
         _lib = L
@@ -112,6 +113,27 @@ def _chk(rc, allow=()):
 
 def _dptr(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+CHECK_STATIC_MAX_NSRC = 16
+
+
+def check_delta_static(acc_now, acc_prev, out=None, stream=None):
+    """emm_check_delta_static: acc_now, acc_prev = CUDA torch tensors, complex128 [nsrc][6][nchk]; returns (or fills) a
+    CUDA float64 tensor [nsrc][2].  Marshalling only: the library call allocates nothing; `out` lets the caller supply
+    the output too (otherwise torch allocates those 16 * nsrc bytes here, outside the library)."""
+    import torch
+    assert acc_now.is_cuda and acc_prev.is_cuda and acc_now.dtype == acc_prev.dtype == torch.complex128
+    assert acc_now.is_contiguous() and acc_prev.is_contiguous() and acc_now.shape == acc_prev.shape and acc_now.dim() == 3 and acc_now.shape[1] == 6
+    nsrc, nchk = int(acc_now.shape[0]), int(acc_now.shape[2])
+    if out is None:
+        out = torch.empty((nsrc, 2), dtype=torch.float64, device=acc_now.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 2 * nsrc
+    st = stream if stream is not None else torch.cuda.current_stream(acc_now.device)
+    with torch.cuda.device(acc_now.device):
+        _chk(lib().emm_check_delta_static(C.c_void_p(acc_now.data_ptr()), C.c_void_p(acc_prev.data_ptr()), nchk, nsrc,
+                                          C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream)))
+    return out
 
 
 def emm_nugrid(n, length, dx):
@@ -320,8 +342,10 @@ class Grid:
             out = np.zeros(self._shape_out[1], dtype=np.complex128)
         elif what == "DELTA":
             out = np.zeros(2)
-        elif what == "DTFT_GROUP":
+        elif what in ("DTFT_GROUP", "CHECK_N"):
             out = np.zeros(1, dtype=np.int32)
+        elif what == "CHECK_ACC":
+            out = np.zeros((6, int(self.get("CHECK_N")[0])), dtype=np.complex128)
         elif what.startswith("F_"):
             out = np.zeros(self.shape, dtype=np.complex64)
         else:
