@@ -1081,3 +1081,61 @@ int emmo_get(emmo_grid *g, int isrc, int what, int ifreq, void *host_out) {
   if (what == EMMO_GET_DELTA) { memcpy(host_out, S->delta, sizeof(double) * 2); return 0; }
   return fail(EMMO_EINVAL, "get: unknown item %d", what);
 }
+
+/* ------------------------------------------------------------------------------------------ */
+/* Sensitivity kernel, DESIGN.md [R14].  The diffusive equations (Eq. 1) read curl H - sigma E = J, so a change
+ * d sigma of the medium acts on the field E like the source current d sigma * E: the datum changes by
+ *   d d = integral G(receiver; x) d sigma(x) E(x) dV,  G(receiver; x) = G(x; receiver) by reciprocity.
+ * On the grid sigma enters only through the effective conductivities sigma_bar_c of the E nodes (model_set, [R3]),
+ * so the derivative with respect to one cell is the chain rule over the nodes whose average contains that cell;
+ * the volume element of node n is the V(n) of the source injection [R7].  Plain scatter loop, node by node.     */
+int emmo_sensitivity(emmo_grid *g, int isrc, int iadj, int ifreq, double *out_h_, double *out_v_) {
+  if (!g || !g->run || !out_h_ || !out_v_) return fail(EMMO_EINVAL, "sensitivity: no run in progress or null output");
+  runstate *R = g->run;
+  if (isrc < 0 || isrc >= R->nsrc || iadj < 0 || iadj >= R->nsrc || ifreq < 0 || ifreq >= R->nf) return fail(EMMO_EINVAL, "sensitivity: bad source or frequency index");
+  if (R->sparse) return fail(EMMO_EINVAL, "sensitivity: needs full-grid accumulators (sparse_dft = 0)");
+  const srcstate *Sa = &R->s[isrc], *Sb = &R->s[iadj];
+  if (Sa->magnetic || Sb->magnetic) return fail(EMMO_EINVAL, "sensitivity: electric sources only");
+  if (R->dtft_every != 1) return fail(EMMO_EINVAL, "sensitivity: needs every term of the DTFT");
+  cplx *out_h = (cplx *)out_h_, *out_v = (cplx *)out_v_;
+  const int nx = g->nc[0], ny = g->nc[1], nz = g->nc[2], nf = R->nf;
+  const size_t ncell = (size_t)nx * ny * nz;
+  for (size_t t = 0; t < ncell; t++) { out_h[t] = 0; out_v[t] = 0; }
+  const cplx sq = csqrt(-I * 2 * M_PI * R->freqs[ifreq] / (2 * g->w0));       /* Eq. 7a: G^EE = sq F_E / J' */
+  const cplx ga = sq / Sa->Jw[ifreq], gb = sq / Sb->Jw[ifreq];
+  const double *X[3] = {g->xn[0], g->xn[1], g->xn[2]};
+  for (size_t p = 0; p < R->ndft; p++) {
+    const size_t t = R->dft_idx[p];
+    const int i = (int)(t % (size_t)g->N[0]), j = (int)((t / (size_t)g->N[0]) % (size_t)g->N[1]), k = (int)(t / ((size_t)g->N[0] * g->N[1]));
+    const int idx[3] = {i, j, k};
+    for (int c = 0; c < 3; c++) {
+      const cplx P = (ga * Sa->F[((size_t)c * nf + ifreq) * R->ndft + p]) * (gb * Sb->F[((size_t)c * nf + ifreq) * R->ndft + p]);
+      if (P == 0) continue;
+      const double V = node_width(g, 0, LAT[c][0], i) * node_width(g, 1, LAT[c][1], j) * node_width(g, 2, LAT[c][2], k);
+      /* the four cells sharing the edge of component c at this node, and their area weights: as in emmo_model_set */
+      const int a1 = (c + 1) % 3, a2 = (c + 2) % 3;
+      double w[4], wsum = 0; int q1[4], q2[4];
+      for (int d1 = -1, n = 0; d1 <= 0; d1++) for (int d2 = -1; d2 <= 0; d2++, n++) {
+        q1[n] = idx[a1] + d1 > 0 ? idx[a1] + d1 : 0;
+        q2[n] = idx[a2] + d2 > 0 ? idx[a2] + d2 : 0;
+        w[n] = (X[a1][q1[n] + 1] - X[a1][q1[n]]) * (X[a2][q2[n] + 1] - X[a2][q2[n]]);
+      }
+      /* the denominator of the average is (d0 + d1) of either transverse axis */
+      {
+        const int m1 = idx[a1] > 0 ? idx[a1] - 1 : 0, m2 = idx[a2] > 0 ? idx[a2] - 1 : 0;
+        wsum = ((X[a1][m1 + 1] - X[a1][m1]) + (X[a1][idx[a1] + 1] - X[a1][idx[a1]])) * ((X[a2][m2 + 1] - X[a2][m2]) + (X[a2][idx[a2] + 1] - X[a2][idx[a2]]));
+      }
+      for (int n = 0; n < 4; n++) {
+        int q[3]; q[c] = idx[c]; q[a1] = q1[n]; q[a2] = q2[n];
+        int ci = q[0] - g->lo[0], cj = q[1] - g->lo[1], ck = q[2] - g->lo[2];
+        if (g->top == EMMO_TOP_AIR && ck < 0) continue;                       /* air above the surface: not a model parameter */
+        ci = ci < 0 ? 0 : (ci > nx - 1 ? nx - 1 : ci);                        /* padding replicates the edge cell [R1] */
+        cj = cj < 0 ? 0 : (cj > ny - 1 ? ny - 1 : cj);
+        ck = ck < 0 ? 0 : (ck > nz - 1 ? nz - 1 : ck);
+        const size_t cell = (size_t)ci + (size_t)nx * ((size_t)cj + (size_t)ny * (size_t)ck);
+        if (c == 2) out_v[cell] += w[n] / wsum * V * P; else out_h[cell] += w[n] / wsum * V * P;
+      }
+    }
+  }
+  return 0;
+}

@@ -118,6 +118,18 @@ int emmo_run_steps(emmo_grid *g, int n, int *nsteps /* [nsrc] steps executed so 
 int emmo_run_end(emmo_grid *g, double *out, int *nsteps);
 int emmo_get(emmo_grid *g, int isrc, int what, int ifreq, void *host_out);
 
+/* Sensitivity (Frechet) kernel of a measured electric field with respect to the cell conductivities -- what the
+ * full-grid frequency-domain fields are kept for (inversion is the stated perspective; the paper
+ * gives no formula, DESIGN.md [R14] states the one used).  Needs a run in progress with full-grid accumulators
+ * (sparse_dft = 0) holding two electric sources: `isrc` = the transmitter, `iadj` = a unit dipole at the receiver,
+ * polarised along the receiver channel.  For the datum d = sum_c dir_c G^EE_c(receiver; transmitter) of frequency ifreq:
+ *   out_h[cell] = d d / d sigma_h[cell],  out_v[cell] = d d / d sigma_v[cell]   (complex double [nz][ny][nx] each),
+ * = sum over the E nodes n whose effective conductivity (Eq. 26, [R3]) contains the cell:
+ *   (d sigma_bar_c(n) / d sigma[cell]) * V(n) * G_c(n; transmitter) * G_c(n; receiver dipole),
+ * G = Green's functions on the grid (Eq. 7), V(n) = node volume of the component's lattice ([R7]); sigma_h collects the
+ * x and y components, sigma_v the z component.  Padding cells count towards the model cell they replicate.            */
+int emmo_sensitivity(emmo_grid *g, int isrc, int iadj, int ifreq, double *out_h, double *out_v);
+
 const char *emmo_last_error(void);
 
 #ifdef __cplusplus

@@ -80,6 +80,7 @@ def lib():
         L.emmo_run_steps.argtypes = [vp, C.c_int, ip, ip]
         L.emmo_run_end.argtypes = [vp, dp, ip]
         L.emmo_get.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+        L.emmo_sensitivity.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, dp]
         _lib = L
     return _lib
 
@@ -220,6 +221,12 @@ class Grid:
         ns = np.zeros(self._shape_out[0], dtype=np.int32)
         _chk(lib().emmo_run_end(self._h, out.ctypes.data_as(C.POINTER(C.c_double)), ns.ctypes.data_as(C.POINTER(C.c_int))))
         return out, ns
+
+    def sensitivity(self, isrc, iadj, ifreq):
+        nx, ny, nz = self.ncell
+        kh, kv = np.zeros((nz, ny, nx), dtype=np.complex128), np.zeros((nz, ny, nx), dtype=np.complex128)
+        _chk(lib().emmo_sensitivity(self._h, isrc, iadj, ifreq, kh.ctypes.data_as(C.POINTER(C.c_double)), kv.ctypes.data_as(C.POINTER(C.c_double))))
+        return kh, kv
 
     def get(self, what, isrc=0, ifreq=0):
         code = _GET[what]

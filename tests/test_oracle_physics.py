@@ -391,3 +391,62 @@ def test_wholespace_magnetic_dipole_by_duality(oracle):
     ref = wholespace_dipole(src, rec, 1.0, 1.0, p=m / np.linalg.norm(m))
     refM = np.concatenate([-ref[:, 3:], (1j * 1.0 / (2 * np.pi * 1.0 * MU0)) * ref[:, :3]], axis=1)
     assert _relerr(out[0, 0], refM).max() < 5e-3           # measured 1.0e-3 .. 1.6e-3
+
+
+# ---- sensitivity kernel (DESIGN.md [R14]) --------------------------------------------------------------
+def _datum(oracle, x, sh, sv, src, rec_pos, rec_dir, nsteps):
+    g = oracle.Grid(x, x, x, rd=2, nb=6, ne=-1)
+    g.model_set(sh, sv)
+    out, _ = g.run([src], [1.0], [rec_pos], dict(fixed_steps=nsteps))
+    dt = g.info()["dt"]
+    g.close()
+    return out[0, 0, 0, :3] @ rec_dir, dt
+
+
+@pytest.mark.parametrize("which", ["h", "v"])
+def test_sensitivity_kernel_equals_finite_differences_of_the_datum(oracle, which):
+    """Brute force on a small grid: the datum d = dir . G^EE(receiver; transmitter) is recomputed with the conductivity of a
+    2 x 2 x 2 block of cells raised and lowered by 2 % (sigma_h or sigma_v alone); the central difference must equal the sum of
+    the kernel over the block.  Off-grid transmitter and receiver, oblique polarisations, VTI background, so that every
+    component, both conductivities and the interpolation weights take part.  A wrong sign, a missing node volume, a factor
+    of 2 or 4 in the cell weights, a conjugate, or sigma_h / sigma_v mixed up are all far outside the 0.2 % bound (measured:
+    3.2e-4 for either conductivity, the size of the neglected third-order term and of the asymmetry of the 4th-order operators
+    at the absorbing layer)."""
+    n = 16
+    x = np.arange(n + 1) * 100.0
+    sh = np.full((n, n, n), 1.0, np.float32)
+    sv = np.full((n, n, n), 0.7, np.float32)
+    sh[0, 0, 0] = sv[0, 0, 0] = 0.4                      # the slowest-decaying corner fixes the time step in all three runs
+    src = ((640.0, 730.0, 780.0), (1.0, 0.4, -0.3))
+    rec_pos = (1060.0, 870.0, 830.0)
+    rec_dir = np.array([0.3, 0.8, 0.5]) / np.linalg.norm([0.3, 0.8, 0.5])
+    blk = (slice(7, 9), slice(7, 9), slice(8, 10))       # between the two
+    g = oracle.Grid(x, x, x, rd=2, nb=6, ne=-1)
+    g.model_set(sh, sv)
+    nsteps = int(4.5 / g.info()["dt"])
+    g.run_begin([src, (rec_pos, tuple(rec_dir))], [1.0], [rec_pos], dict(fixed_steps=nsteps))
+    g.run_steps(nsteps)
+    kh, kv = g.sensitivity(0, 1, 0)
+    kh2, kv2 = g.sensitivity(1, 0, 0)
+    assert np.array_equal(kh, kh2) and np.array_equal(kv, kv2)       # the kernel does not care which of the two is called the transmitter
+    out, _ = g.run_end()
+    d0 = out[0, 0, 0, :3] @ rec_dir
+    g.close()
+    k = kh if which == "h" else kv
+    assert np.abs(k[blk]).min() > 1e-3 * np.abs(k).max()              # the block sits where the kernel lives
+    eps = 0.02
+    dd, dts = [], []
+    for sgn in (+1, -1):
+        a, b = sh.copy(), sv.copy()
+        (a if which == "h" else b)[blk] *= (1 + sgn * eps)
+        d, dt = _datum(oracle, x, a, b, src, rec_pos, rec_dir, nsteps)
+        dd.append(d)
+        dts.append(dt)
+    assert dts[0] == dts[1]
+    base = float((sh if which == "h" else sv)[blk].flat[0])
+    fd = (dd[0] - dd[1]) / (2 * eps * base)
+    assert abs(fd) > 1e-4 * abs(d0) / base                               # a measurable change, far above round-off
+    pred = k[blk].sum()
+    assert abs(pred - fd) < 2e-3 * abs(fd), (pred, fd, abs(pred - fd) / abs(fd))
+    other = (kv if which == "h" else kh)[blk].sum()
+    assert abs(other - fd) > 0.2 * abs(fd)                               # and the other conductivity's kernel is not it
