@@ -191,6 +191,20 @@ int emm_run_enqueue(emm_grid *g, int n);
 int emm_run_end(emm_grid *g, double *out, int *nsteps);
 int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_out);
 
+/* Sensitivity (Frechet) kernel of a measured electric field with respect to the cell conductivities: what the full-grid
+ * frequency-domain fields are accumulated for (inversion is the stated purpose; the paper gives no
+ * formula, DESIGN.md [R14] states the one used).  Needs a run in progress (between emm_run_begin and emm_run_end) with
+ * full-grid accumulators (sparse_dft = 0, dtft_every = 1) that holds two electric sources resident together: `isrc` = the
+ * transmitter, `iadj` = a unit dipole at the receiver, polarised along the receiver channel.  For the datum
+ * d = sum_c dir_c G^EE_c(receiver; transmitter) of frequency `ifreq`:
+ *   out_h[cell] = d d / d sigma_h[cell],  out_v[cell] = d d / d sigma_v[cell]
+ * HOST buffers, double complex [nz][ny][nx] as (re,im) pairs, caller-owned, overwritten.  Each value is the cell volume / 4
+ * times the sum, over the cell's four edges per direction, of the product of the two sources' Green's functions (Eq. 7) at
+ * the edge node: x and y edges into sigma_h, z edges into sigma_v; edge nodes outside the DTFT box do not count, padding
+ * cells count towards the model cell they replicate.  fp64 products of the fp32 accumulators, a fixed summation order.
+ * Errors: EMM_EINVAL (no run, magnetic source, receivers-only or decimated DTFT, a run with one source, bad index).      */
+int emm_sensitivity(emm_grid *g, int isrc, int iadj, int ifreq, double *out_h, double *out_v);
+
 /* Optional timing of the two fused update kernels: emm_profile(g,1) brackets every later launch of the
  * E and H update kernel with CUDA events on the bound stream; emm_profile_read drains the stream and
  * returns the summed durations and launch counts, then resets.  ms[6], counts[6]: {E, H} one-term (or decimated)

@@ -35,6 +35,9 @@ struct DevRun {
   // air boundary scratch: complex planes [1 + r][M2][M1] (plane route) or sep_air_scratch() elements (separable route)
   float2 *air = nullptr;
   void *sp_ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // cuFFT work areas of the separable route
+  // emm_sensitivity: [2][sens_layers][ny][nx] (d/d sigma_h, d/d sigma_v) of the cell layers in flight
+  double2 *sens = nullptr;
+  int sens_layers = 0;
 };
 
 // one E (is_h=0) or H (is_h=1) update of every unfinished source: curl + CPML + update + DTFT
@@ -74,5 +77,9 @@ int launch_model_scan(emm_grid *g, const float *d_sh, const float *d_sv, unsigne
 int launch_gather_cells(emm_grid *g, const float *d_sh, const float *d_sv, const long long *d_idx, const int *d_which, int n, float *d_out);
 int launch_sigma_min(emm_grid *g, const float *d_sh, const float *d_sv, double *d_min);
 int launch_make_ce(emm_grid *g, const float *d_sh, const float *d_sv, double scale);
+// sensitivity kernel of an E-field datum (emm_sens.cu): cell layers [ck0, ck0 + nlayers) into d_h / d_v [nlayers][ny][nx]
+constexpr int kSensLayers = 8;
+int launch_sensitivity(emm_grid *g, const DevState &s, int isrc, int iadj, int ifreq, double scale_re, double scale_im, int ck0,
+                       int nlayers, double2 *d_h, double2 *d_v);
 
 }  // namespace emm

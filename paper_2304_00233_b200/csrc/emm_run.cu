@@ -168,6 +168,9 @@ static void layout_run(emm_grid *g, Arena &A, int nsrc, int nf, int nf_rec, int 
   for (int a = 0; a < 3; ++a)            // CPML coefficients (Eq. 24) at node and half-node positions
     for (int q = 0; q < 4; ++q) r.cpml[a][q] = A.take<float>(2 * g->nb);
   r.red_part = A.take<double>((size_t)nsrc * 6 * 2 * kCheckBlocks);
+  // emm_sensitivity: the kernel leaves the device a few cell layers at a time (two sources with full-grid accumulators needed)
+  r.sens_layers = nf > 0 && nsrc >= 2 ? std::min(g->nc[2], kSensLayers) : 0;
+  r.sens = A.take<double2>((size_t)2 * r.sens_layers * g->nc[1] * g->nc[0]);
 }
 
 template <class T>
@@ -963,6 +966,35 @@ extern "C" int emm_get(emm_grid *g, int isrc, int what, int ifreq, void *host_ou
     return 0;
   }
   return fail(EMM_EINVAL, "emm_get: unknown item %d", what);
+}
+
+// Sensitivity kernel of an electric-field datum with respect to the cell conductivities (DESIGN.md [R14]):
+// Eq. 7 scaling of the two sources' accumulators on the host (fp64), the gather over edges and padded cells on the device
+// (emm_sens.cu), a few cell layers at a time through the run's scratch.
+extern "C" int emm_sensitivity(emm_grid *g, int isrc, int iadj, int ifreq, double *out_h, double *out_v) {
+  if (!g || !g->run || !out_h || !out_v) return fail(EMM_EINVAL, "emm_sensitivity: no run in progress or null output");
+  Run *R = g->run;
+  if (isrc < 0 || isrc >= R->nsrc || iadj < 0 || iadj >= R->nsrc || ifreq < 0 || ifreq >= R->nf)
+    return fail(EMM_EINVAL, "emm_sensitivity: bad source or frequency index");
+  if (R->sparse || R->ds.nf < 1) return fail(EMM_EINVAL, "emm_sensitivity: needs full-grid accumulators (sparse_dft = 0)");
+  if (R->mag[isrc] || R->mag[iadj]) return fail(EMM_EINVAL, "emm_sensitivity: electric sources only");
+  if (R->dtft_every != 1) return fail(EMM_EINVAL, "emm_sensitivity: needs every term of the DTFT (dtft_every = 1)");
+  if (R->dr.sens_layers < 1) return fail(EMM_EINVAL, "emm_sensitivity: the run holds a single source (transmitter and receiver dipole must be resident together)");
+  int rc;
+  if ((rc = fetch_flags(g))) return rc;
+  const std::complex<double> I(0, 1);
+  const std::complex<double> sc = std::sqrt(-I * 2.0 * kPi * R->freqs[ifreq] / (2 * g->w0));   // Eq. 7a, principal root
+  const std::complex<double> scale = (sc / source_spectrum(g, R, isrc, ifreq)) * (sc / source_spectrum(g, R, iadj, ifreq)) * 0.25;
+  const size_t layer = (size_t)g->nc[0] * g->nc[1];
+  double2 *dh = R->dr.sens, *dv = R->dr.sens + (size_t)R->dr.sens_layers * layer;
+  for (int k = 0; k < g->nc[2]; k += R->dr.sens_layers) {
+    const int n = std::min(R->dr.sens_layers, g->nc[2] - k);
+    if ((rc = launch_sensitivity(g, R->ds, isrc, iadj, ifreq, scale.real(), scale.imag(), k, n, dh, dv))) return rc;
+    CU(cudaMemcpyAsync(out_h + 2 * (size_t)k * layer, dh, sizeof(double2) * n * layer, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaMemcpyAsync(out_v + 2 * (size_t)k * layer, dv, sizeof(double2) * n * layer, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+  }
+  return 0;
 }
 
 // ---- optional per-kernel timing (bench evidence for the roofline of the dominant kernel) ----

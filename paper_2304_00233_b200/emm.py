@@ -12,7 +12,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libemm_b200.so")
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu", "emm_noalloc.cu")]
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu", "emm_sens.cu", "emm_noalloc.cu")]
 _HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh", "emm_device.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
 
@@ -28,7 +28,7 @@ _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "
 SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_dipole_direction", "emm_receiver_channels", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
            "emm_grid_fdcoef", "emm_workspace_bytes", "emm_bind_device", "emm_model_set", "emm_run", "emm_run_begin",
            "emm_run_steps", "emm_run_enqueue", "emm_run_end", "emm_get", "emm_profile", "emm_profile_read",
-           "emm_launch_count", "emm_last_error", "emm_check_delta_static")
+           "emm_launch_count", "emm_last_error", "emm_check_delta_static", "emm_sensitivity")
 
 
 def build(force=False, verbose=False):
@@ -96,6 +96,7 @@ def lib():
         L.emm_run_enqueue.argtypes = [vp, C.c_int]
         L.emm_run_end.argtypes = [vp, dp, ip]
         L.emm_get.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+        L.emm_sensitivity.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, dp]
         L.emm_profile.argtypes = [vp, C.c_int]
         L.emm_profile_read.argtypes = [vp, dp, ip]
         L.emm_check_delta_static.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
@@ -352,6 +353,13 @@ class Grid:
             out = np.zeros(self.shape, dtype=np.float32)
         _chk(lib().emm_get(self._h, isrc, code, ifreq, out.ctypes.data_as(C.c_void_p)))
         return out
+
+    def sensitivity(self, isrc, iadj, ifreq):
+        """(d/d sigma_h, d/d sigma_v) of the E-field datum of transmitter `isrc` and receiver dipole `iadj`, complex [nz][ny][nx]."""
+        nx, ny, nz = self.ncell
+        kh, kv = np.zeros((nz, ny, nx), dtype=np.complex128), np.zeros((nz, ny, nx), dtype=np.complex128)
+        _chk(lib().emm_sensitivity(self._h, isrc, iadj, ifreq, kh.ctypes.data_as(C.POINTER(C.c_double)), kv.ctypes.data_as(C.POINTER(C.c_double))))
+        return kh, kv
 
     def profile(self, enable=True):
         _chk(lib().emm_profile(self._h, int(enable)))

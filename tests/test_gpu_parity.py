@@ -330,6 +330,65 @@ def test_magnetic_and_mixed_sources_match_oracle(emm, oracle):
     _field_parity(emm, oracle, w, 120, sources=srcs, batched=1)
 
 
+@pytest.mark.parametrize("case", ["air_nonuniform_vti", "wholespace_cpml"])
+def test_sensitivity_kernel_matches_oracle(emm, oracle, case):
+    """SURVEY 8f rank 4 (gradient accumulation, DESIGN.md [R14]): emm_sensitivity against emmo_sensitivity, cell by cell,
+    for d/d sigma_h and d/d sigma_v.  The oracle chains every E node through its Eq. 26 weights and node volume; the CUDA
+    path gathers cell volume / 4 times the edge products per cell -- two derivations of the same sum.  Oblique off-grid
+    dipoles so that all three components carry weight; the non-uniform case has the air layer (not a parameter) and VTI
+    cells, the whole-space case a CPML on all six faces (padding cells fold into the edge cells on every side).
+    Tolerance: the accumulators of either source are within 2e-5 relative L2 of the oracle's (the accumulator tolerance
+    above), their product within 4e-5; 1e-4 on each kernel as a whole, and 1e-3 on the outermost shell of model cells taken
+    alone (values 1e-3 .. 1e-6 of the peak: what the fold of the padding cells produces)."""
+    if case == "air_nonuniform_vti":
+        w = W.build("cfg3", oracle.nugrid, nx=40, nz=36, rd=2, nb=8, n_water=8, n_rec_side=3, aux_dx=50.0)
+        w["sigma_v"] = (w["sigma_v"] * 0.6).astype(np.float32)
+        srcs = [((-150.0, 30.0, 950.0), (1.0, 0.2, 0.1)), ((260.0, -110.0, 1000.0), (0.3, 0.8, 0.5))]
+        nsteps = 300
+    else:
+        w = W.cfg1(n=30, dx=100.0, rd=3, nb=7)
+        c = np.array(w["sources"][0][0])
+        srcs = [(tuple(c + [-340.0, 30.0, 20.0]), (1.0, 0.4, -0.3)), (tuple(c + [330.0, -60.0, 110.0]), (0.2, 0.5, 0.8))]
+        nsteps = 200
+    ga, gb = make_grid(emm, w), make_grid(oracle, w)
+    opts = dict(fixed_steps=nsteps, batched=1)
+    for g in (ga, gb):
+        g.run_begin(srcs, w["freqs"][:2] if len(w["freqs"]) > 1 else w["freqs"], w["receivers"], opts)
+        g.run_steps(nsteps)
+    f = 1 if len(w["freqs"]) > 1 else 0
+    ka, kb = ga.sensitivity(0, 1, f), gb.sensitivity(0, 1, f)
+    kswap = ga.sensitivity(1, 0, f)
+    shell = np.ones(kb[0].shape, bool)
+    shell[1:-1, 1:-1, 1:-1] = False
+    for q, name in enumerate(("sigma_h", "sigma_v")):
+        A, B = ka[q], kb[q]
+        assert np.all(np.isfinite(A.view(np.float64)))
+        assert np.array_equal(A, kswap[q])                                   # symmetric in the two sources, to the last bit
+        assert np.linalg.norm(B) > 0 and np.abs(B[~shell]).max() > 0
+        assert _rel_l2(A, B) < 1e-4, (case, name, _rel_l2(A, B))
+        assert np.linalg.norm(B[shell]) > 0
+        assert _rel_l2(A[shell], B[shell]) < 1e-3, (case, name, "shell", _rel_l2(A[shell], B[shell]))
+        assert np.all(A[B == 0] == 0), (case, name)                          # cells out of reach of the DTFT box are exactly zero
+    # the calls it must refuse
+    with pytest.raises(emm.EmmError):
+        ga.sensitivity(0, 2, f)
+    with pytest.raises(emm.EmmError):
+        ga.sensitivity(0, 1, 7)
+    ga.run_end()
+    ga.run_begin(srcs[:1], w["freqs"][:1], w["receivers"], dict(fixed_steps=8))
+    ga.run_steps(8)
+    with pytest.raises(emm.EmmError):
+        ga.sensitivity(0, 0, 0)                                              # a run with a single resident source
+    ga.run_end()
+    ga.run_begin([srcs[0], srcs[1] + ("M",)], w["freqs"][:1], w["receivers"], dict(fixed_steps=8, batched=1))
+    ga.run_steps(8)
+    with pytest.raises(emm.EmmError):
+        ga.sensitivity(0, 1, 0)                                              # magnetic receiver dipole
+    ga.run_end()
+    ga.close()
+    gb.close()
+
+
 def test_converged_run_matches_oracle_steps_and_receivers(emm, oracle):
     """configs[1] scaled, run to convergence: integer step count exact, receivers within 1e-3."""
     w = W.cfg2(nx=40, nz=28, dx=100.0, rd=2, nb=8)
