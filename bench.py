@@ -45,16 +45,22 @@ def build_workload(args, nugrid):
                 w["receivers"] = np.zeros((0, 3))
     else:
         w = W.build(args.workload, None, **({"rd": args.rd} if args.rd else {}))
+    if args.air_route:
+        w["grid"] = dict(w["grid"], air_route=args.air_route)
     return w
 
 
 def describe(w, info, nsrc):
-    return {"workload": "%s: %dx%dx%d cells, rd=%d (order %d), %s, nf=%d, nsrc=%d, padded %dx%dx%d" % (
+    d = {"workload": "%s: %dx%dx%d cells, rd=%d (order %d), %s, nf=%d, nsrc=%d, padded %dx%dx%d" % (
         w["name"], len(w["x"]) - 1, len(w["y"]) - 1, len(w["z"]) - 1, w["grid"]["rd"], 2 * w["grid"]["rd"],
         "non-uniform" if not info["uniform_xy"] else "uniform x-y", len(w["freqs"]), nsrc, info["N1"], info["N2"], info["N3"]),
         "padded_nodes": info["N1"] * info["N2"] * info["N3"],
         "air_plane": [info["aux_M1"], info["aux_M2"]],
         "l2": "working set (fields + DTFT accumulators) is >> the 126 MB L2; no flush needed"}
+    if "air_cluster" in info:             # the CUDA library's grid (the oracle has its own plain transforms)
+        d["air_boundary"] = ("none" if info["k0"] < 0 else "one launch per pass: %d-CTA cluster, plane in distributed shared memory" % info["air_cluster"]
+                             if info["air_cluster"] else "library 2-D transforms" if info["uniform_xy"] else "separable route, batched 1-D library transforms")
+    return d
 
 
 def algorithmic_bytes(info, nf, nb, kernel, m=1):
@@ -124,6 +130,7 @@ def oracle_rate(w_full, budget_s, steps, warmup, args):
     for _ in range(3):
         a2 = argparse.Namespace(**vars(args))
         a2.scale = scale
+        a2.air_route = 0                  # a scheduling option of the CUDA library, not of the method
         w = build_workload(a2, O.nugrid)
         g = O.Grid(w["x"], w["y"], w["z"], **w["grid"])
         g.model_set(w["sigma_h"], w.get("sigma_v"))
@@ -146,6 +153,7 @@ def oracle_rate(w_full, budget_s, steps, warmup, args):
         scale = new_scale
     a2 = argparse.Namespace(**vars(args))
     a2.scale = scale
+    a2.air_route = 0
     w = build_workload(a2, O.nugrid)
     g = O.Grid(w["x"], w["y"], w["z"], **w["grid"])
     g.model_set(w["sigma_h"], w.get("sigma_v"))
@@ -501,6 +509,7 @@ def main():
     ap.add_argument("--nf", type=int, default=0, help="keep only the first nf frequencies; -1 = none (pure E/H update, no DTFT)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the cell counts (debugging only)")
     ap.add_argument("--aux-dx", type=float, default=0.0)
+    ap.add_argument("--air-route", type=int, default=0, help="emm_grid_opts.air_route (1 = library / plane-sized route of the air-water boundary)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-rd2", action="store_true", help="skip the extra 4th-order (rd = 2) run of configs[3]")
     ap.add_argument("--converge", action="store_true", help="time to converged in the four DTFT schedules instead of the step benchmark")

@@ -51,7 +51,10 @@ typedef struct {
   int air_route; /* air boundary on a non-uniform x-y grid: 0 = separable route (interpolation and transform one
                     axis at a time, batched 1-D transforms; default), 1 = plane-sized route (interpolate to the whole
                     auxiliary plane, 2-D transforms): the same linear map up to rounding order, about twice the
-                    work; kept as the cross-check of the separable route.  Ignored on uniform x-y.              */
+                    work; kept as the cross-check of the separable route.  On a uniform x-y grid: 0 = the whole boundary in
+                    one launch per pass by a thread-block cluster that holds the plane in shared memory (hand-written
+                    transforms; planes up to about 280 x 280, larger ones take the library route), 1 = library route
+                    (pack, 2-D cuFFT, filter, 2-D cuFFT, unpack): the same linear map up to rounding order.          */
 } emm_grid_opts;
 
 typedef struct {
@@ -107,6 +110,8 @@ enum { EMM_I_N1 = 0, EMM_I_N2, EMM_I_N3,          /* padded array dims n?pad (L3
        EMM_I_BOX_HI1, EMM_I_BOX_HI2, EMM_I_BOX_HI3, /* inclusive                                         */
        EMM_I_AUX_M1, EMM_I_AUX_M2,                /* FFT plane of the air boundary                       */
        EMM_I_PITCH,                               /* floats per x row in device memory                   */
+       EMM_I_AIR_CLUSTER,                         /* CTAs of the cluster that runs the air boundary in one launch
+                                                     (uniform x-y, after emm_bind_device); 0 = library / separable route */
        EMM_I_COUNT };
 
 /* items for emm_get(): state of the run in progress / last finished run */

@@ -174,6 +174,7 @@ __global__ void k_air_filter_H(const AirArgs a, const float *__restrict__ kx, co
 
 int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st) {
   if (g->sep_air) return launch_air_sep(g, s, r, is_h, st);
+  if (g->air_cluster) return launch_air_cluster(g, s, r, is_h, st);
   const int R = g->r;
   const int nlev = is_h ? R : R - 1;
   if (nlev <= 0) return 0;

@@ -297,6 +297,7 @@ extern "C" int emm_grid_info(const emm_grid *g, int *ints, double *dt) {
     ints[EMM_I_AUX_M1] = g->M1;
     ints[EMM_I_AUX_M2] = g->M2;
     ints[EMM_I_PITCH] = g->P1;
+    ints[EMM_I_AIR_CLUSTER] = g->air_cluster;
   }
   if (dt) *dt = g->have_model ? g->dt : 0.0;
   return 0;

@@ -92,6 +92,7 @@ struct DevTables {             // device pointers of the per-grid region
   int *ta_start[2][2], *fa_start[2][2];   // [axis][lattice]: lattice -> aux plane, aux plane -> lattice
   float *ta_w[2][2], *fa_w[2][2];
   float *kx, *ky;                          // signed wavenumbers of the FFT plane
+  float2 *tw1, *tw2;                       // e^{-2 pi i k/M1}, e^{-2 pi i k/M2}: twiddles of the cluster route (emm_air_cluster.cu)
   void *fft_ws[3];
 };
 
@@ -116,6 +117,8 @@ struct emm_grid {
   int P1 = 0, XS = 0;
   // air boundary
   int M1 = 0, M2 = 0;
+  int air_cluster = 0;                   // uniform x-y: cluster size of the one-launch boundary (emm_air_cluster.cu), 0 = library route
+  int air_cluster_lg = 0;                // ... and the ghost levels it holds in shared memory at a time
   bool sep_air = false;                  // non-uniform x-y: separable route (emm_air_sep.cu) instead of plane-sized 2-D transforms
   double dxa = 0, dya = 0;
   std::vector<emm::Stencil1> toaux[2][2], fromaux[2][2];

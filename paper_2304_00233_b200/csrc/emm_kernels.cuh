@@ -70,6 +70,10 @@ int launch_rec_interp(emm_grid *g, const DevState &s, const DevRun &r, int nf, i
 int launch_air(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
 // separable route of the same boundary for non-uniform x-y (emm_air_sep.cu); launch_air dispatches to it when g->sep_air
 int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
+// one-launch route for a uniform x-y plane that fits the shared memory of a thread-block cluster (emm_air_cluster.cu);
+// air_cluster_plan picks the cluster size on the current device (0: does not fit), launch_air dispatches when g->air_cluster
+int air_cluster_plan(emm_grid *g);
+int launch_air_cluster(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cudaStream_t st);
 size_t sep_air_scratch(const emm_grid *g, int nsrc);
 int sep_air_make_plans(emm_grid *g, int nsrc);
 // model: effective medium (Eq. 26) -> min sigma (for Eq. 15) and dt/eps

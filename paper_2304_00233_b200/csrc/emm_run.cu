@@ -87,6 +87,8 @@ static void layout_fixed(emm_grid *g, Arena &A) {
   if (g->top == EMM_TOP_AIR) {
     g->T.kx = A.take<float>(g->M1);
     g->T.ky = A.take<float>(g->M2);
+    g->T.tw1 = A.take<float2>(g->M1);
+    g->T.tw2 = A.take<float2>(g->M2);
     if (!g->uniform_xy)
       for (int a = 0; a < 2; ++a)
         for (int l = 0; l < 2; ++l) {
@@ -267,6 +269,9 @@ extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, voi
       std::vector<float> k(M);
       for (int n = 0; n < M; ++n) k[n] = (float)(2.0 * kPi * (double)(n <= M / 2 ? n : n - M) / ((double)M * d));
       if ((rc = upload(g, a == 0 ? g->T.kx : g->T.ky, k))) return rc;
+      std::vector<float2> tw(M);
+      for (int n = 0; n < M; ++n) tw[n] = make_float2((float)std::cos(2.0 * kPi * n / M), (float)-std::sin(2.0 * kPi * n / M));
+      if ((rc = upload(g, a == 0 ? g->T.tw1 : g->T.tw2, tw))) return rc;
       if (!g->uniform_xy)
         for (int l = 0; l < 2; ++l) {
           std::vector<int> st(M), sf(g->N[a]);
@@ -277,6 +282,7 @@ extern "C" int emm_bind_device(emm_grid *g, void *d_workspace, size_t bytes, voi
               (rc = upload(g, g->T.fa_start[a][l], sf)) || (rc = upload(g, g->T.fa_w[a][l], wf))) return rc;
         }
     }
+    air_cluster_plan(g);
     cufftHandle pl[3] = {g->plan_fwd, g->plan_inv_e, g->plan_inv_h};
     const int batch[3] = {1, g->r - 1, g->r};
     for (int q = 0; q < 3; ++q) {

@@ -12,7 +12,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libemm_b200.so")
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_run.cu", "emm_sens.cu", "emm_noalloc.cu")]
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("emm_host.cu", "emm_kernels.cu", "emm_tile.cu", "emm_air.cu", "emm_air_sep.cu", "emm_air_cluster.cu", "emm_run.cu", "emm_sens.cu", "emm_noalloc.cu")]
 _HDR = [os.path.join(_HERE, "csrc", f) for f in ("emm_internal.h", "emm_kernels.cuh", "emm_device.cuh")] + \
        [os.path.join(os.path.dirname(_HERE), "include", "emm.h")]
 
@@ -23,7 +23,7 @@ _GET = {"E1": 0, "E2": 1, "E3": 2, "H1": 3, "H2": 4, "H3": 5,
         "F_E1": 10, "F_E2": 11, "F_E3": 12, "F_H1": 13, "F_H2": 14, "F_H3": 15,
         "CE1": 20, "CE2": 21, "CE3": 22, "JW": 30, "DELTA": 31, "DTFT_GROUP": 32, "CHECK_N": 33, "CHECK_ACC": 34}
 _INFO = ("N1", "N2", "N3", "lo1", "lo2", "lo3", "k0", "uniform_xy", "box_lo1", "box_lo2", "box_lo3",
-         "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2", "pitch")
+         "box_hi1", "box_hi2", "box_hi3", "aux_M1", "aux_M2", "pitch", "air_cluster")
 # every symbol include/emm.h declares (tests check that the library exports all of them)
 SYMBOLS = ("emm_nugrid", "emm_fd_weights", "emm_dipole_direction", "emm_receiver_channels", "emm_grid_create", "emm_grid_destroy", "emm_grid_info", "emm_grid_coords",
            "emm_grid_fdcoef", "emm_workspace_bytes", "emm_bind_device", "emm_model_set", "emm_run", "emm_run_begin",

@@ -321,6 +321,42 @@ def test_plane_and_separable_air_routes_agree(emm, oracle):
     assert de / ne < 1e-5 and dh / nh < 1e-5
 
 
+@pytest.mark.parametrize("rd,nx,ny_extra", [(1, 36, 0), (2, 52, 9), (3, 44, 5)])
+def test_cluster_and_library_air_routes_agree(emm, oracle, rd, nx, ny_extra):
+    """Uniform x-y: the one-launch cluster route (hand-written shared-memory transforms, emm_air_cluster.cu, default) and the
+    library route (emm_grid_opts.air_route = 1: pack, 2-D cuFFT, filter, 2-D cuFFT, unpack) are the same linear map up to
+    rounding order.  Planes of several 7-smooth sizes (radix 2, 3, 4, 5 and 7 passes, rectangular, rows and columns that do
+    not divide by the cluster size), two sources in one launch.  The ghost planes the boundary writes are compared directly,
+    then every field; the oracle comparison of this route is test_fields_layered_air_uniform."""
+    w = W.cfg2(nx=nx, nz=24, dx=100.0, rd=rd, nb=8)
+    if ny_extra:                                                     # rectangular plane
+        w["y"] = np.concatenate([w["y"], w["y"][-1] + 100.0 * np.arange(1, ny_extra + 1)])
+        w["sigma_h"] = np.concatenate([w["sigma_h"], w["sigma_h"][:, -ny_extra:, :]], axis=1)
+    srcs = [((-150.0, 30.0, 950.0), (1.0, 0.2, 0.1)), ((120.0, -60.0, 930.0), (0.1, 1.0, 0.3), "M")]
+    fields, k0 = {}, None
+    for route in (0, 1):
+        g = make_grid(emm, w, air_route=route)
+        info = g.info()
+        assert (info["air_cluster"] > 0) == (route == 0), info
+        k0 = info["k0"]
+        g.run_begin(srcs, w["freqs"], w["receivers"], dict(fixed_steps=150, batched=1))
+        g.run_steps(150)
+        fields[route] = [[np.asarray(g.get(c, isrc=q), np.float64) for c in FIELDS] for q in range(2)]
+        g.run_end()
+        g.close()
+    for q in range(2):
+        for lo, hi in ((0, 3), (3, 6)):
+            n = np.sqrt(sum(np.sum(a ** 2) for a in fields[0][q][lo:hi]))
+            d = np.sqrt(sum(np.sum((a - b) ** 2) for a, b in zip(fields[0][q][lo:hi], fields[1][q][lo:hi])))
+            assert n > 0 and d / n < 1e-5, (q, lo, d / n)
+            # the ghost planes above the surface are written by the boundary alone (Ex, Ey on rd - 1 levels; Hx, Hy on rd)
+            for c in (lo, lo + 1):
+                for m in range(1, rd + (1 if lo == 3 else 0)):
+                    a, b = fields[0][q][c][k0 - m], fields[1][q][c][k0 - m]
+                    assert np.linalg.norm(b) > 0
+                    assert np.linalg.norm(a - b) < 2e-5 * np.linalg.norm(b), (q, c, m, np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
 def test_magnetic_and_mixed_sources_match_oracle(emm, oracle):
     """a magnetic dipole (injected into H at the half step), alone and batched together with
     an electric dipole; fields, accumulators and receivers against the oracle."""
