@@ -8,12 +8,12 @@
 // launch latency, not by bytes or flops.  Here:
 //
 //   CTA c of the C-CTA cluster owns rows [c*rpc, (c+1)*rpc) of the plane: loads them from the surface plane (Ex + i Ey, or
-//   Hz), transforms them along x in shared memory;                                             cluster barrier
-//   gathers its columns [c*cpc, (c+1)*cpc) from the row blocks of all CTAs through distributed shared memory (the
-//   transpose), transforms them along y: the 2-D spectrum, one column block per CTA, kept for all levels;
+//   Hz), transforms them along x in shared memory;
+//   sends every element to the CTA that owns its column [c*cpc, (c+1)*cpc) with stores into that CTA's shared memory (the
+//   transpose through distributed shared memory);                                              cluster barrier
+//   transforms its columns along y: the 2-D spectrum, one column block per CTA, kept for all levels;
 //   per ghost level: multiplies by the filter of that level (Eq. 21 for E; Eq. 17-20 with the half-cell phase factors for
-//   H), inverse transform along y;                                                            cluster barrier
-//   gathers its rows back from the column blocks of all CTAs;                                   cluster barrier
+//   H), inverse transform along y, sends every element back to the CTA that owns its row;       cluster barrier
 //   inverse transform along x, real part -> component 1, imaginary part -> component 2 of the ghost plane.
 //
 // Transforms: Stockham autosort passes of radix 8, 4, 2, 3, 5, 7 (every plane size is 7-smooth, [R1]) between two
@@ -49,7 +49,7 @@ struct ClusterArgs {
   int np1, np2;
   unsigned char rad1[kMaxPass], rad2[kMaxPass];
   FastDiv nb1[kMaxPass], st1[kMaxPass], nb2[kMaxPass], st2[kMaxPass];   // per pass: butterflies per line, sub-transform stride
-  FastDiv dM1, dM2, drpc, dcpc, drlast, dclast;   // drlast / dclast: rows / columns of the last CTA that has any
+  FastDiv dM1, dM2, drpc, dcpc;
   const float2 *tw1, *tw2;
   const float *kx, *ky;
   const float *f_in1, *f_in2;
@@ -136,10 +136,18 @@ __device__ __forceinline__ void dft(float2 (&a)[P]) {
   }
 }
 
+// The dynamic shared memory of the CTA as complex numbers.  The transform routines address it by offsets from this symbol,
+// not through pointers handed across the call: the compiler then emits shared-memory loads and stores (LDS / STS)
+// instead of generic ones.
+extern __shared__ __align__(16) float2 g_sm[];
+
 // one Stockham pass of radix P over `nlines` lines of length N = P * nb (pitch ld): sub-transform stride s, x -> y
+// (xo, yo, two: offsets into g_sm)
 template <int P>
-__device__ __forceinline__ void fft_pass(const float2 *__restrict__ x, float2 *__restrict__ y, const FastDiv nb, const FastDiv s,
-                                         int nlines, int ld, const float2 *__restrict__ tw) {
+__device__ __forceinline__ void fft_pass(unsigned xo, unsigned yo_, const FastDiv nb, const FastDiv s, int nlines, int ld, unsigned two) {
+  const float2 *__restrict__ x = g_sm + xo;
+  float2 *__restrict__ y = g_sm + yo_;
+  const float2 *__restrict__ tw = g_sm + two;
   const unsigned ntask = (unsigned)nlines * nb.d;
   for (unsigned t = threadIdx.x; t < ntask; t += kClThreads) {
     const unsigned line = fdiv(t, nb), b = t - line * nb.d;
@@ -160,13 +168,14 @@ __device__ __forceinline__ void fft_pass(const float2 *__restrict__ x, float2 *_
 // thread in every pass)
 struct PassTab { unsigned rad; FastDiv nb, st; };
 
-// all passes of a forward 1-D transform over the lines of a block, ping-pong between a and b (the last pass into `last`
-// if given); returns the buffer that holds the result
-__device__ __noinline__ float2 *fft_lines(float2 *a, float2 *b, float2 *last, int np, const PassTab *pt, int nlines, int ld,
-                                          const float2 *tw) {
-  float2 *src = a;
+// all passes of a forward 1-D transform over the lines of a block, ping-pong between the buffers at offsets a and b of
+// g_sm (the last pass into `last` unless kNone); returns the offset of the buffer that holds the result
+constexpr unsigned kNone = 0xffffffffu;
+__device__ __noinline__ unsigned fft_lines(unsigned a, unsigned b, unsigned last, int np, unsigned pt_off, int nlines, int ld, unsigned tw) {
+  const PassTab *pt = reinterpret_cast<const PassTab *>(g_sm + pt_off);
+  unsigned src = a;
   for (int i = 0; i < np; ++i) {
-    float2 *dst = (i == np - 1 && last) ? last : (src == a ? b : a);
+    const unsigned dst = (i == np - 1 && last != kNone) ? last : (src == a ? b : a);
     const PassTab p = pt[i];
     switch (p.rad) {
       case 2: fft_pass<2>(src, dst, p.nb, p.st, nlines, ld, tw); break;
@@ -187,32 +196,25 @@ __global__ void __launch_bounds__(kClThreads, 1) k_air_cluster(const __grid_cons
   const int c = (int)cluster.block_rank();
   const int src = blockIdx.x / A.C;
   const unsigned tid = threadIdx.x;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
   const int M1 = A.M1, M2 = A.M2, ld1 = A.ld1, ld2 = A.ld2, rpc = A.rpc, cpc = A.cpc;
-  float2 *tw1 = reinterpret_cast<float2 *>(smem_raw);
-  float2 *tw2 = tw1 + M1;
-  float2 *S = tw2 + M2;
-  float2 *R0 = S + cpc * ld2;
-  float2 *R1 = R0 + A.LG * rpc * ld1;
-  float2 *T0 = R1 + A.LG * rpc * ld1;
-  float2 *T1 = T0 + A.LG * cpc * ld2;
-  float2 *phx = T1 + A.LG * cpc * ld2;                     // per column of mine: i kx e^{-i kx dx/2} (H filter, Nyquist bin zeroed)
-  float2 *phy = phx + cpc;                                 // per row: the same with ky
-  float *kxs = reinterpret_cast<float *>(phy + M2);
+  // offsets into g_sm (complex numbers)
+  const unsigned oTw1 = 0, oTw2 = oTw1 + M1, oS = oTw2 + M2;
+  const unsigned oR0 = oS + cpc * ld2, oR1 = oR0 + A.LG * rpc * ld1;
+  const unsigned oT0 = oR1 + A.LG * rpc * ld1, oT1 = oT0 + A.LG * cpc * ld2;
+  const unsigned oPhx = oT1 + A.LG * cpc * ld2, oPhy = oPhx + cpc;
+  const unsigned oPt1 = oPhy + M2, oPt2 = oPt1 + kMaxPass * sizeof(PassTab) / sizeof(float2);
+  float2 *tw1 = g_sm + oTw1, *tw2 = g_sm + oTw2, *S = g_sm + oS, *R0 = g_sm + oR0, *T0 = g_sm + oT0;
+  float2 *phx = g_sm + oPhx;                               // per column of mine: i kx e^{-i kx dx/2} (H filter, Nyquist bin zeroed)
+  float2 *phy = g_sm + oPhy;                               // per row: the same with ky
+  PassTab *pt1 = reinterpret_cast<PassTab *>(g_sm + oPt1), *pt2 = reinterpret_cast<PassTab *>(g_sm + oPt2);
+  float *kxs = reinterpret_cast<float *>(g_sm + oPt2 + kMaxPass * sizeof(PassTab) / sizeof(float2));
   float *kys = kxs + cpc;
-  PassTab *pt1 = reinterpret_cast<PassTab *>(kys + M2 + ((cpc + M2) & 1));
-  PassTab *pt2 = pt1 + kMaxPass;
   const int j0 = c * rpc, nrow = max(0, min(rpc, M2 - j0));
   const int i0 = c * cpc, ncol = max(0, min(cpc, M1 - i0));
-  // the last CTA with rows / columns may hold fewer than the others; the level blocks of a CTA are packed by its own count
-  // (tested on the remainders, not as `nrow == rpc`: nvcc 12.9 folds min(rpc, x) == rpc into x <= rpc)
-  const bool full_r = M2 - j0 >= rpc, full_c = M1 - i0 >= cpc;
-  FastDiv dnrow, dncol;
-  dnrow.d = full_r ? A.drpc.d : A.drlast.d;
-  dnrow.m = full_r ? A.drpc.m : A.drlast.m;
-  dncol.d = full_c ? A.dcpc.d : A.dclast.d;
-  dncol.m = full_c ? A.dcpc.m : A.dclast.m;
 
+  // every CTA of the cluster must be running before its shared memory is written from outside: arrive now, wait just
+  // before the first remote store (the row transforms in between hide the barrier)
+  cluster.barrier_arrive();
   for (unsigned t = tid; t < (unsigned)M1; t += kClThreads) tw1[t] = A.tw1[t];
   for (unsigned t = tid; t < (unsigned)M2; t += kClThreads) {
     tw2[t] = A.tw2[t];
@@ -242,18 +244,19 @@ __global__ void __launch_bounds__(kClThreads, 1) k_air_cluster(const __grid_cons
     }
   }
   __syncthreads();
-  float2 *Rres = fft_lines(R0, R1, nullptr, A.np1, pt1, nrow, ld1, tw1);
-  cluster.sync();
-  // transpose through distributed shared memory: my columns of everybody's rows
+  const float2 *Rres = g_sm + fft_lines(oR0, oR1, kNone, A.np1, oPt1, nrow, ld1, oTw1);
+  cluster.barrier_wait();
+  // transpose through distributed shared memory: every element of my rows goes to the CTA that owns its column (stores to
+  // remote shared memory are not waited for; the cluster barrier publishes them).  T0 is idle everywhere at this point.
 #pragma unroll 4
-  for (unsigned t = tid; t < (unsigned)(ncol * M2); t += kClThreads) {
-    const unsigned j = fdiv(t, dncol), ii = t - j * ncol;
-    const unsigned owner = fdiv(j, A.drpc), jj = j - owner * rpc;
-    const float2 *rem = cluster.map_shared_rank(Rres, owner);
-    T0[ii * ld2 + j] = rem[jj * ld1 + i0 + ii];
+  for (unsigned t = tid; t < (unsigned)(nrow * M1); t += kClThreads) {
+    const unsigned jj = fdiv(t, A.dM1), n1 = t - jj * M1;
+    const unsigned owner = fdiv(n1, A.dcpc), ii = n1 - owner * cpc;
+    float2 *rem = cluster.map_shared_rank(T0, owner);
+    rem[ii * ld2 + j0 + jj] = Rres[jj * ld1 + n1];
   }
-  __syncthreads();
-  fft_lines(T0, T1, S, A.np2, pt2, ncol, ld2, tw2);                         // the 2-D spectrum of my columns, kept in S
+  cluster.sync();
+  fft_lines(oT0, oT1, oS, A.np2, oPt2, ncol, ld2, oTw2);                    // the 2-D spectrum of my columns, kept in S
 
   for (int g0 = 0; g0 < A.nlev; g0 += A.LG) {
     const int L = min(A.LG, A.nlev - g0);
@@ -274,20 +277,22 @@ __global__ void __launch_bounds__(kClThreads, 1) k_air_cluster(const __grid_cons
       }
     }
     __syncthreads();
-    float2 *Tres = fft_lines(T0, T1, nullptr, A.np2, pt2, L * ncol, ld2, tw2);
-    cluster.sync();
-    for (int l = 0; l < L; ++l) {                                           // transpose back: my rows of everybody's columns
+    const float2 *Tres = g_sm + fft_lines(oT0, oT1, kNone, A.np2, oPt2, L * ncol, ld2, oTw2);
+    // transpose back: every element of my columns goes to the CTA that owns its row; the level blocks of a CTA are packed
+    // by its own row count (the last CTA with rows may hold fewer).  R0 is idle everywhere: the forward transpose has been
+    // read before the first barrier, and a further group waits for the barrier at the end of this loop.
+    for (int l = 0; l < L; ++l) {
 #pragma unroll 4
-      for (unsigned t = tid; t < (unsigned)(nrow * M1); t += kClThreads) {
-        const unsigned n1 = fdiv(t, dnrow), jj = t - n1 * nrow;
-        const unsigned owner = fdiv(n1, A.dcpc), ii = n1 - owner * cpc;
-        const int ncol_owner = min(cpc, M1 - (int)owner * cpc);
-        const float2 *rem = cluster.map_shared_rank(Tres, owner);
-        R0[(l * nrow + jj) * ld1 + n1] = rem[(l * ncol_owner + ii) * ld2 + j0 + jj];
+      for (unsigned t = tid; t < (unsigned)(ncol * M2); t += kClThreads) {
+        const unsigned ii = fdiv(t, A.dM2), j = t - ii * M2;
+        const unsigned owner = fdiv(j, A.drpc), jj = j - owner * rpc;
+        const int nrow_owner = min(rpc, M2 - (int)owner * rpc);
+        float2 *rem = cluster.map_shared_rank(R0, owner);
+        rem[(l * nrow_owner + jj) * ld1 + i0 + ii] = Tres[(l * ncol + ii) * ld2 + j];
       }
     }
-    cluster.sync();                                                          // the column blocks may be overwritten from here on
-    float2 *Rr = fft_lines(R0, R1, nullptr, A.np1, pt1, L * nrow, ld1, tw1);
+    cluster.sync();
+    const float2 *Rr = g_sm + fft_lines(oR0, oR1, kNone, A.np1, oPt1, L * nrow, ld1, oTw1);
     for (int l = 0; l < L; ++l) {
       float *o1 = A.f_o1 + (size_t)src * A.VS + (size_t)(A.k0 - 1 - (g0 + l)) * A.PS;
       float *o2 = A.f_o2 + (size_t)src * A.VS + (size_t)(A.k0 - 1 - (g0 + l)) * A.PS;
@@ -299,7 +304,7 @@ __global__ void __launch_bounds__(kClThreads, 1) k_air_cluster(const __grid_cons
         o2[o] = -v.y;
       }
     }
-    __syncthreads();                                                         // R0 / R1 are refilled by the next group
+    if (g0 + A.LG < A.nlev) cluster.sync();                                  // the row blocks are refilled by the next group's transpose
   }
 }
 
@@ -389,8 +394,6 @@ int launch_air_cluster(emm_grid *g, const DevState &s, const DevRun &r, int is_h
   for (int q = 0, st_ = 1; q < a.np1; st_ *= a.rad1[q], ++q) { a.nb1[q] = make_fastdiv(g->M1 / a.rad1[q]); a.st1[q] = make_fastdiv(st_); }
   for (int q = 0, st_ = 1; q < a.np2; st_ *= a.rad2[q], ++q) { a.nb2[q] = make_fastdiv(g->M2 / a.rad2[q]); a.st2[q] = make_fastdiv(st_); }
   a.dM1 = make_fastdiv(g->M1); a.dM2 = make_fastdiv(g->M2); a.drpc = make_fastdiv(a.rpc); a.dcpc = make_fastdiv(a.cpc);
-  a.drlast = make_fastdiv(g->M2 % a.rpc ? g->M2 % a.rpc : a.rpc);
-  a.dclast = make_fastdiv(g->M1 % a.cpc ? g->M1 % a.cpc : a.cpc);
   a.tw1 = g->T.tw1; a.tw2 = g->T.tw2;
   a.kx = g->T.kx; a.ky = g->T.ky;
   a.f_in1 = is_h ? s.H[2] : s.E[0];
