@@ -11,7 +11,7 @@ receiver stencils and the check set: pointwise identical values, see test_conver
     python tests/golden/make_goldens.py cfg4s 1000 0 fields 500   # configs[3] on its default auxiliary plane (3125 x 3125,
                                                           # what bench.py times) with source and receivers 150 m below the
                                                           # surface and a 20 Hz wavelet (workloads.cfg4s), 1000 fixed
-                                                          # steps, field planes: ~2-3 h on 8 cores
+                                                          # steps, field planes: 92 min on 8 cores
 
 Output: tests/golden/<name>_converged[_aux<dx>].json or <name>_<n>steps[_aux<dx>].json with the inputs' SHA-256, nsteps, delta and the complex receivers.
 With `fields` also <name>_<n>steps[_aux<dx>]_fields.npz at every listed checkpoint and at the last step: the six time-domain

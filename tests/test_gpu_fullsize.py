@@ -362,12 +362,15 @@ def test_cfg5_full_size_200_steps_batched_fields_match_live_oracle(emm, oracle):
 def test_cfg4_default_aux_plane_1000_steps_fields_match_oracle_golden(emm):
     """configs[3]'s grid, model and DEFAULT auxiliary plane (3125 x 3125: the air-water boundary exactly as bench.py times
     it) with the shallow source of workloads.cfg4s, 1000 steps: by then the wave has been through the boundary for several
-    hundred steps.  Oracle values stored by `tests/golden/make_goldens.py cfg4s 1000 0 fields 500` (oracle only, ~3 h):
-    the six fields on four whole z planes (the ghost plane the boundary writes, the surface plane, the one below, the seabed
-    plane) and on the x-z slice through the source, the L2 norm of every z plane, the partial Green's functions at 441
-    receivers.  Field tolerance: north_star's 1e-5 relative L2 is stated for 200 steps; fp32 rounding accumulates like the
-    square root of the step count, so 1000 steps are given 1e-5 * sqrt(5) = 2.24e-5, per plane and per field, against
-    that field's own norm on the plane (planes on which the field is identically zero in the oracle must be zero)."""
+    hundred steps.  Oracle values stored by `tests/golden/make_goldens.py cfg4s 1000 0 fields 500` (oracle only, 92 min on
+    8 cores): the six fields on four whole z planes (the ghost plane the boundary writes, the surface plane, the one below,
+    the seabed plane) and on the x-z slice through the source, the L2 norm of every z plane, the partial Green's functions
+    at 441 receivers.  Field tolerance: north_star's 1e-5 relative L2 is stated for 200 steps; fp32 rounding accumulates
+    like the square root of the step count, so 1000 steps are given 1e-5 * sqrt(5) = 2.24e-5, per plane and per field,
+    against that field's own norm on the plane.  Planes on which the field is identically zero in the oracle must be zero;
+    a plane the wave has not reached (the seabed plane: 1e-11 of the strongest plane in the oracle after 0.29 s of
+    fictitious time, below what fp32 resolves) is held to silence, the same bound against the strongest plane.  The
+    receivers in reach of the wave (within ~500 m of the source: 5 E and 19 H channels above 1e-3 of the peak) within 1e-3."""
     path = os.path.join(HERE, "golden", "cfg4s_1000steps_fields.npz")
     if not os.path.exists(path):
         pytest.skip("tests/golden/cfg4s_1000steps_fields.npz has not been generated (make_goldens.py cfg4s 1000 0 fields 500, ~2 h of oracle time)")
@@ -383,7 +386,7 @@ def test_cfg4_default_aux_plane_1000_steps_fields_match_oracle_golden(emm):
     assert int(ns[0]) == nsteps and done
     tol = 1e-5 * np.sqrt(nsteps / 200.0)
     planes, jsl = [int(k) for k in gold["planes_k"]], int(gold["slice_j"])
-    checked = 0
+    checked, silent = 0, 0
     for c in ("E1", "E2", "E3", "H1", "H2", "H3"):
         f = g.get(c).astype(np.float64)
         assert np.all(np.isfinite(f))
@@ -396,19 +399,22 @@ def test_cfg4_default_aux_plane_1000_steps_fields_match_oracle_golden(emm):
             if nr == 0.0:
                 assert np.all(f[k] == 0.0), (c, k)
                 continue
-            assert nr > 1e-6 * ref_norms.max(), (c, k)               # the plane carries signal: the wave has reached it
+            if nr < 1e-6 * ref_norms.max():                          # the wave has not reached this plane: silence on both sides
+                assert np.linalg.norm(f[k] - ref) <= tol * ref_norms.max() and np.linalg.norm(f[k]) < 1e-6 * ref_norms.max(), (c, k)
+                silent += 1
+                continue
             e = np.linalg.norm(f[k] - ref) / nr
             checked += 1
             assert e < tol, (c, "plane", k, e)
         ref = gold["slice_" + c].astype(np.float64)
         e = np.linalg.norm(f[:, jsl, :] - ref) / np.linalg.norm(ref)
         assert e < tol, (c, "slice", e)
-    assert checked >= 20                                             # 6 fields x 4 planes, minus the components the ghost plane does not hold
+    assert checked == 16 and silent == 6        # 6 fields x (ghost, surface, sub-surface) minus Ez, Hz on the ghost plane; the seabed plane
     out, _ = g.run_end()
     ref = gold["receivers"]
-    for sl in (slice(0, 3), slice(3, 6)):
+    for sl, nmin in ((slice(0, 3), 5), (slice(3, 6), 15)):
         A, B = out[0][..., sl], ref[..., sl]
         big = np.abs(B) > 1e-3 * np.abs(B).max()
-        assert big.sum() >= 50, big.sum()
+        assert big.sum() >= nmin, big.sum()
         assert (np.abs(A - B)[big] / np.abs(B)[big]).max() < 1e-3
     g.close()
