@@ -308,11 +308,15 @@ __global__ void __launch_bounds__(kClThreads, 1) k_air_cluster(const __grid_cons
   }
 }
 
+// Radices of the passes, odd ones first: a pass with sub-transform stride s stores runs of s consecutive numbers, the first
+// pass (s = 1) stores with a stride of its radix: 3, 5 or 7 complex numbers spread over the banks, 8 would hit two of them.
 int factor7(int n, unsigned char *rad) {
   int np = 0;
-  while (n % 8 == 0) { rad[np++] = 8; n /= 8; }
-  const int ps[5] = {4, 2, 3, 5, 7};
-  for (int p : ps) while (n % p == 0 && np < kMaxPass) { rad[np++] = (unsigned char)p; n /= p; }
+  const int odd[3] = {3, 5, 7};
+  for (int p : odd) while (n % p == 0 && np < kMaxPass) { rad[np++] = (unsigned char)p; n /= p; }
+  while (n % 8 == 0 && np < kMaxPass) { rad[np++] = 8; n /= 8; }
+  const int even[2] = {4, 2};
+  for (int p : even) while (n % p == 0 && np < kMaxPass) { rad[np++] = (unsigned char)p; n /= p; }
   return n == 1 ? np : -1;
 }
 
