@@ -687,9 +687,17 @@ static void launch_update_nf(const DevGrid &dg, const DevState &s, int nf, dim3 
 // term (accumulator-free instance), 2 = the step in which it takes two (PAIR instance)
 // harg: mode 2 = history levels (earlier buffers of the ring) the closing pass takes; unused in the other modes
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st) {
-  const DevGrid &dg = g->dg;
-  const int quads = dg.P1 / 4;
-  const int nk = dg.N3 - dg.r - dg.klo;               // updated planes
+  const int quads = g->dg.P1 / 4;
+  // Split of the updated planes for the overlap with the air-water boundary (part 1 = surface, 2 = bulk, 0 = everything):
+  // the surface part is the r + 1 planes whose z stencils reach the ghost planes, one thin chunk -- it heads the chain
+  // surface update -> boundary -> surface update of the other field, so it is kept as short as it can be; the bulk is the
+  // rest, in chunks of kc planes counted from its own first plane (the kernels take the first plane from DevGrid::klo).
+  const int nk_all = g->dg.N3 - g->dg.r - g->dg.klo;  // updated planes
+  const int ks = part == 0 ? 0 : std::min(nk_all, g->dg.r + 1);
+  DevGrid dg = g->dg;
+  if (part == 2) dg.klo += ks;
+  const int nk = part == 0 ? nk_all : (part == 1 ? ks : nk_all - ks);
+  if (nk <= 0) return 0;
   // launch one instance (nf = accumulators it is compiled for) over the chunks of `part`
   auto launch = [&](int nf, int sel, bool pair = false) -> int {
     if (nf == 0 && !pair && g->tile_ok) {
@@ -698,10 +706,9 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
       tile_dims(&tx, &ty);
       const long long xy = (long long)((dg.N1 + tx - 1) / tx) * ((dg.N2 + ty - 1) / ty) * s.nsrc;
       while (kc > 4 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;        // kc <= 32 (kMaxKC of emm_tile.cu)
-      const int nall = (nk + kc - 1) / kc, nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);
-      const int chunk0 = part == 2 ? nsurf : 0, nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
-      if (nchunks <= 0) return 0;
-      const int rc = launch_tile(g, s, is_h, kc, nchunks, chunk0, sel, st);
+      if (part == 1) kc = ks;
+      const int nchunks = (nk + kc - 1) / kc;
+      const int rc = launch_tile(g, dg, s, is_h, kc, nchunks, 0, sel, st);
       if (rc) return rc;
       EMM_LAUNCH_CHECK(g, is_h ? "k_tile<H>" : "k_tile<E>");
       return 0;
@@ -719,11 +726,8 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
       const long long xy = (long long)((quads + TX - 1) / TX) * ((dg.N2 + TY - 1) / TY) * s.nsrc;
       while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 8) kc /= 2;
     }
-    const int nall = (nk + kc - 1) / kc;
-    const int nsurf = std::min(nall, (dg.r + 1 + kc - 1) / kc);        // chunks whose stencils reach the ghost planes
-    const int chunk0 = part == 2 ? nsurf : 0;
-    const int nchunks = part == 0 ? nall : (part == 1 ? nsurf : nall - nsurf);
-    if (nchunks <= 0) return 0;
+    if (part == 1) kc = ks;
+    const int nchunks = (nk + kc - 1) / kc, chunk0 = 0;
     dim3 block(TX, TY, 1), grid((quads + TX - 1) / TX, (dg.N2 + TY - 1) / TY, nchunks * s.nsrc);
     if (grid.z > 65535) return fail(EMM_EINVAL, "launch_update: too many z chunks x sources");
     if (pair) {

@@ -46,7 +46,7 @@ struct DevRun {
 int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, int harg, cudaStream_t st);
 // tile pipeline of the accumulator-free update (emm_tile.cu): descriptors for a run's field rings; one launch over z chunks
 int tile_make_maps(emm_grid *g, const DevState &s);
-int launch_tile(emm_grid *g, const DevState &s, int is_h, int kc, int nchunks, int chunk0, int sel, cudaStream_t st);
+int launch_tile(emm_grid *g, const DevGrid &dg, const DevState &s, int is_h, int kc, int nchunks, int chunk0, int sel, cudaStream_t st);
 void tile_dims(int *tx, int *ty);
 constexpr int kCheckBlocks = 148;   // blocks per (source, component) of the convergence reduction
 constexpr int kPairMaxNF = 5;       // grouped-DTFT instances exist for 1..5 frequencies (the staged, unrolled ones)

@@ -418,8 +418,8 @@ int tile_make_maps(emm_grid *g, const DevState &s) {
 }
 
 // the accumulator-free update of the z chunks [chunk0, chunk0 + nchunks) through the tile pipeline
-int launch_tile(emm_grid *g, const DevState &s, int is_h, int kc, int nchunks, int chunk0, int sel, cudaStream_t st) {
-  const DevGrid &dg = g->dg;
+// (dg: the grid's device view, with klo = first plane of the part of the grid this launch covers)
+int launch_tile(emm_grid *g, const DevGrid &dg, const DevState &s, int is_h, int kc, int nchunks, int chunk0, int sel, cudaStream_t st) {
   // which buffers of the rings the launch reads (the pointers of this launch against the ring bases)
   const float *a = is_h ? s.E[0] : s.H[0], *u = is_h ? s.H[0] : s.E[0];
   const int bufA = (int)((a - g->tile_base[is_h ? 0 : 1][0]) / g->tile_hstride), bufU = (int)((u - g->tile_base[is_h ? 1 : 0][0]) / g->tile_hstride);
