@@ -321,12 +321,13 @@ def test_plane_and_separable_air_routes_agree(emm, oracle):
     assert de / ne < 1e-5 and dh / nh < 1e-5
 
 
-@pytest.mark.parametrize("rd,nx,ny_extra", [(1, 36, 0), (2, 52, 9), (3, 44, 5)])
+@pytest.mark.parametrize("rd,nx,ny_extra", [(1, 36, 0), (2, 52, 9), (3, 44, 5), (2, 200, 0)])
 def test_cluster_and_library_air_routes_agree(emm, oracle, rd, nx, ny_extra):
     """Uniform x-y: the one-launch cluster route (hand-written shared-memory transforms, emm_air_cluster.cu, default) and the
     library route (emm_grid_opts.air_route = 1: pack, 2-D cuFFT, filter, 2-D cuFFT, unpack) are the same linear map up to
     rounding order.  Planes of several 7-smooth sizes (radix 2, 3, 4, 5 and 7 passes, rectangular, rows and columns that do
-    not divide by the cluster size), two sources in one launch.  The ghost planes the boundary writes are compared directly,
+    not divide by the cluster size; a 240 x 240 plane whose two H ghost levels do not fit shared memory together and go
+    through the kernel one after the other), two sources in one launch.  The ghost planes the boundary writes are compared directly,
     then every field; the oracle comparison of this route is test_fields_layered_air_uniform."""
     w = W.cfg2(nx=nx, nz=24, dx=100.0, rd=rd, nb=8)
     if ny_extra:                                                     # rectangular plane
