@@ -120,3 +120,8 @@ def test_error_codes_without_device(emm):
     assert rc == emm.ECUDA and b"workspace" in emm.lib().emm_last_error()
     rc = emm.lib().emm_run_steps(g._h, 1, None, None)
     assert rc == emm.EINVAL
+    # the sensitivity kernel needs a run in progress; the one-launch boundary is planned on the device, not before
+    out = np.zeros((8, 8, 8), np.complex128)
+    dp = out.ctypes.data_as(C.POINTER(C.c_double))
+    assert emm.lib().emm_sensitivity(g._h, 0, 1, 0, dp, dp) == emm.EINVAL and b"no run" in emm.lib().emm_last_error()
+    assert g.info()["air_cluster"] == 0
