@@ -1,0 +1,107 @@
+"""Semi-analytic field of a horizontal electric dipole in a horizontally layered earth (no code shared with oracle/ or
+the CUDA path): the reference the layered-model pins of the oracle are held against.
+
+Quasi-static Maxwell equations in the paper's convention (Eq. 1: e^{-i w t}, curl E = i w mu H,
+curl H = sigma E + J), unit x-directed point dipole at (0, 0, zs), z positive downward.  In the horizontal wavenumber
+domain the field splits into two scalar transmission lines along z (s = unit vector along the wavenumber, t = z x s):
+
+  TE  (E along t):  e'' - g^2 e = -i w mu j_t delta(z - zs),                    g^2 = kappa^2 - i w mu sigma
+                    whole space  e = i w mu / (2 g) * j_t * exp(-g |z - zs|);   e, e' continuous: r = (g1 - g2) / (g1 + g2)
+  TM  (E along s):  e' = -(g^2 / sigma) h,  h' = -sigma e - j_s delta(z - zs)   (h = H along t, e_z = i kappa h / sigma)
+                    whole space  e = -g / (2 sigma) * j_s * exp(-g |z - zs|);   e, h continuous: r = (Y1 - Y2) / (Y1 + Y2),
+                    Y = sigma / g (air: Y = 0, r = +1)
+
+With j_s = kx / kappa, j_t = -ky / kappa and Ex = e_s kx / kappa - e_t ky / kappa the angular integral leaves two Hankel
+transforms (r, phi = horizontal offset and azimuth of the receiver):
+
+  Ex = 1/(4 pi) int_0^inf [ (G_TM + G_TE) J0(kappa r) - cos(2 phi) (G_TM - G_TE) J2(kappa r) ] kappa d kappa
+  Ey = -1/(4 pi) sin(2 phi) int_0^inf (G_TM - G_TE) J2(kappa r) kappa d kappa
+
+G = whole-space amplitude x [primary + reflections from the stacks above and below the source layer].  Source and receiver
+sit in the same layer.  The primary part is the closed-form whole-space field (tests/helpers.py); only the reflected part
+-- smooth, decaying like exp(-kappa x distance to the nearest image) -- is integrated numerically (composite Simpson on
+a grid fine against both the decay and the Bessel oscillation)."""
+import numpy as np
+from scipy.special import jv
+
+from helpers import MU0, wholespace_dipole
+
+
+def _stack_reflection(kappa, w, sig, thick, mode):
+    """Generalised reflection coefficient seen from a layer looking into the stack sig[0], sig[1], ... (sig[0] = the
+    layer itself, thick[i] = thickness of sig[i], the last one a half-space), for the transmission-line voltage
+    (tangential E) of the mode."""
+    g = [np.sqrt(kappa ** 2 - 1j * w * MU0 * s + 0j) for s in sig]
+    Y = [gi if mode == "TE" else (s / gi) for s, gi in zip(sig, g)]
+    R = np.zeros_like(kappa, dtype=complex)
+    for i in range(len(sig) - 2, -1, -1):
+        r = (Y[i] - Y[i + 1]) / (Y[i] + Y[i + 1])
+        if i + 1 < len(sig) - 1:
+            p = R * np.exp(-2 * g[i + 1] * thick[i + 1])
+            R = (r + p) / (1 + r * p)
+        else:
+            R = r
+    return R
+
+
+def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
+    """Ex, Ey of a unit x-directed electric dipole at (0, 0, zs) at the receivers rec[n] = (x, y, z).
+    sigma[l] = conductivity of layer l (0 = air), z_top[l] = its upper boundary (z_top[0] = -inf for the top half-space,
+    given as None); the last layer is a half-space.  Source and receivers must lie in the same layer.
+    primary = "hankel" integrates the primary field numerically as well (needs z != zs): the self-check of the
+    amplitudes and of the angular integrals against the closed form."""
+    sigma = [float(s) for s in sigma]
+    rec = np.asarray(rec, dtype=float)
+    w = 2 * np.pi * f
+    tops = [(-np.inf if t is None else float(t)) for t in z_top]
+    bots = tops[1:] + [np.inf]
+    fits = [l for l in range(len(sigma)) if tops[l] <= zs <= bots[l] and np.all((rec[:, 2] >= tops[l]) & (rec[:, 2] <= bots[l]))]
+    assert fits, "source and receivers must lie in one layer"
+    L = fits[0]
+    zt, zb = tops[L], bots[L]
+    sL = sigma[L]
+    up_sig = [sigma[l] for l in range(L, -1, -1)]
+    up_thk = [bots[l] - tops[l] for l in range(L, -1, -1)]
+    dn_sig = [sigma[l] for l in range(L, len(sigma))]
+    dn_thk = [bots[l] - tops[l] for l in range(L, len(sigma))]
+    out = np.zeros((len(rec), 2), dtype=complex)
+    prim = wholespace_dipole((0.0, 0.0, zs), rec, f, sL)
+    for n, (x, y, z) in enumerate(rec):
+        r, phi = np.hypot(x, y), np.arctan2(y, x)
+        # distance to the nearest image sets the decay of the reflected part, the offset its oscillation
+        dimg = min((zs - zt) + (z - zt) if np.isfinite(zt) else np.inf, (zb - zs) + (zb - z) if np.isfinite(zb) else np.inf)
+        if primary == "hankel":
+            dimg = min(dimg, abs(z - zs))
+        kmax = 40.0 / max(dimg, 1.0)
+        dk = min(2 * np.pi / max(r, 1.0) / 40.0, kmax / 4000.0, 1.0 / max(dimg, 1.0) / 20.0)
+        nk = int(np.ceil(kmax / dk)) // 2 * 2 + 2
+        kap = np.linspace(0.0, kmax, nk + 1)
+        kap[0] = 1e-12
+        g = np.sqrt(kap ** 2 - 1j * w * MU0 * sL)
+        G = {}
+        for mode in ("TE", "TM"):
+            Ru = _stack_reflection(kap, w, up_sig, up_thk, mode) if len(up_sig) > 1 else 0.0 * kap
+            Rd = _stack_reflection(kap, w, dn_sig, dn_thk, mode) if len(dn_sig) > 1 else 0.0 * kap
+            eu = np.exp(-g * (zs - zt)) if np.isfinite(zt) else 0.0 * kap      # source -> top
+            ed = np.exp(-g * (zb - zs)) if np.isfinite(zb) else 0.0 * kap      # source -> bottom
+            d = zb - zt
+            ee = np.exp(-g * d) if np.isfinite(d) else 0.0 * kap
+            den = 1 - Ru * Rd * ee * ee
+            A = Ru * (eu + Rd * ee * ed) / den                                   # down-going wave leaving the top
+            B = Rd * (ed + Ru * ee * eu) / den                                   # up-going wave leaving the bottom
+            refl = (A * np.exp(-g * (z - zt)) if np.isfinite(zt) else 0.0) + (B * np.exp(-g * (zb - z)) if np.isfinite(zb) else 0.0)
+            if primary == "hankel":
+                refl = refl + np.exp(-g * abs(z - zs))
+            amp = 1j * w * MU0 / (2 * g) if mode == "TE" else -g / (2 * sL)
+            G[mode] = amp * refl
+        f0 = (G["TM"] + G["TE"]) * jv(0, kap * r) * kap
+        f2 = (G["TM"] - G["TE"]) * jv(2, kap * r) * kap
+        wts = np.ones(nk + 1)
+        wts[1:-1:2] = 4.0
+        wts[2:-1:2] = 2.0
+        wts *= (kap[-1] - 0.0) / nk / 3.0
+        I0, I2 = np.sum(wts * f0), np.sum(wts * f2)
+        p0 = prim[n] if primary != "hankel" else np.zeros(6)
+        out[n, 0] = p0[0] + (I0 - np.cos(2 * phi) * I2) / (4 * np.pi)
+        out[n, 1] = p0[1] - np.sin(2 * phi) * I2 / (4 * np.pi)
+    return out

@@ -218,6 +218,46 @@ def test_air_boundary_matches_explicit_air_layer(oracle, rd):
     assert e_no[2] > 0.15 and e_no[4] > 0.1 and e_no.max() > 10 * e_bc.max()
 
 
+def test_layered_marine_model_matches_semi_analytic_solution(oracle):
+    """Physical accuracy of a layered marine model with the air-water boundary (Eq. 17-21) against an independent
+    semi-analytic solution (tests/layered1d.py: TE / TM transmission lines per horizontal wavenumber, generalised
+    reflection coefficients, Hankel transforms; itself checked against the closed-form whole space in test_layered1d.py).
+    Air / 400 m of sea water (3.2 S/m) / sediment (1 S/m) with a 100 m layer of 0.2 S/m 400 m below the seabed; x-dipole
+    50 m above the seabed, off the grid nodes; receivers on the seabed in-line, broadside and oblique (Ey != 0) at 300-800 m
+    (1-2.5 skin depths of the water at 0.75 Hz); 50 m cells, rd = 2.  The oracle is within 2 % of the semi-analytic Ex and
+    Ey (measured: 0.1-0.8 %, 1.5 % at the nearest oblique receiver), while the same solution without the air (water continued
+    upward) is off by up to 34 % and without the resistive layer by up to 6 %: a wrong sign, factor or decay law in the boundary condition, or a wrong
+    effective medium at the interfaces, lands far outside the bound."""
+    from layered1d import layered_hed_exy
+    dx = 50.0
+    x = (np.arange(49) - 24) * dx
+    z = np.arange(33) * dx
+    sig = np.ones((32, 48, 48), np.float32)
+    sig[:8] = 3.2
+    sig[16:18] = 0.2
+    zs, f = 350.0, 0.75
+    offs = np.array([300.0, 450.0, 600.0, 800.0])
+    rel = np.concatenate([np.stack([offs, 0 * offs, 0 * offs + 400.0], axis=1),
+                          np.stack([0 * offs, offs, 0 * offs + 400.0], axis=1),
+                          np.stack([0.6 * offs, 0.8 * offs, 0 * offs + 400.0], axis=1)])
+    rec = rel + np.array([-25.0, 0.0, 0.0])
+    g = oracle.Grid(x, x, z, rd=2, nb=8, ne=-1, top=oracle.TOP_AIR)
+    g.model_set(sig)
+    out, _ = g.run([((-25.0, 0.0, zs), (1, 0, 0))], [f], rec, dict(fixed_steps=int(4.0 / g.info()["dt"])))
+    got = out[0, 0, :, :2]
+    layers = ([0.0, 3.2, 1.0, 0.2, 1.0], [None, 0.0, 400.0, 800.0, 900.0])
+    ref = layered_hed_exy(zs, rel, f, *layers)
+    noair = layered_hed_exy(zs, rel, f, [3.2] + layers[0][1:], layers[1])
+    nores = layered_hed_exy(zs, rel, f, [0.0, 3.2, 1.0], [None, 0.0, 400.0])
+    scale = np.abs(ref[:, :1])
+    err = (np.abs(got - ref) / scale).max()
+    assert err < 2e-2 and np.median(np.abs(got[:, 0] - ref[:, 0]) / scale[:, 0]) < 5e-3, (err, np.abs(got - ref) / scale)
+    assert np.abs(got[:8, 1]).max() < 1e-4 * np.abs(got[:8, 0]).min()          # in-line and broadside: Ey vanishes by symmetry
+    assert np.abs(got[8:, 1]).min() > 0.3 * np.abs(got[8:, 0]).min()           # oblique: Ey carries weight
+    e_air, e_res = (np.abs(noair - ref) / scale).max(), (np.abs(nores - ref) / scale).max()
+    assert e_air > 0.25 and e_res > 3 * err, (err, e_air, e_res)
+
+
 def test_auxiliary_plane_route_reduces_to_direct_route(oracle):
     """[R10]: on a grid that is uniform up to a 1 mm perturbation (which forces the interpolate-to-a-
     uniform-plane route of L288) the result equals the direct FFT route with half-cell phase factors."""
