@@ -258,6 +258,36 @@ def test_layered_marine_model_matches_semi_analytic_solution(oracle):
     assert e_air > 0.25 and e_res > 3 * err, (err, e_air, e_res)
 
 
+def test_cfg2_converged_golden_is_the_layered_earth_response():
+    """configs[1] at full size, run to convergence by the stopping rule [R9] (the stored oracle run the GPU is held to within
+    1e-3, tests/golden/cfg2_converged.json): its in-line Ex at the 54 seabed receivers beyond 300 m is the semi-analytic
+    response of air / 1000 m of sea water / sediment / 50 m resistor at 2500 m (tests/layered1d.py) to within 1.1 % at
+    0.25 Hz, 1.5 % at 0.75 Hz and 1.9 % at 1.25 Hz (second-order dispersion of 50 m cells: grows with frequency), over five
+    decades of amplitude out to 2950 m.  The resistor changes these data by up to 20 %, the air by up to 31 % at 0.25 Hz.
+    (The four receivers within 150 m of the dipole sit inside its 4-node stencil: 4 % at 150 m, no agreement at 50 m.)"""
+    import json
+    import os
+    from layered1d import layered_hed_exy
+    gold = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg2_converged.json")))
+    w = W.build("cfg2", None)
+    rec = np.asarray(w["receivers"])
+    G = np.array(gold["receivers_re"]) + 1j * np.array(gold["receivers_im"])
+    assert G.shape == (3, 60, 6) and gold["nsteps"] > 0
+    far = np.abs(rec[:, 0]) > 300.0
+    assert far.sum() == 54
+    layers = ([0.0, 3.2, 1.0, 0.02, 1.0], [None, 0.0, 1000.0, 2500.0, 2550.0])
+    for fi, (f, bound) in enumerate(zip(w["freqs"], (1.5e-2, 2.0e-2, 2.5e-2))):
+        ref = layered_hed_exy(950.0, rec, f, *layers)[:, 0]
+        rel = np.abs(G[fi, :, 0] - ref) / np.abs(ref)
+        assert rel[far].max() < bound and np.median(rel[far]) < 0.7 * bound, (f, rel[far].max(), np.median(rel[far]))
+        assert np.abs(ref[far]).min() < 1e-4 * np.abs(ref[far]).max()                  # the agreement spans the decades
+        nores = layered_hed_exy(950.0, rec, f, [0.0, 3.2, 1.0], [None, 0.0, 1000.0])[:, 0]
+        assert (np.abs(nores - ref) / np.abs(ref))[far].max() > 0.15
+    noair = layered_hed_exy(950.0, rec, w["freqs"][0], [3.2] + layers[0][1:], layers[1])[:, 0]
+    ref = layered_hed_exy(950.0, rec, w["freqs"][0], *layers)[:, 0]
+    assert (np.abs(noair - ref) / np.abs(ref))[far].max() > 0.25
+
+
 def test_auxiliary_plane_route_reduces_to_direct_route(oracle):
     """[R10]: on a grid that is uniform up to a 1 mm perturbation (which forces the interpolate-to-a-
     uniform-plane route of L288) the result equals the direct FFT route with half-cell phase factors."""
