@@ -262,8 +262,8 @@ def test_cfg2_converged_golden_is_the_layered_earth_response():
     """configs[1] at full size, run to convergence by the stopping rule [R9] (the stored oracle run the GPU is held to within
     1e-3, tests/golden/cfg2_converged.json): its in-line Ex at the 54 seabed receivers beyond 300 m is the semi-analytic
     response of air / 1000 m of sea water / sediment / 50 m resistor at 2500 m (tests/layered1d.py) to within 1.1 % at
-    0.25 Hz, 1.5 % at 0.75 Hz and 1.9 % at 1.25 Hz (second-order dispersion of 50 m cells: grows with frequency), over five
-    decades of amplitude out to 2950 m.  The resistor changes these data by up to 20 %, the air by up to 31 % at 0.25 Hz.
+    0.25 Hz, 1.5 % at 0.75 Hz and 1.9 % at 1.25 Hz (second-order dispersion of 50 m cells: grows with frequency), over three
+    and a half decades of amplitude out to 2950 m.  The resistor changes these data by up to 20 %, the air by up to 31 % at 0.25 Hz.
     (The four receivers within 150 m of the dipole sit inside its 4-node stencil: 4 % at 150 m, no agreement at 50 m.)"""
     import json
     import os
@@ -280,7 +280,7 @@ def test_cfg2_converged_golden_is_the_layered_earth_response():
         ref = layered_hed_exy(950.0, rec, f, *layers)[:, 0]
         rel = np.abs(G[fi, :, 0] - ref) / np.abs(ref)
         assert rel[far].max() < bound and np.median(rel[far]) < 0.7 * bound, (f, rel[far].max(), np.median(rel[far]))
-        assert np.abs(ref[far]).min() < 1e-4 * np.abs(ref[far]).max()                  # the agreement spans the decades
+        assert np.abs(ref[far]).min() < 1e-3 * np.abs(ref[far]).max()                  # the agreement spans the decades
         nores = layered_hed_exy(950.0, rec, f, [0.0, 3.2, 1.0], [None, 0.0, 1000.0])[:, 0]
         assert (np.abs(nores - ref) / np.abs(ref))[far].max() > 0.15
     noair = layered_hed_exy(950.0, rec, w["freqs"][0], [3.2] + layers[0][1:], layers[1])[:, 0]
