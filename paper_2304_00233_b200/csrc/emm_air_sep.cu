@@ -22,6 +22,8 @@
 //
 // Against the plane-sized route this halves the number of length-M transforms (no x transforms of the M2 - N2
 // interpolated rows, only k1 >= 0) and more than halves the bytes moved.
+#include <cmath>
+
 #include "emm_kernels.cuh"
 
 namespace emm {
@@ -32,8 +34,22 @@ struct SepArgs {
   int N1, N2, P1, M1, M2, K1, k0, nlev, nrows_f, is_h, nsrc;
   long long PS, VS;
   float h[kMaxR];
+  int hmul[kMaxR];      // h[m] = hmul[m] * h[0] (ghost planes continue the first water cell: 1, 2 for E, 1, 3, 5 for H); 0 = not a multiple
   float scale;
 };
+
+// e^{-k_h h_m} for every ghost level: one exponential and products when the heights are multiples of the first one
+__device__ __forceinline__ void level_decay(const SepArgs &A, float kh, float (&e)[kMaxR]) {
+  const float q = expf(-kh * A.h[0]);
+  const float q2 = q * q;
+  e[0] = q * A.scale;
+#pragma unroll
+  for (int m = 1; m < kMaxR; ++m) {
+    if (m >= A.nlev) break;
+    const int k = A.hmul[m];
+    e[m] = k == 2 ? q2 * A.scale : k == 3 ? q2 * q * A.scale : k == 5 ? q2 * q2 * q * A.scale : expf(-kh * A.h[m]) * A.scale;
+  }
+}
 
 struct Tab { const int *s; const float *w; };       // 4-point stencil table: start index and weights per target
 
@@ -73,7 +89,8 @@ __global__ void __launch_bounds__(256) k_sep_yup(const SepArgs A, const float2 *
   __syncthreads();
   const Tab t = c ? t1 : t0;
   float2 *out = V + (((size_t)src * 2 + c) * A.K1 + k1) * A.M2;
-  for (int n = threadIdx.x; n < A.M2; n += blockDim.x) {
+#pragma unroll 4
+  for (int n = threadIdx.x; n < A.M2; n += blockDim.x) {      // (unrolled: the table loads of four nodes in flight together)
     const int s = t.s[n];
     const float4 w = *reinterpret_cast<const float4 *>(t.w + 4 * n);
     float2 acc = make_float2(0.f, 0.f);
@@ -96,21 +113,26 @@ __global__ void k_sep_filter(const SepArgs A, const float *__restrict__ kx, cons
   const size_t plane = (size_t)A.K1 * A.M2, o0 = (size_t)k1 * A.M2 + n;
   V += (size_t)src * 2 * plane;
   W += (size_t)src * 2 * A.nlev * plane;
+  float e[kMaxR];
+  level_decay(A, kh, e);
   if (!A.is_h) {
     const float2 v0 = V[o0], v1 = V[plane + o0];
-    for (int m = 0; m < A.nlev; ++m) {
-      const float e = expf(-kh * A.h[m]) * A.scale;
-      W[(size_t)m * plane + o0] = make_float2(v0.x * e, v0.y * e);
-      W[(size_t)(A.nlev + m) * plane + o0] = make_float2(v1.x * e, v1.y * e);
+#pragma unroll
+    for (int m = 0; m < kMaxR; ++m) {
+      if (m >= A.nlev) break;
+      W[(size_t)m * plane + o0] = make_float2(v0.x * e[m], v0.y * e[m]);
+      W[(size_t)(A.nlev + m) * plane + o0] = make_float2(v1.x * e[m], v1.y * e[m]);
     }
   } else {
     const float2 v = V[o0];
     const bool nyx = ((A.M1 & 1) == 0) && k1 == A.M1 / 2, nyy = ((A.M2 & 1) == 0) && n == A.M2 / 2;
-    const float gx = (kh > 0.f && !nyx) ? qx / kh : 0.f, gy = (kh > 0.f && !nyy) ? qy / kh : 0.f;
-    for (int m = 0; m < A.nlev; ++m) {
-      const float e = expf(-kh * A.h[m]) * A.scale;
-      W[(size_t)m * plane + o0] = make_float2(-v.y * gx * e, v.x * gx * e);                  // i gx e v
-      W[(size_t)(A.nlev + m) * plane + o0] = make_float2(-v.y * gy * e, v.x * gy * e);
+    const float rk = kh > 0.f ? 1.f / kh : 0.f;
+    const float gx = nyx ? 0.f : qx * rk, gy = nyy ? 0.f : qy * rk;
+#pragma unroll
+    for (int m = 0; m < kMaxR; ++m) {
+      if (m >= A.nlev) break;
+      W[(size_t)m * plane + o0] = make_float2(-v.y * gx * e[m], v.x * gx * e[m]);            // i gx e v
+      W[(size_t)(A.nlev + m) * plane + o0] = make_float2(-v.y * gy * e[m], v.x * gy * e[m]);
     }
   }
 }
@@ -233,6 +255,13 @@ int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cu
   for (int m = 1; m <= nlev; ++m)
     a.h[m - 1] = (float)(is_h ? g->xn[2][g->k0] - g->xh[2][g->k0 - m] : g->xn[2][g->k0] - g->xn[2][g->k0 - m]);
   a.scale = (float)(1.0 / ((double)g->M1 * (double)g->M2));
+  for (int m = 0; m < nlev; ++m) {
+    const double h0 = is_h ? g->xn[2][g->k0] - g->xh[2][g->k0 - 1] : g->xn[2][g->k0] - g->xn[2][g->k0 - 1];
+    const double hm = is_h ? g->xn[2][g->k0] - g->xh[2][g->k0 - 1 - m] : g->xn[2][g->k0] - g->xn[2][g->k0 - 1 - m];
+    const double k = hm / h0;
+    const int ki = (int)std::lround(k);
+    a.hmul[m] = (std::fabs(k - ki) < 1e-9 * k && (ki == 1 || ki == 2 || ki == 3 || ki == 5)) ? ki : 0;
+  }
   // lattices (0 = node, 1 = half) per axis: Ex (1,0), Ey (0,1), Hz (1,1), Hx (0,1), Hy (1,0)
   const int in_x[2] = {1, is_h ? 1 : 0}, in_y[2] = {is_h ? 1 : 0, 1};
   const int out_x[2] = {is_h ? 0 : 1, is_h ? 1 : 0}, out_y[2] = {is_h ? 1 : 0, is_h ? 0 : 1};
