@@ -705,7 +705,7 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
       int tx, ty, kc = 16;
       tile_dims(&tx, &ty);
       const long long xy = (long long)((dg.N1 + tx - 1) / tx) * ((dg.N2 + ty - 1) / ty) * s.nsrc;
-      while (kc > 4 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;        // kc <= 32 (kMaxKC of emm_tile.cu)
+      while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;        // kc <= 32 (kMaxKC of emm_tile.cu)
       if (part == 1) kc = ks;
       const int nchunks = (nk + kc - 1) / kc;
       const int rc = launch_tile(g, dg, s, is_h, kc, nchunks, 0, sel, st);
