@@ -705,7 +705,12 @@ int launch_update(emm_grid *g, const DevState &s, int is_h, int part, int mode, 
       int tx, ty, kc = 16;
       tile_dims(&tx, &ty);
       const long long xy = (long long)((dg.N1 + tx - 1) / tx) * ((dg.N2 + ty - 1) / ty) * s.nsrc;
-      while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;        // kc <= 32 (kMaxKC of emm_tile.cu)
+      // (kc <= 32 = kMaxKC of emm_tile.cu).  Shorter chunks = more blocks and a shorter march per block, against more z-halo
+      // planes re-read per chunk: down to 8 planes while the grid holds fewer than 12 blocks per SM, below that only while it
+      // holds fewer than 6 (measured: cfg3 16 -> 8 planes 0.385 -> 0.373 ms, cfg2 8 -> 4 planes 0.144 -> 0.158 ms, cfg1 4 -> 2
+      // planes 0.0356 -> 0.0320 ms per step)
+      while (kc > 8 && xy * ((nk + kc - 1) / kc) < 148 * 12) kc /= 2;
+      while (kc > 2 && xy * ((nk + kc - 1) / kc) < 148 * 6) kc /= 2;
       if (part == 1) kc = ks;
       const int nchunks = (nk + kc - 1) / kc;
       const int rc = launch_tile(g, dg, s, is_h, kc, nchunks, 0, sel, st);
