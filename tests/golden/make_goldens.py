@@ -7,6 +7,7 @@ receiver stencils and the check set: pointwise identical values, see test_conver
 
     python tests/golden/make_goldens.py cfg2            # ~15 min on 8 cores
     python tests/golden/make_goldens.py cfg3 0 100        # configs[2] with aux_dx = 100 m, to convergence: ~50 min
+    python tests/golden/make_goldens.py cfg3 0 0          # configs[2] as it ships (auxiliary plane at 25 m), to convergence: 2.4 h
     python tests/golden/make_goldens.py cfg4 300 100      # configs[3] with aux_dx = 100 m, 300 fixed steps: ~50 min
     python tests/golden/make_goldens.py cfg4s 1000 0 fields 500   # configs[3] on its default auxiliary plane (3125 x 3125,
                                                           # what bench.py times) with source and receivers 150 m below the

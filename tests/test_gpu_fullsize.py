@@ -270,6 +270,16 @@ def test_cfg3_full_size_converged_matches_oracle_golden(emm):
                          lambda: W.cfg3(emm.emm_nugrid, aux_dx=100.0))
 
 
+def test_cfg3_full_size_converged_on_its_default_auxiliary_plane_matches_oracle_golden(emm):
+    """configs[2] exactly as it ships: default options, i.e. the auxiliary plane of the air-water boundary at the smallest
+    horizontal spacing (25 m), run to convergence; the oracle's result was stored by `make_goldens.py cfg3 0 0` (about 2.5 h
+    of oracle time on 8 cores).  Step count exact, receivers within 1e-3."""
+    path = os.path.join(HERE, "golden", "cfg3_converged.json")
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/cfg3_converged.json has not been generated (make_goldens.py cfg3 0 0, ~2.5 h of oracle time)")
+    _compare_with_golden(emm, path, lambda: W.cfg3(emm.emm_nugrid))
+
+
 def test_cfg4_full_size_300_steps_match_oracle_golden(emm):
     """configs[3] at full size (400x400x200 non-uniform cells, rd=3, five frequencies, layered background + three
     ellipsoidal resistors): the partial Green's functions after 300 fixed steps against the oracle's, stored by
