@@ -77,28 +77,38 @@ __device__ __forceinline__ float2 real_part_spectrum(const float2 *__restrict__ 
   return part == 0 ? make_float2(0.5f * (u.x + c.x), 0.5f * (u.y - c.y)) : make_float2(0.5f * (u.y + c.y), 0.5f * (c.x - u.x));
 }
 
-// One block per (k1, source, component): the real-part spectra of every lattice row at this k1 are formed once in
-// shared memory, then the block sweeps the M2 aux nodes of its column with coalesced writes.
+// One block per (group of kYupCols wavenumbers k1, source, component): the real-part spectra of every lattice row at these
+// k1 are formed once in shared memory, then the block sweeps the M2 aux nodes of its columns with coalesced writes; a thread
+// loads the stencil of an aux node once and applies it to all columns of the group (the sweep is bound by the latency of
+// those table loads, not by bytes: V stays in L2).
+constexpr int kYupCols = 4;
 __global__ void __launch_bounds__(256) k_sep_yup(const SepArgs A, const float2 *__restrict__ XT, const Tab t0, const Tab t1, float2 *__restrict__ V) {
-  extern __shared__ float2 spec[];                     // [N2]
+  extern __shared__ float2 spec[];                     // [kYupCols][N2]
   const int ncomp = A.is_h ? 1 : 2;
-  const int k1 = blockIdx.x, src = blockIdx.y / ncomp, c = blockIdx.y - src * ncomp;
+  const int kb = blockIdx.x * kYupCols, src = blockIdx.y / ncomp, c = blockIdx.y - src * ncomp;
+  const int nk = min(kYupCols, A.K1 - kb);
   const int nrows = A.nsrc * A.nrows_f, r0 = src * A.nrows_f;
-  for (int j = threadIdx.x; j < A.N2; j += blockDim.x)
-    spec[j] = A.is_h ? real_part_spectrum(XT, nrows, A.M1, k1, r0 + (j >> 1), j & 1) : real_part_spectrum(XT, nrows, A.M1, k1, r0 + j, c);
+  for (int t = threadIdx.x; t < nk * A.N2; t += blockDim.x) {
+    const int q = t / A.N2, j = t - q * A.N2;
+    spec[t] = A.is_h ? real_part_spectrum(XT, nrows, A.M1, kb + q, r0 + (j >> 1), j & 1) : real_part_spectrum(XT, nrows, A.M1, kb + q, r0 + j, c);
+  }
   __syncthreads();
   const Tab t = c ? t1 : t0;
-  float2 *out = V + (((size_t)src * 2 + c) * A.K1 + k1) * A.M2;
-#pragma unroll 4
-  for (int n = threadIdx.x; n < A.M2; n += blockDim.x) {      // (unrolled: the table loads of four nodes in flight together)
+  float2 *out = V + (((size_t)src * 2 + c) * A.K1 + kb) * A.M2;
+  for (int n = threadIdx.x; n < A.M2; n += blockDim.x) {
     const int s = t.s[n];
     const float4 w = *reinterpret_cast<const float4 *>(t.w + 4 * n);
-    float2 acc = make_float2(0.f, 0.f);
-    acc.x = fmaf(w.x, spec[s].x, acc.x); acc.y = fmaf(w.x, spec[s].y, acc.y);
-    acc.x = fmaf(w.y, spec[s + 1].x, acc.x); acc.y = fmaf(w.y, spec[s + 1].y, acc.y);
-    acc.x = fmaf(w.z, spec[s + 2].x, acc.x); acc.y = fmaf(w.z, spec[s + 2].y, acc.y);
-    acc.x = fmaf(w.w, spec[s + 3].x, acc.x); acc.y = fmaf(w.w, spec[s + 3].y, acc.y);
-    out[n] = acc;
+#pragma unroll
+    for (int q = 0; q < kYupCols; ++q) {
+      if (q >= nk) break;
+      const float2 *sp = spec + q * A.N2 + s;
+      float2 acc = make_float2(0.f, 0.f);
+      acc.x = fmaf(w.x, sp[0].x, acc.x); acc.y = fmaf(w.x, sp[0].y, acc.y);
+      acc.x = fmaf(w.y, sp[1].x, acc.x); acc.y = fmaf(w.y, sp[1].y, acc.y);
+      acc.x = fmaf(w.z, sp[2].x, acc.x); acc.y = fmaf(w.z, sp[2].y, acc.y);
+      acc.x = fmaf(w.w, sp[3].x, acc.x); acc.y = fmaf(w.w, sp[3].y, acc.y);
+      out[(size_t)q * A.M2 + n] = acc;
+    }
   }
 }
 
@@ -280,7 +290,7 @@ int launch_air_sep(emm_grid *g, const DevState &s, const DevRun &r, int is_h, cu
   k_sep_xup<<<dim3((a.M1 + 127) / 128, a.nrows_f, ns), blk, 0, st>>>(a, f_a, f_b, ta(0, in_x[0]), ta(0, in_x[1]), XR);
   EMM_SEP_CHECK(g, "k_sep_xup");
   if (cufftExecC2C(g->sp[0 + is_h], XR, XT, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (x forward) failed");
-  k_sep_yup<<<dim3(a.K1, ns * ncomp, 1), dim3(256, 1, 1), (size_t)a.N2 * sizeof(float2), st>>>(a, XT, ta(1, in_y[0]), ta(1, in_y[1]), V);
+  k_sep_yup<<<dim3((a.K1 + kYupCols - 1) / kYupCols, ns * ncomp, 1), dim3(256, 1, 1), (size_t)kYupCols * a.N2 * sizeof(float2), st>>>(a, XT, ta(1, in_y[0]), ta(1, in_y[1]), V);
   EMM_SEP_CHECK(g, "k_sep_yup");
   if (cufftExecC2C(g->sp[2 + is_h], V, V, CUFFT_FORWARD) != CUFFT_SUCCESS) return fail(EMM_ECUDA, "cufftExecC2C (y forward) failed");
   k_sep_filter<<<dim3((a.M2 + 127) / 128, a.K1, ns), blk, 0, st>>>(a, g->T.kx, g->T.ky, V, W);
