@@ -12,9 +12,11 @@
  * CUDA path under paper_2304_00233_b200/ (own header, own symbols `emmo_*`).
  *
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): see DESIGN.md section
- * "Oracle pins".  Physical accuracy of the air-water boundary on layered
- * models against a semi-analytic solver is *parity unpinned* (no such solver
- * in the container); its sign/decay are pinned by brute force and identities.
+ * "Oracle, pins and parity tolerances".  Layered models with the air-water
+ * boundary are pinned against a semi-analytic layered-earth solution
+ * (tests/layered1d.py).  Physical accuracy on the 3-D models (configs[2..4])
+ * is *parity unpinned*: no finite-element / integral-equation solver in the
+ * container; they rest on the pins of the scheme's parts.
  *
  * All functions return 0 on success and a negative EMMO_E* code otherwise;
  * emmo_last_error() gives a message.  Arrays passed in are copied; output
