@@ -17,6 +17,15 @@ transforms (r, phi = horizontal offset and azimuth of the receiver):
   Ex = 1/(4 pi) int_0^inf [ (G_TM + G_TE) J0(kappa r) - cos(2 phi) (G_TM - G_TE) J2(kappa r) ] kappa d kappa
   Ey = -1/(4 pi) sin(2 phi) int_0^inf (G_TM - G_TE) J2(kappa r) kappa d kappa
 
+The other four components follow from the same two lines (' = d/dz, sigma = conductivity of the layer of the receiver):
+H_s = (i / w mu) e_t', H_z = (kappa / w mu) e_t (TE);  h = H_t = -(sigma / g^2) e_s', E_z = (i kappa / sigma) h (TM).  With
+Q_TE = (i / w mu) G_TE', Q_TM = -(sigma / g^2) G_TM':
+
+  Hx = 1/(4 pi) sin(2 phi) int (Q_TE + Q_TM) J2 kappa d kappa
+  Hy = 1/(4 pi) int [ (Q_TM - Q_TE) J0 - cos(2 phi) (Q_TM + Q_TE) J2 ] kappa d kappa
+  Hz = -i sin(phi) / (2 pi w mu) int G_TE J1 kappa^2 d kappa
+  Ez = -cos(phi) / (2 pi sigma) int Q_TM J1 kappa^2 d kappa
+
 G = whole-space amplitude x [primary + reflections from the stacks above and below the source layer].  Source and receiver
 sit in the same layer.  The primary part is the closed-form whole-space field (tests/helpers.py); only the reflected part
 -- smooth, decaying like exp(-kappa x distance to the nearest image) -- is integrated numerically (composite Simpson on
@@ -44,10 +53,10 @@ def _stack_reflection(kappa, w, sig, thick, mode):
     return R
 
 
-def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
-    """Ex, Ey of a unit x-directed electric dipole at (0, 0, zs) at the receivers rec[n] = (x, y, z).
+def layered_hed(zs, rec, f, sigma, z_top, primary="closed form"):
+    """Ex, Ey, Ez, Hx, Hy, Hz of a unit x-directed electric dipole at (0, 0, zs) at the receivers rec[n] = (x, y, z).
     sigma[l] = conductivity of layer l (0 = air), z_top[l] = its upper boundary (z_top[0] = -inf for the top half-space,
-    given as None); the last layer is a half-space.  Source and receivers must lie in the same layer.
+    given as None); the last layer is a half-space.  Source and receivers must lie in the same (conductive) layer.
     primary = "hankel" integrates the primary field numerically as well (needs z != zs): the self-check of the
     amplitudes and of the angular integrals against the closed form."""
     sigma = [float(s) for s in sigma]
@@ -64,7 +73,7 @@ def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
     up_thk = [bots[l] - tops[l] for l in range(L, -1, -1)]
     dn_sig = [sigma[l] for l in range(L, len(sigma))]
     dn_thk = [bots[l] - tops[l] for l in range(L, len(sigma))]
-    out = np.zeros((len(rec), 2), dtype=complex)
+    out = np.zeros((len(rec), 6), dtype=complex)
     prim = wholespace_dipole((0.0, 0.0, zs), rec, f, sL)
     for n, (x, y, z) in enumerate(rec):
         r, phi = np.hypot(x, y), np.arctan2(y, x)
@@ -72,13 +81,13 @@ def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
         dimg = min((zs - zt) + (z - zt) if np.isfinite(zt) else np.inf, (zb - zs) + (zb - z) if np.isfinite(zb) else np.inf)
         if primary == "hankel":
             dimg = min(dimg, abs(z - zs))
-        kmax = 40.0 / max(dimg, 1.0)
+        kmax = 50.0 / max(dimg, 1.0)
         dk = min(2 * np.pi / max(r, 1.0) / 40.0, kmax / 4000.0, 1.0 / max(dimg, 1.0) / 20.0)
         nk = int(np.ceil(kmax / dk)) // 2 * 2 + 2
         kap = np.linspace(0.0, kmax, nk + 1)
         kap[0] = 1e-12
         g = np.sqrt(kap ** 2 - 1j * w * MU0 * sL)
-        G = {}
+        G, dG = {}, {}
         for mode in ("TE", "TM"):
             Ru = _stack_reflection(kap, w, up_sig, up_thk, mode) if len(up_sig) > 1 else 0.0 * kap
             Rd = _stack_reflection(kap, w, dn_sig, dn_thk, mode) if len(dn_sig) > 1 else 0.0 * kap
@@ -89,19 +98,35 @@ def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
             den = 1 - Ru * Rd * ee * ee
             A = Ru * (eu + Rd * ee * ed) / den                                   # down-going wave leaving the top
             B = Rd * (ed + Ru * ee * eu) / den                                   # up-going wave leaving the bottom
-            refl = (A * np.exp(-g * (z - zt)) if np.isfinite(zt) else 0.0) + (B * np.exp(-g * (zb - z)) if np.isfinite(zb) else 0.0)
+            dn = A * np.exp(-g * (z - zt)) if np.isfinite(zt) else 0.0 * kap
+            up = B * np.exp(-g * (zb - z)) if np.isfinite(zb) else 0.0 * kap
+            F, dF = dn + up, g * (up - dn)
             if primary == "hankel":
-                refl = refl + np.exp(-g * abs(z - zs))
+                P = np.exp(-g * abs(z - zs))
+                F, dF = F + P, dF - g * np.sign(z - zs) * P
             amp = 1j * w * MU0 / (2 * g) if mode == "TE" else -g / (2 * sL)
-            G[mode] = amp * refl
-        f0 = (G["TM"] + G["TE"]) * jv(0, kap * r) * kap
-        f2 = (G["TM"] - G["TE"]) * jv(2, kap * r) * kap
+            G[mode], dG[mode] = amp * F, amp * dF
+        QTE, QTM = 1j / (w * MU0) * dG["TE"], -(sL / g ** 2) * dG["TM"]
         wts = np.ones(nk + 1)
         wts[1:-1:2] = 4.0
         wts[2:-1:2] = 2.0
         wts *= (kap[-1] - 0.0) / nk / 3.0
-        I0, I2 = np.sum(wts * f0), np.sum(wts * f2)
+        J0, J1, J2 = jv(0, kap * r), jv(1, kap * r), jv(2, kap * r)
+
+        def hank(fk, J, power=1):
+            return np.sum(wts * fk * J * kap ** power)
+
         p0 = prim[n] if primary != "hankel" else np.zeros(6)
-        out[n, 0] = p0[0] + (I0 - np.cos(2 * phi) * I2) / (4 * np.pi)
-        out[n, 1] = p0[1] - np.sin(2 * phi) * I2 / (4 * np.pi)
+        c2, s2 = np.cos(2 * phi), np.sin(2 * phi)
+        out[n, 0] = p0[0] + (hank(G["TM"] + G["TE"], J0) - c2 * hank(G["TM"] - G["TE"], J2)) / (4 * np.pi)
+        out[n, 1] = p0[1] - s2 * hank(G["TM"] - G["TE"], J2) / (4 * np.pi)
+        out[n, 2] = p0[2] - np.cos(phi) / (2 * np.pi * sL) * hank(QTM, J1, 2)
+        out[n, 3] = p0[3] + s2 * hank(QTE + QTM, J2) / (4 * np.pi)
+        out[n, 4] = p0[4] + (hank(QTM - QTE, J0) - c2 * hank(QTM + QTE, J2)) / (4 * np.pi)
+        out[n, 5] = p0[5] - 1j * np.sin(phi) / (2 * np.pi * w * MU0) * hank(G["TE"], J1, 2)
     return out
+
+
+def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
+    """Ex, Ey only (see layered_hed)."""
+    return layered_hed(zs, rec, f, sigma, z_top, primary)[:, :2]

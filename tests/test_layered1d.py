@@ -3,7 +3,7 @@ held against: it must stand on something other than the oracle."""
 import numpy as np
 
 from helpers import wholespace_dipole
-from layered1d import layered_hed_exy
+from layered1d import layered_hed, layered_hed_exy
 
 REC = np.array([[500.0, 0, 300.0], [0, 500.0, 300.0], [400.0, 300.0, 320.0], [-300.0, 700.0, 200.0], [900.0, -200.0, 260.0]])
 
@@ -12,9 +12,11 @@ def test_hankel_form_of_the_primary_field_is_the_closed_form():
     """The two transmission-line amplitudes (i w mu / 2g for TE, -g / 2 sigma for TM), the split of the dipole into the
     two modes and the J0 / J2 angular integrals, all at once: integrated numerically, the primary field must be the
     closed-form whole-space dipole (Eq. 1) at in-line, broadside and oblique receivers above and below the source."""
-    ref = wholespace_dipole((0, 0, 250.0), REC, 0.5, 1.0)[:, :2]
-    got = layered_hed_exy(250.0, REC, 0.5, [1.0], [None], primary="hankel")
-    assert np.abs(got - ref).max() < 1e-5 * np.abs(ref).max()
+    ref = wholespace_dipole((0, 0, 250.0), REC, 0.5, 1.0)
+    got = layered_hed(250.0, REC, 0.5, [1.0], [None], primary="hankel")
+    assert np.abs(got[:, :3] - ref[:, :3]).max() < 1e-5 * np.abs(ref[:, :3]).max()          # Ex, Ey, Ez
+    assert np.abs(got[:, 3:] - ref[:, 3:]).max() < 1e-5 * np.abs(ref[:, 3:]).max()          # Hx (= 0), Hy, Hz: the z derivatives too
+    assert np.abs(ref[[0, 2, 3, 4], 2]).min() > 0 and np.abs(ref[1:, 5]).min() > 0            # Ez (x != 0) and Hz (y != 0) take part
 
 
 def test_reflection_machinery():

@@ -218,43 +218,63 @@ def test_air_boundary_matches_explicit_air_layer(oracle, rd):
     assert e_no[2] > 0.15 and e_no[4] > 0.1 and e_no.max() > 10 * e_bc.max()
 
 
-def test_layered_marine_model_matches_semi_analytic_solution(oracle):
-    """Physical accuracy of a layered marine model with the air-water boundary (Eq. 17-21) against an independent
-    semi-analytic solution (tests/layered1d.py: TE / TM transmission lines per horizontal wavenumber, generalised
-    reflection coefficients, Hankel transforms; itself checked against the closed-form whole space in test_layered1d.py).
-    Air / 400 m of sea water (3.2 S/m) / sediment (1 S/m) with a 100 m layer of 0.2 S/m 400 m below the seabed; x-dipole
-    50 m above the seabed, off the grid nodes; receivers on the seabed in-line, broadside and oblique (Ey != 0) at 300-800 m
-    (1-2.5 skin depths of the water at 0.75 Hz); 50 m cells, rd = 2.  The oracle is within 2 % of the semi-analytic Ex and
-    Ey (measured: 0.1-0.8 %, 1.5 % at the nearest oblique receiver), while the same solution without the air (water continued
-    upward) is off by up to 34 % and without the resistive layer by up to 6 %: a wrong sign, factor or decay law in the boundary condition, or a wrong
-    effective medium at the interfaces, lands far outside the bound."""
-    from layered1d import layered_hed_exy
+def _layered_marine_case():
+    """the model and the two receiver sets of the layered-earth pins: on the seabed (the CSEM geometry) and inside the water
+    layer, 75 m above the dipole (every component smooth there: the 4-point receiver interpolation does not cross an interface)"""
     dx = 50.0
     x = (np.arange(49) - 24) * dx
     z = np.arange(33) * dx
     sig = np.ones((32, 48, 48), np.float32)
     sig[:8] = 3.2
     sig[16:18] = 0.2
-    zs, f = 350.0, 0.75
     offs = np.array([300.0, 450.0, 600.0, 800.0])
-    rel = np.concatenate([np.stack([offs, 0 * offs, 0 * offs + 400.0], axis=1),
-                          np.stack([0 * offs, offs, 0 * offs + 400.0], axis=1),
-                          np.stack([0.6 * offs, 0.8 * offs, 0 * offs + 400.0], axis=1)])
+    one = np.concatenate([np.stack([offs, 0 * offs, 0 * offs], axis=1), np.stack([0 * offs, offs, 0 * offs], axis=1),
+                          np.stack([0.6 * offs, 0.8 * offs, 0 * offs], axis=1)])
+    rel = np.concatenate([one + [0, 0, 400.0], one + [0, 0, 275.0]])
+    layers = ([0.0, 3.2, 1.0, 0.2, 1.0], [None, 0.0, 400.0, 800.0, 900.0])
+    return x, z, sig, 350.0, 0.75, rel, layers
+
+
+def _layered_marine_check(got, rel, zs, f, layers):
+    """got: [24][6] Green's functions of a code under test; returns (max Ex / Ey error on the seabed, max error of the six
+    components in the water) after asserting the bounds of the pin"""
+    from layered1d import layered_hed
+    ref = layered_hed(zs, rel, f, *layers)
+    sE, sH = np.abs(ref[:, :3]).max(axis=1, keepdims=True), np.abs(ref[:, 3:]).max(axis=1, keepdims=True)
+    err = np.abs(got - ref) / np.concatenate([sE, sE, sE, sH, sH, sH], axis=1)
+    bed, wat = err[:12], err[12:]
+    assert bed[:, :2].max() < 2e-2 and np.median(bed[:, 0]) < 5e-3, bed[:, :2]              # Ex, Ey on the seabed
+    assert bed[:, 5].max() < 1e-2, bed[:, 5]                                                # Hz is smooth across the seabed
+    assert wat[:, :3].max() < 1.5e-2 and wat[:, 3:].max() < 3e-2, wat                       # all six inside the water layer
+    assert np.abs(got[:8, 1]).max() < 1e-4 * np.abs(got[:8, 0]).min()                       # in-line and broadside: Ey vanishes by symmetry
+    assert np.abs(got[8:12, 1]).min() > 0.3 * np.abs(got[8:12, 0]).min()                    # oblique: Ey carries weight
+    assert np.abs(ref[20:, 3]).min() > 0.05 * sH[20:].min() and np.abs(ref[16:, 5]).min() > 0.05 * sH[16:].min()   # Hx, Hz take part
+    return bed[:, :2].max(), wat.max(), ref
+
+
+def test_layered_marine_model_matches_semi_analytic_solution(oracle):
+    """Physical accuracy of a layered marine model with the air-water boundary (Eq. 17-21) against an independent
+    semi-analytic solution (tests/layered1d.py: TE / TM transmission lines per horizontal wavenumber, generalised
+    reflection coefficients, Hankel transforms; itself checked against the closed-form whole space in test_layered1d.py).
+    Air / 400 m of sea water (3.2 S/m) / sediment (1 S/m) with a 100 m layer of 0.2 S/m 400 m below the seabed; x-dipole
+    50 m above the seabed, off the grid nodes; receivers in-line, broadside and oblique at 300-800 m (1-2.5 skin depths of
+    the water at 0.75 Hz), on the seabed and inside the water layer; 50 m cells, rd = 2.  On the seabed Ex and Ey are within
+    2 % (measured: 0.1-0.8 %, 1.5 % at the nearest oblique receiver) and Hz within 1 % (0.35 %); inside the water layer ALL
+    SIX components are within 1.5 % (E: 0.1-0.7 %) / 3 % (H: 0.1-2.3 %) of the largest component of their field at the receiver.
+    (Hx, Hy and Ez on the seabed itself are not compared: their vertical derivative / value jumps with sigma there, and the
+    4-point receiver interpolation across that kink costs 5-25 % in either code -- a property of [R7], not of the time stepping.)
+    The same solution without the air (water continued upward) is off by up to 34 %, without the resistive layer by 6 %."""
+    from layered1d import layered_hed
+    x, z, sig, zs, f, rel, layers = _layered_marine_case()
     rec = rel + np.array([-25.0, 0.0, 0.0])
     g = oracle.Grid(x, x, z, rd=2, nb=8, ne=-1, top=oracle.TOP_AIR)
     g.model_set(sig)
     out, _ = g.run([((-25.0, 0.0, zs), (1, 0, 0))], [f], rec, dict(fixed_steps=int(4.0 / g.info()["dt"])))
-    got = out[0, 0, :, :2]
-    layers = ([0.0, 3.2, 1.0, 0.2, 1.0], [None, 0.0, 400.0, 800.0, 900.0])
-    ref = layered_hed_exy(zs, rel, f, *layers)
-    noair = layered_hed_exy(zs, rel, f, [3.2] + layers[0][1:], layers[1])
-    nores = layered_hed_exy(zs, rel, f, [0.0, 3.2, 1.0], [None, 0.0, 400.0])
-    scale = np.abs(ref[:, :1])
-    err = (np.abs(got - ref) / scale).max()
-    assert err < 2e-2 and np.median(np.abs(got[:, 0] - ref[:, 0]) / scale[:, 0]) < 5e-3, (err, np.abs(got - ref) / scale)
-    assert np.abs(got[:8, 1]).max() < 1e-4 * np.abs(got[:8, 0]).min()          # in-line and broadside: Ey vanishes by symmetry
-    assert np.abs(got[8:, 1]).min() > 0.3 * np.abs(got[8:, 0]).min()           # oblique: Ey carries weight
-    e_air, e_res = (np.abs(noair - ref) / scale).max(), (np.abs(nores - ref) / scale).max()
+    err, _, ref = _layered_marine_check(out[0, 0], rel, zs, f, layers)
+    noair = layered_hed(zs, rel[:12], f, [3.2] + layers[0][1:], layers[1])
+    nores = layered_hed(zs, rel[:12], f, [0.0, 3.2, 1.0], [None, 0.0, 400.0])
+    scale = np.abs(ref[:12, :1])
+    e_air, e_res = (np.abs(noair - ref[:12])[:, :2] / scale).max(), (np.abs(nores - ref[:12])[:, :2] / scale).max()
     assert e_air > 0.25 and e_res > 3 * err, (err, e_air, e_res)
 
 
