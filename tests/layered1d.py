@@ -26,6 +26,11 @@ Q_TE = (i / w mu) G_TE', Q_TM = -(sigma / g^2) G_TM':
   Hz = -i sin(phi) / (2 pi w mu) int G_TE J1 kappa^2 d kappa
   Ez = -cos(phi) / (2 pi sigma) int Q_TM J1 kappa^2 d kappa
 
+Vertical transverse isotropy (sigma_v for E_z, sigma = sigma_h for the horizontal E) only enters the TM line:
+i kappa h = sigma_v e_z turns its series impedance into kappa^2 / sigma_v - i w mu, so g_TM^2 = (sigma_h / sigma_v) kappa^2 -
+i w mu sigma_h, Y = sigma_h / g_TM, whole-space amplitude -g_TM / (2 sigma_h), h = -(sigma_h / g_TM^2) e_s', E_z = i kappa h /
+sigma_v; the TE line sees sigma_h only.
+
 G = whole-space amplitude x [primary + reflections from the stacks above and below the source layer].  Source and receiver
 sit in the same layer.  The primary part is the closed-form whole-space field (tests/helpers.py); only the reflected part
 -- smooth, decaying like exp(-kappa x distance to the nearest image) -- is integrated numerically (composite Simpson on
@@ -36,11 +41,16 @@ from scipy.special import jv
 from helpers import MU0, wholespace_dipole
 
 
-def _stack_reflection(kappa, w, sig, thick, mode):
+def _gamma(kappa, w, sh, sv, mode):
+    lam2 = 1.0 if (mode == "TE" or sh == 0.0) else sh / sv
+    return np.sqrt(lam2 * kappa ** 2 - 1j * w * MU0 * sh + 0j)
+
+
+def _stack_reflection(kappa, w, sig, sigv, thick, mode):
     """Generalised reflection coefficient seen from a layer looking into the stack sig[0], sig[1], ... (sig[0] = the
     layer itself, thick[i] = thickness of sig[i], the last one a half-space), for the transmission-line voltage
     (tangential E) of the mode."""
-    g = [np.sqrt(kappa ** 2 - 1j * w * MU0 * s + 0j) for s in sig]
+    g = [_gamma(kappa, w, s, v, mode) for s, v in zip(sig, sigv)]
     Y = [gi if mode == "TE" else (s / gi) for s, gi in zip(sig, g)]
     R = np.zeros_like(kappa, dtype=complex)
     for i in range(len(sig) - 2, -1, -1):
@@ -53,13 +63,16 @@ def _stack_reflection(kappa, w, sig, thick, mode):
     return R
 
 
-def layered_hed(zs, rec, f, sigma, z_top, primary="closed form"):
+def layered_hed(zs, rec, f, sigma, z_top, primary="closed form", sigma_v=None):
     """Ex, Ey, Ez, Hx, Hy, Hz of a unit x-directed electric dipole at (0, 0, zs) at the receivers rec[n] = (x, y, z).
     sigma[l] = conductivity of layer l (0 = air), z_top[l] = its upper boundary (z_top[0] = -inf for the top half-space,
     given as None); the last layer is a half-space.  Source and receivers must lie in the same (conductive) layer.
+    sigma_v[l]: vertical conductivity of layer l (None: isotropic); with anisotropy in the source layer the primary field has
+    no closed form here and is integrated numerically (primary = "hankel", needs z != zs).
     primary = "hankel" integrates the primary field numerically as well (needs z != zs): the self-check of the
     amplitudes and of the angular integrals against the closed form."""
     sigma = [float(s) for s in sigma]
+    sigv = [float(s) for s in (sigma if sigma_v is None else sigma_v)]
     rec = np.asarray(rec, dtype=float)
     w = 2 * np.pi * f
     tops = [(-np.inf if t is None else float(t)) for t in z_top]
@@ -68,7 +81,11 @@ def layered_hed(zs, rec, f, sigma, z_top, primary="closed form"):
     assert fits, "source and receivers must lie in one layer"
     L = fits[0]
     zt, zb = tops[L], bots[L]
-    sL = sigma[L]
+    sL, vL = sigma[L], sigv[L]
+    if vL != sL:
+        primary = "hankel"
+    up_sigv = [sigv[l] for l in range(L, -1, -1)]
+    dn_sigv = [sigv[l] for l in range(L, len(sigma))]
     up_sig = [sigma[l] for l in range(L, -1, -1)]
     up_thk = [bots[l] - tops[l] for l in range(L, -1, -1)]
     dn_sig = [sigma[l] for l in range(L, len(sigma))]
@@ -86,11 +103,11 @@ def layered_hed(zs, rec, f, sigma, z_top, primary="closed form"):
         nk = int(np.ceil(kmax / dk)) // 2 * 2 + 2
         kap = np.linspace(0.0, kmax, nk + 1)
         kap[0] = 1e-12
-        g = np.sqrt(kap ** 2 - 1j * w * MU0 * sL)
-        G, dG = {}, {}
+        G, dG, gm = {}, {}, {}
         for mode in ("TE", "TM"):
-            Ru = _stack_reflection(kap, w, up_sig, up_thk, mode) if len(up_sig) > 1 else 0.0 * kap
-            Rd = _stack_reflection(kap, w, dn_sig, dn_thk, mode) if len(dn_sig) > 1 else 0.0 * kap
+            g = gm[mode] = _gamma(kap, w, sL, vL, mode)
+            Ru = _stack_reflection(kap, w, up_sig, up_sigv, up_thk, mode) if len(up_sig) > 1 else 0.0 * kap
+            Rd = _stack_reflection(kap, w, dn_sig, dn_sigv, dn_thk, mode) if len(dn_sig) > 1 else 0.0 * kap
             eu = np.exp(-g * (zs - zt)) if np.isfinite(zt) else 0.0 * kap      # source -> top
             ed = np.exp(-g * (zb - zs)) if np.isfinite(zb) else 0.0 * kap      # source -> bottom
             d = zb - zt
@@ -106,7 +123,7 @@ def layered_hed(zs, rec, f, sigma, z_top, primary="closed form"):
                 F, dF = F + P, dF - g * np.sign(z - zs) * P
             amp = 1j * w * MU0 / (2 * g) if mode == "TE" else -g / (2 * sL)
             G[mode], dG[mode] = amp * F, amp * dF
-        QTE, QTM = 1j / (w * MU0) * dG["TE"], -(sL / g ** 2) * dG["TM"]
+        QTE, QTM = 1j / (w * MU0) * dG["TE"], -(sL / gm["TM"] ** 2) * dG["TM"]
         wts = np.ones(nk + 1)
         wts[1:-1:2] = 4.0
         wts[2:-1:2] = 2.0
@@ -120,13 +137,13 @@ def layered_hed(zs, rec, f, sigma, z_top, primary="closed form"):
         c2, s2 = np.cos(2 * phi), np.sin(2 * phi)
         out[n, 0] = p0[0] + (hank(G["TM"] + G["TE"], J0) - c2 * hank(G["TM"] - G["TE"], J2)) / (4 * np.pi)
         out[n, 1] = p0[1] - s2 * hank(G["TM"] - G["TE"], J2) / (4 * np.pi)
-        out[n, 2] = p0[2] - np.cos(phi) / (2 * np.pi * sL) * hank(QTM, J1, 2)
+        out[n, 2] = p0[2] - np.cos(phi) / (2 * np.pi * vL) * hank(QTM, J1, 2)
         out[n, 3] = p0[3] + s2 * hank(QTE + QTM, J2) / (4 * np.pi)
         out[n, 4] = p0[4] + (hank(QTM - QTE, J0) - c2 * hank(QTM + QTE, J2)) / (4 * np.pi)
         out[n, 5] = p0[5] - 1j * np.sin(phi) / (2 * np.pi * w * MU0) * hank(G["TE"], J1, 2)
     return out
 
 
-def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form"):
+def layered_hed_exy(zs, rec, f, sigma, z_top, primary="closed form", sigma_v=None):
     """Ex, Ey only (see layered_hed)."""
-    return layered_hed(zs, rec, f, sigma, z_top, primary)[:, :2]
+    return layered_hed(zs, rec, f, sigma, z_top, primary, sigma_v)[:, :2]

@@ -35,3 +35,22 @@ def test_reflection_machinery():
     assert np.abs(a - c).max() > 0.1 * np.abs(a).max()
     s = layered_hed_exy(250.0, np.array([[400.0, 100.0, 350.0]]), 0.5, [1.0, 1e9], [None, 350.0])
     assert np.abs(s).max() < 1e-3 * np.abs(wholespace_dipole((0, 0, 250.0), [[400.0, 100.0, 350.0]], 0.5, 1.0)[0, :2]).max()
+
+
+def test_vti_reduces_to_the_isotropic_solution_and_stretches_the_tm_mode():
+    """sigma_v = sigma_h is the isotropic solution; and the textbook property of a uniaxial medium: its TM part is the
+    isotropic TM part of a medium of conductivity sigma_v with the vertical axis stretched by lambda = sqrt(sigma_h / sigma_v)
+    (here through Ez, which only the TM mode feeds: Ez_vti(sigma_h, sigma_v; x, z) = Ez_iso(sigma_v; x, lambda z))."""
+    lay = ([0.0, 3.2, 1.0, 0.2, 1.0], [None, 0.0, 400.0, 800.0, 900.0])
+    rec = REC.copy()
+    rec[:, 2] = [300.0, 300.0, 320.0, 200.0, 260.0]
+    a = layered_hed(350.0, rec, 0.75, *lay)
+    b = layered_hed(350.0, rec, 0.75, *lay, sigma_v=lay[0])
+    assert np.abs(a - b).max() < 1e-9 * np.abs(a).max()
+    lam = np.sqrt(1.0 / 0.4)
+    r1 = np.array([[400.0, 0.0, 100.0], [700.0, 0.0, 160.0], [1000.0, 0.0, 60.0]])
+    r2 = r1 * np.array([1.0, 1.0, lam])
+    vti = layered_hed(0.0, r1, 1.0, [1.0], [None], sigma_v=[0.4])[:, 2]
+    iso = layered_hed(0.0, r2, 1.0, [0.4], [None], primary="hankel")[:, 2]
+    assert np.abs(vti / iso - 1).max() < 1e-4
+

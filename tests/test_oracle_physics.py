@@ -278,6 +278,48 @@ def test_layered_marine_model_matches_semi_analytic_solution(oracle):
     assert e_air > 0.25 and e_res > 3 * err, (err, e_air, e_res)
 
 
+def test_vti_models_match_semi_analytic_solution(oracle):
+    """Vertical transverse isotropy (sigma_v for Ez, L43; Eq. 26c, [R3]) against the semi-analytic solution, whose TM line
+    carries sigma_v (tests/layered1d.py), all six components, in-line / broadside / oblique receivers:
+    (1) the layered marine model with an anisotropic sediment (sigma_h = 1, sigma_v = 0.4; resistive layer 0.2 / 0.05 S/m),
+        receivers inside the (isotropic) water layer: within 1.5 % (E) / 3 % (H); measured 0.1-0.7 % / 0.1-1.6 %;
+    (2) an anisotropic whole space (sigma_h = 1, sigma_v = 0.4, CPML on six faces), receivers 300 m below the dipole at
+        600-1200 m: within 1.5 %; measured < 0.7 %.
+    The isotropic solution (sigma_v = sigma_h) is 20-80 % away in either case: sigma_h / sigma_v swapped, sigma_v ignored, or
+    the harmonic / arithmetic means of [R3] applied to the wrong conductivity would show."""
+    from layered1d import layered_hed
+    x, z, sh, zs, f, rel, layers = _layered_marine_case()
+    rel = rel[12:]
+    sv = np.where(sh == 3.2, 3.2, np.where(sh == 1.0, 0.4, 0.05)).astype(np.float32)
+    g = oracle.Grid(x, x, z, rd=2, nb=8, ne=-1, top=oracle.TOP_AIR)
+    g.model_set(sh, sv)
+    out, _ = g.run([((-25.0, 0.0, zs), (1, 0, 0))], [f], rel + np.array([-25.0, 0.0, 0.0]), dict(fixed_steps=int(4.0 / g.info()["dt"])))
+    ref = layered_hed(zs, rel, f, *layers, sigma_v=[0.0, 3.2, 0.4, 0.05, 0.4])
+    iso = layered_hed(zs, rel, f, *layers)
+
+    def errs(got, ref):
+        sE, sH = np.abs(ref[:, :3]).max(axis=1, keepdims=True), np.abs(ref[:, 3:]).max(axis=1, keepdims=True)
+        return np.abs(got - ref) / np.concatenate([sE, sE, sE, sH, sH, sH], axis=1)
+
+    e = errs(out[0, 0], ref)
+    assert e[:, :3].max() < 1.5e-2 and e[:, 3:].max() < 3e-2, e
+    assert errs(iso, ref).max() > 0.3
+    n = 40
+    xw = (np.arange(n + 1) - n // 2) * 100.0
+    src = (-50.0, 0.0, 30.0)
+    offs = np.array([600.0, 900.0, 1200.0])
+    relw = np.concatenate([np.stack([offs, 0 * offs, 0 * offs + 330.0], axis=1), np.stack([0 * offs, offs, 0 * offs + 330.0], axis=1),
+                           np.stack([0.6 * offs, 0.8 * offs, 0 * offs + 330.0], axis=1)])
+    g = oracle.Grid(xw, xw, xw, rd=2, nb=8, ne=-1, top=oracle.TOP_CPML)
+    g.model_set(np.full((n, n, n), 1.0, np.float32), np.full((n, n, n), 0.4, np.float32))
+    out, _ = g.run([(src, (1, 0, 0))], [1.0], relw + np.array([src[0], src[1], 0.0]), dict(fixed_steps=int(5.0 / g.info()["dt"])))
+    ref = layered_hed(src[2], relw, 1.0, [1.0], [None], sigma_v=[0.4])
+    iso = layered_hed(src[2], relw, 1.0, [1.0], [None], primary="hankel")
+    e = errs(out[0, 0], ref)
+    assert e.max() < 1.5e-2, e
+    assert errs(iso, ref).max() > 0.5
+
+
 def test_cfg2_converged_golden_is_the_layered_earth_response():
     """configs[1] at full size, run to convergence by the stopping rule [R9] (the stored oracle run the GPU is held to within
     1e-3, tests/golden/cfg2_converged.json): its in-line Ex at the 54 seabed receivers beyond 300 m is the semi-analytic
