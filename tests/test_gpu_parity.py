@@ -444,6 +444,20 @@ def test_layered_marine_model_matches_semi_analytic_solution_on_the_gpu(emm):
     g.close()
 
 
+def test_stretched_grid_marine_model_matches_semi_analytic_solution_on_the_gpu(emm):
+    """The separable auxiliary-plane route of the air-water boundary (non-uniform x-y, emm_air_sep.cu) against physics
+    directly: the layered marine model on a grid stretched in x, y and z, same case and bounds as the oracle's pin
+    (tests/test_oracle_physics.py::test_stretched_grid_marine_model_matches_semi_analytic_solution)."""
+    from test_oracle_physics import _stretched_marine_case, _stretched_marine_check
+    x, zb, sig, zs, f, rel, layers, shift = _stretched_marine_case()
+    g = emm.Grid(x, x, zb, rd=2, nb=8, ne=-1, top=emm.TOP_AIR)
+    g.model_set(sig)
+    assert g.info()["uniform_xy"] == 0 and g.info()["air_cluster"] == 0
+    out, _ = g.run([((shift[0], shift[1], zs), (1, 0, 0))], [f], rel + shift, dict(fixed_steps=int(4.0 / g.info()["dt"])))
+    _stretched_marine_check(out[0, 0], rel, zs, f, layers)
+    g.close()
+
+
 def test_vti_whole_space_matches_semi_analytic_solution_on_the_gpu(emm):
     """sigma_v in the CUDA path against physics directly: an anisotropic whole space (sigma_h = 1, sigma_v = 0.4 S/m, CPML
     on six faces), all six components at in-line, broadside and oblique receivers 300 m below the dipole, against the

@@ -278,6 +278,51 @@ def test_layered_marine_model_matches_semi_analytic_solution(oracle):
     assert e_air > 0.25 and e_res > 3 * err, (err, e_air, e_res)
 
 
+def _stretched_marine_case():
+    """the layered marine model on a grid stretched in x, y and z (40 m cells at the centre growing by 6 % to 136 m; 50 m
+    cells in the water, growing by 5 % below): the air-water boundary goes through the auxiliary uniform plane of [R10]"""
+    x = _stretched(22, 40.0, 1.06)
+    zb = np.concatenate((np.arange(9) * 50.0, 400.0 + np.cumsum(50.0 * 1.05 ** np.arange(24))))
+    zc = 0.5 * (zb[1:] + zb[:-1])
+    n = len(x) - 1
+    sig = np.ones((len(zc), n, n), np.float32)
+    sig[zc < 400.0] = 3.2
+    kres = np.where((zc > 800.0) & (zc < 920.0))[0]
+    sig[kres] = 0.2
+    layers = ([0.0, 3.2, 1.0, 0.2, 1.0], [None, 0.0, 400.0, float(zb[kres[0]]), float(zb[kres[-1] + 1])])
+    offs = np.array([300.0, 450.0, 600.0, 800.0])
+    one = np.concatenate([np.stack([offs, 0 * offs, 0 * offs], axis=1), np.stack([0 * offs, offs, 0 * offs], axis=1),
+                          np.stack([0.6 * offs, 0.8 * offs, 0 * offs], axis=1)])
+    rel = np.concatenate([one + [0, 0, 400.0], one + [0, 0, 275.0]])
+    return x, zb, sig, 350.0, 0.75, rel, layers, np.array([-13.0, 7.0, 0.0])
+
+
+def _stretched_marine_check(got, rel, zs, f, layers):
+    from layered1d import layered_hed
+    ref = layered_hed(zs, rel, f, *layers)
+    sE, sH = np.abs(ref[:, :3]).max(axis=1, keepdims=True), np.abs(ref[:, 3:]).max(axis=1, keepdims=True)
+    err = np.abs(got - ref) / np.concatenate([sE, sE, sE, sH, sH, sH], axis=1)
+    bed, wat = err[:12], err[12:]
+    assert bed[:, :2].max() < 2.5e-2 and bed[:, 5].max() < 1e-2, bed[:, [0, 1, 5]]
+    assert wat[:, :3].max() < 1.5e-2 and wat[:, 3:].max() < 6e-2 and np.median(wat[:, 3:]) < 5e-3, wat
+    return err
+
+
+def test_stretched_grid_marine_model_matches_semi_analytic_solution(oracle):
+    """The non-uniform x-y treatment of the air-water boundary ([R10]: interpolate to an auxiliary uniform plane, transform
+    there, interpolate back -- the route the paper names at L288 and forbids at L660, and the one configs[2..4] run through)
+    against the semi-analytic layered-earth solution: the layered marine model on a grid stretched in all three directions,
+    dipole off the nodes.  Seabed: Ex within 2.5 % (measured 0.1-2.0 %), Ey 0.5 %, Hz 0.4 %; inside the water layer all six
+    components: E within 1.5 % (0.9 %), H within 6 % with a median below 0.5 % (Hy at the two nearest in-line receivers,
+    300 and 450 m: 4.6 and 2.2 %; everything else below 0.8 %)."""
+    x, zb, sig, zs, f, rel, layers, shift = _stretched_marine_case()
+    g = oracle.Grid(x, x, zb, rd=2, nb=8, ne=-1, top=oracle.TOP_AIR)
+    g.model_set(sig)
+    assert g.info()["uniform_xy"] == 0 and g.info()["aux_M1"] > len(x)
+    out, _ = g.run([((shift[0], shift[1], zs), (1, 0, 0))], [f], rel + shift, dict(fixed_steps=int(4.0 / g.info()["dt"])))
+    _stretched_marine_check(out[0, 0], rel, zs, f, layers)
+
+
 def test_vti_models_match_semi_analytic_solution(oracle):
     """Vertical transverse isotropy (sigma_v for Ez, L43; Eq. 26c, [R3]) against the semi-analytic solution, whose TM line
     carries sigma_v (tests/layered1d.py), all six components, in-line / broadside / oblique receivers:
