@@ -426,7 +426,8 @@ def test_sensitivity_kernel_matches_oracle(emm, oracle, case):
     gb.close()
 
 
-def test_layered_marine_model_matches_semi_analytic_solution_on_the_gpu(emm):
+@pytest.mark.parametrize("rd", [2, 3])
+def test_layered_marine_model_matches_semi_analytic_solution_on_the_gpu(emm, rd):
     """The CUDA path against physics directly, no oracle in between: the layered marine model of the oracle's pin
     (tests/test_oracle_physics.py: air / 400 m of sea water / sediment with a resistive layer, dipole 50 m above the seabed,
     in-line, broadside and oblique receivers on the seabed and inside the water layer) run through the C ABI in fp32 with the
@@ -436,7 +437,7 @@ def test_layered_marine_model_matches_semi_analytic_solution_on_the_gpu(emm):
     from test_oracle_physics import _layered_marine_case, _layered_marine_check
     x, z, sig, zs, f, rel, layers = _layered_marine_case()
     rec = rel + np.array([-25.0, 0.0, 0.0])
-    g = emm.Grid(x, x, z, rd=2, nb=8, ne=-1, top=emm.TOP_AIR)
+    g = emm.Grid(x, x, z, rd=rd, nb=8, ne=-1, top=emm.TOP_AIR)
     g.model_set(sig)
     assert g.info()["air_cluster"] > 0
     out, _ = g.run([((-25.0, 0.0, zs), (1, 0, 0))], [f], rec, dict(fixed_steps=int(4.0 / g.info()["dt"])))
